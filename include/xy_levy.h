@@ -1,0 +1,67 @@
+/*
+ * xy_levy.h -- host-side Levy-graph builder and greedy colouring (C ABI, no CUDA).
+ *
+ * This is the SEEDED INPUT GENERATOR shared by the CUDA path's harness and by the tests that
+ * drive the oracle (BASELINE.json north_star, subsystem (1)).  It
+ * holds none of the Monte-Carlo arithmetic.  oracle/xy_oracle.c carries an independent,
+ * definition-level restatement (orc_levy_edges, orc_colour_smallest_last) against which the
+ * output of this library is checked bit-exactly in tests/test_builder.py.
+ *
+ * a0 (Eq. 6): N z / 2 distinct bonds on the L x L periodic lattice,
+ *    P(bond ij) ~ r_ij^-rho, r the minimum-image Euclidean distance (r_max = [L/2] sqrt 2).
+ *    Reading R1/R2: draw k = 0,1,2,... takes Philox4x32-10 counter
+ *    (k_lo, k_hi, sample, 3), key (seed_lo, seed_hi);  i = (x0 * N) >> 32;
+ *    v = (((x1 << 21) | (x2 >> 11)) + 0.5) 2^-53;  displacement d = dy L + dx in [1, N-1] is the
+ *    first index whose running sum of w_d = (r_d^2)^(-rho/2) (summed in index order, fp64)
+ *    exceeds v * total;  j = ((y_i+dy) mod L) L + (x_i+dx) mod L;  a bond already present
+ *    discards the draw.
+ * a1 (App. B.a): smallest-last ordering (remove the vertex of minimum current
+ *    degree, ties to the smallest id), greedy smallest-free colour in reverse removal order.
+ *    Then sites are renumbered colour-major ("sites with a common color are
+ *    consecutive in the array"), old (lattice) order kept inside a class; neighbour lists are
+ *    ascending in the new numbering.
+ *
+ * All arrays are HOST memory owned by the caller.  Return 0 on success, negative on error
+ * (XY_LEVY_EINVAL bad argument, XY_LEVY_ENOMEM, XY_LEVY_EDRAWS draw limit hit); the message is
+ * in xy_levy_last_error() (thread-local).  No exceptions, no aborts.
+ */
+#ifndef XY_LEVY_H
+#define XY_LEVY_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define XY_LEVY_OK 0
+#define XY_LEVY_EINVAL (-1)
+#define XY_LEVY_ENOMEM (-2)
+#define XY_LEVY_EDRAWS (-3)
+
+/* Build S samples (global sample ids sample_base .. sample_base+S-1), colour and renumber them.
+ *   row_ptr    [S][N+1]   CSR row pointers, nnz = N*z for every sample
+ *   col_idx    [S][N*z]   neighbour ids (new numbering), ascending per row
+ *   colour     [S][N]     colour of each (new) site id, non-decreasing in the id
+ *   new_to_old [S][N]     lattice id y*L+x of each new site id        (may be NULL)
+ *   n_colours  [S]        Q per sample                                 (may be NULL)
+ *   n_draws    [S]        Philox draws consumed per sample             (may be NULL)
+ * n_threads <= 0 picks the hardware concurrency; samples are built independently. */
+int xy_levy_build(int L, double rho, int z, uint64_t seed, uint32_t sample_base, int S,
+                  int n_threads, int32_t *row_ptr, int32_t *col_idx, int32_t *colour,
+                  int32_t *new_to_old, int32_t *n_colours, int64_t *n_draws);
+
+/* Smallest-last greedy colouring of any symmetric CSR graph; returns Q (>= 0) or a negative error. */
+int xy_colour_smallest_last(int N, const int32_t *row_ptr, const int32_t *col_idx,
+                            int32_t *colour /*[N]*/);
+
+/* Colour-major renumbering of any coloured CSR graph (same outputs as the per-sample arrays above). */
+int xy_renumber_colour_major(int N, const int32_t *row_ptr, const int32_t *col_idx,
+                             const int32_t *colour, int32_t *new_to_old, int32_t *row_ptr_new,
+                             int32_t *col_idx_new, int32_t *colour_new);
+
+const char *xy_levy_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,73 @@
+"""In-tree build of the two shared libraries (no pip, no JIT cache):
+
+  libxy_levy.so   host-only Levy-graph builder / colouring   (g++)
+  libxy_b200.so   the C-ABI hot-path library, sm_100a only   (nvcc -gencode arch=compute_100a,code=sm_100a)
+
+Both are rebuilt only when a source is newer than the library.  __graft_entry__.build() calls
+build_all(); the bindings call the per-library functions lazily and fail loudly if a build fails.
+"""
+import os
+import shutil
+import subprocess
+
+PKG = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(PKG)
+CSRC = os.path.join(PKG, "csrc")
+INCLUDE = os.path.join(ROOT, "include")
+
+LEVY_LIB = os.path.join(PKG, "libxy_levy.so")
+XY_LIB = os.path.join(PKG, "libxy_b200.so")
+
+NVCC_ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
+
+
+def _stale(lib, sources):
+    if not os.path.exists(lib):
+        return True
+    t = os.path.getmtime(lib)
+    return any(os.path.getmtime(s) > t for s in sources)
+
+
+def _sources(patterns):
+    out = []
+    for d, exts in patterns:
+        for f in sorted(os.listdir(d)):
+            if f.endswith(exts):
+                out.append(os.path.join(d, f))
+    return out
+
+
+def build_levy(force=False, verbose=False):
+    src = [os.path.join(CSRC, "levy_graph.cpp")]
+    deps = src + [os.path.join(INCLUDE, "xy_levy.h")]
+    if force or _stale(LEVY_LIB, deps):
+        cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-pthread", "-Wall", "-Wextra",
+               "-I", INCLUDE, *src, "-o", LEVY_LIB]
+        if verbose:
+            print(" ".join(cmd))
+        subprocess.run(cmd, check=True)
+    return LEVY_LIB
+
+
+def nvcc_path():
+    for p in (shutil.which("nvcc"), "/usr/local/cuda/bin/nvcc"):
+        if p and os.path.exists(p):
+            return p
+    raise RuntimeError("nvcc not found: the CUDA library cannot be built (there is no CPU fallback)")
+
+
+def build_xy(force=False, verbose=False, extra_flags=()):
+    src = [os.path.join(CSRC, "xy_b200.cu")]
+    deps = _sources([(CSRC, (".cu", ".cuh", ".h")), (INCLUDE, (".h",))])
+    if force or _stale(XY_LIB, deps):
+        cmd = [nvcc_path(), *NVCC_ARCH, "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC",
+               "-shared", "-Xptxas", "-v" if verbose else "-O3", "-I", INCLUDE, "-I", CSRC,
+               *extra_flags, *src, "-o", XY_LIB, "-lcudart"]
+        if verbose:
+            print(" ".join(cmd))
+        subprocess.run(cmd, check=True)
+    return XY_LIB
+
+
+def build_all(force=False, verbose=False):
+    return build_levy(force, verbose), build_xy(force, verbose)

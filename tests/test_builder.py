@@ -1,0 +1,92 @@
+"""The shared builder (libxy_levy.so) against the oracle's definition-level restatement, bit-exact
+(BASELINE.json north_star: 'integer work (graph, colouring ...) must match bit-exactly'), plus
+structure checks at the sizes only the fast builder reaches."""
+import numpy as np
+import pytest
+
+import graphs as G
+import oracle as O
+from paper_1211_3991_b200 import levy, workloads
+
+SEED = workloads.BASE_SEED
+
+
+@pytest.mark.parametrize("L,rho,z,sample", [(8, 3.5, 6, 0), (16, 3.5, 6, 0), (16, 3.5, 6, 7), (16, 0.0, 6, 1),
+                                            (12, 2.5, 4, 2), (32, 4.5, 6, 0), (8, 100.0, 4, 0), (20, 1.0, 3, 5)])
+def test_builder_matches_oracle_bit_exact(L, rho, z, sample):
+    N = L * L
+    g = levy.build(L, rho, z, SEED, S=1, sample_base=sample)
+    edges, draws = O.levy_edges(L, rho, z, SEED, sample)
+    rp, ci = O.csr_from_edges(N, edges)
+    colour, Q = O.colour_smallest_last(rp, ci)
+    n2o, rp2, ci2, c2 = O.renumber_colour_major(rp, ci, colour)
+    assert int(g.n_draws[0]) == draws and int(g.n_colours[0]) == Q
+    assert np.array_equal(g.new_to_old[0], n2o)
+    assert np.array_equal(g.row_ptr[0], rp2) and np.array_equal(g.col_idx[0], ci2) and np.array_equal(g.colour[0], c2)
+
+
+def test_builder_sample_indexing_is_global():
+    """sample s of a batch equals a batch of one built with sample_base = s (multi-GPU sharding relies on it)."""
+    g = levy.build(16, 3.5, 6, SEED, S=4, sample_base=0, n_threads=3)
+    for s in (0, 3):
+        g1 = levy.build(16, 3.5, 6, SEED, S=1, sample_base=s)
+        assert np.array_equal(g.col_idx[s], g1.col_idx[0]) and np.array_equal(g.colour[s], g1.colour[0])
+    assert not np.array_equal(g.col_idx[0], g.col_idx[1])
+
+
+def test_colouring_and_renumber_entry_points_match_oracle():
+    for N, edges in [(9, G.ring_edges(9)), (12, G.chain_edges(12)), (16, G.square_lattice_edges(4)),
+                     (6, [(0, k) for k in range(1, 6)]), (5, [])]:
+        rp, ci = G.csr_from_edges(N, edges)
+        col, Q = levy.colour_smallest_last(rp, ci)
+        col_o, Q_o = O.colour_smallest_last(rp, ci)
+        assert Q == Q_o and np.array_equal(col, col_o)
+        out = levy.renumber_colour_major(rp, ci, col)
+        ref = O.renumber_colour_major(rp, ci, col_o)
+        for a, b in zip(out, ref):
+            assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2])
+def test_config_graphs_structure(cfg):
+    w = workloads.CONFIGS[cfg]
+    S = min(w.S, 2)
+    g = levy.build(w.L, w.rho, w.z, w.seed, S=S)
+    N = w.N
+    for s in range(S):
+        rp, ci, col = g.row_ptr[s], g.col_idx[s], g.colour[s]
+        assert rp[0] == 0 and rp[-1] == N * w.z                                   # E_b = N z / 2
+        src = np.repeat(np.arange(N), np.diff(rp))
+        assert np.all(src != ci)                                                   # no self loop
+        key = src.astype(np.int64) * N + ci
+        assert len(np.unique(key)) == len(key)                                     # no duplicate
+        assert np.array_equal(np.sort(key), np.sort(ci.astype(np.int64) * N + src))  # symmetric
+        assert np.all(col[src] != col[ci])                                         # no monochromatic edge
+        assert np.all(np.diff(col) >= 0) and col.max() + 1 == g.n_colours[s] <= 7
+        old = g.new_to_old[s]
+        dx = np.abs(old[src] % w.L - old[ci] % w.L); dy = np.abs(old[src] // w.L - old[ci] // w.L)
+        dx = np.minimum(dx, w.L - dx); dy = np.minimum(dy, w.L - dy)
+        assert (dx * dx + dy * dy).max() <= 2 * (w.L // 2) ** 2                    # r_max
+        for e in range(0, len(ci), 997):                                           # rows ascending
+            pass
+        assert all(np.all(np.diff(ci[rp[i]:rp[i + 1]]) > 0) for i in range(0, N, max(1, N // 500)))
+
+
+def test_builder_errors():
+    with pytest.raises(levy.LevyError):
+        levy.build(1, 3.5, 6, SEED)
+    with pytest.raises(levy.LevyError):
+        levy.build(3, 3.5, 3, SEED)          # N*z odd
+    with pytest.raises(levy.LevyError):
+        levy.build(4, 3.5, 40, SEED)         # more bonds than pairs
+    with pytest.raises(levy.LevyError):
+        levy.build(8, 400.0, 6, SEED)        # weights beyond nearest neighbours underflow: draw limit
+
+
+def test_workload_recipes():
+    w = workloads.CONFIGS[4]
+    assert (w.L, w.R, w.S, w.rho) == (512, 64, 8, 3.0) and abs(w.bytes_per_update() - 32.375) < 1e-12
+    T = w.temperatures()
+    assert T[0] == 1.5 and abs(T[-1] - 4.0) < 1e-12 and np.allclose(T[1:] / T[:-1], (4.0 / 1.5) ** (1 / 63))
+    assert np.allclose(O.geometric_temperatures(w.R, w.T_min, w.T_max), T, rtol=1e-15)
+    assert workloads.lscan(64).L == 64 and workloads.lscan(64).R * workloads.lscan(64).S == 512
