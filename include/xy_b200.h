@@ -1,0 +1,136 @@
+/*
+ * xy_b200.h -- C ABI of the B200 (sm_100a) hot path of arXiv 1211.3991:
+ * graph-coloured Metropolis + over-relaxation sweeps of the XY model
+ *     H = - sum_<ij> cos(theta_i - theta_j)                      (Eq. 5, n = 2)
+ * on S independent graph samples (Eq. 12) x R parallel-tempering replicas
+ * (PAPER.md:460-472), with per-sweep E / m reductions (Eq. 13-16) and on-device
+ * temperature-label swaps.  Every step runs in hand-written CUDA kernels; there is no CPU fallback:
+ * without a CUDA device every call that touches the device returns XY_ECUDA.
+ *
+ * Conventions
+ *   - every function returns int: XY_OK (0) or a negative code; the message of the last failure on the
+ *     calling thread is xy_last_error().  No exceptions, no aborts.
+ *   - "host" pointers are borrowed for the duration of the call and copied; "device" pointers must stay
+ *     valid while the handle lives.  Handles are owned by the library (xy_graph_free / xy_pt_destroy).
+ *   - `stream` is a cudaStream_t passed as void* (e.g. torch.cuda.current_stream().cuda_stream);
+ *     xy_pt_create(stream = NULL) makes the library create a private non-blocking stream (CUDA graphs
+ *     cannot be captured on the legacy default stream).  All work of a handle is enqueued on its stream;
+ *     calls return without synchronising unless they hand data back to the host.
+ *   - layouts: theta[S][N][R] fp32 radians in [0, 2pi_f], replica (memory slot) fastest
+ *     (BASELINE.json north_star); labels temp_of_slot[S][R], slot_of_temp[S][R] int32, mutually inverse;
+ *     "slot" = memory lane of a replica, "temperature" = index into T[]; swaps move labels, not spins.
+ *   - site numbering must be COLOUR-MAJOR: colour[] non-decreasing in the site id (PAPER.md:490
+ *     "sites with a common color are consecutive in the array"); xy_renumber_colour_major() in
+ *     xy_levy.h produces it for any coloured graph.
+ *   - random numbers: Philox4x32-10, key = (seed_lo, seed_hi),
+ *     counter = (site, sweep, (global_sample << 16) | (slot >> 1), domain); even slot takes (x0, x1),
+ *     odd slot (x2, x3); u = ((x >> 9) + 0.5) 2^-23.  domain 0 = init, 1 = Metropolis, 2 = swap
+ *     (site = t, sweep = round, slot = 0).  global_sample = sample_base + s < 65536, R <= 131072.
+ *   - order of one PT cycle (binds this library and the oracle):
+ *       repeat sweeps_per_swap times: sweep += 1; Metropolis colours 0..Q-1; or_per_sweep x (OR colours
+ *       0..Q-1); measure+accumulate iff sweep % measure_every == 0;   then one swap round; round += 1.
+ */
+#ifndef XY_B200_H
+#define XY_B200_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define XY_OK 0
+#define XY_EINVAL (-1) /* bad argument */
+#define XY_ENOMEM (-2) /* host or device allocation failed */
+#define XY_ECUDA (-3)  /* CUDA runtime error, or no CUDA device */
+#define XY_EGRAPH (-4) /* malformed graph or improper colouring */
+#define XY_ESTATE (-5) /* call not valid in the handle's current state */
+
+#define XY_NACC 8 /* accumulator columns: n, E, E^2, |m|, m^2, m^4, Mx/N, My/N */
+
+typedef struct xy_graph xy_graph;
+typedef struct xy_pt xy_pt;
+
+const char *xy_last_error(void);
+/* ABI version of this header (bumped on any signature change). */
+int xy_abi_version(void);
+
+/* ---- graph (SURVEY.md 8(b); PAPER.md:94 J_ij in {0,1}; :452-456 colouring; :490 adjacency list) ----
+ * S samples of N sites each.  row_ptr [S][N+1] (each sample starts at 0), col_idx = the S neighbour
+ * arrays concatenated (sample s has row_ptr[s][N] entries, site ids local to the sample), colour [S][N].
+ * Validated per sample: row_ptr monotone from 0; ids in range; no self-loop; no duplicate; symmetric;
+ * colour >= 0 and non-decreasing in the site id; NO MONOCHROMATIC EDGE.  Any violation -> XY_EGRAPH.
+ * Degree-0 sites, trees, rings, 2-site graphs are all fine.  Copies everything to the device. */
+int xy_graph_load(int S, int N, const int32_t *row_ptr /*host*/, const int32_t *col_idx /*host*/,
+                  const int32_t *colour /*host*/, void *stream, xy_graph **out);
+int xy_graph_free(xy_graph *g);
+/* any output pointer may be NULL */
+int xy_graph_info(const xy_graph *g, int *S, int *N, int64_t *nnz_total, int *q_max, int *max_degree);
+
+/* ---- PT ensemble ----
+ * T [R] host, strictly positive, ascending (T = +inf allowed: beta = 0).  width [R] host or NULL;
+ * NULL selects the BASELINE.json proposal width 2 pi min(1, T/2).  beta and width are rounded to fp32
+ * per temperature for the Metropolis kernel; the swap rule uses 1/T in fp64.
+ * theta_dev: device buffer [S][N][R] fp32 owned by the caller (8-byte aligned), or NULL to let the
+ * library allocate.  Initialises theta = 2pi_f * u (Philox domain 0), identity labels, counters 0,
+ * accumulators 0.  The graph must outlive the ensemble. */
+int xy_pt_create(const xy_graph *g, int R, const double *T /*host*/, const double *width /*host|NULL*/,
+                 uint64_t seed, uint32_t sample_base, float *theta_dev /*device|NULL*/, void *stream,
+                 xy_pt **out);
+int xy_pt_destroy(xy_pt *pt);
+
+/* ---- the hot-path calls named by BASELINE.json north_star ---- */
+/* n Metropolis sweeps: colours 0..Q-1 in order, sweep counter += 1 per sweep. */
+int xy_sweep(xy_pt *pt, int n_sweeps);
+/* n over-relaxation sweeps (ref 66): no randoms, counters untouched. */
+int xy_overrelax(xy_pt *pt, int n_sweeps);
+/* one swap round (ref 65): pairs (t,t+1), t = round mod 2 (mod 2); energies are
+ * recomputed first unless still fresh; accept iff u < exp((beta_t-beta_t+1)(E_a-E_b)); round += 1. */
+int xy_pt_swap(xy_pt *pt);
+/* E, M_x, M_y of every replica (Eq. 5, Eq. 16), added to the fp64 accumulators of the replica's
+ * current temperature (Eq. 13-15).  out_host: [S][R][3] doubles (E, Mx, My) indexed by TEMPERATURE,
+ * or NULL; a non-NULL out_host synchronises the stream. */
+int xy_measure(xy_pt *pt, double *out_host);
+
+/* n_cycles PT cycles in the order stated at the top, replayed from a captured CUDA graph (SURVEY.md
+ * 8(a) row a6).  measure_every = 0 disables measurements (energies are still computed for the swap).
+ * sweeps_per_swap >= 1, or_per_sweep >= 0. */
+int xy_run(xy_pt *pt, int n_cycles, int sweeps_per_swap, int or_per_sweep, int measure_every);
+
+/* Samples are independent, so a cycle may be executed for groups of `samples_per_group` samples at a
+ * time (all sweeps of the cycle for group 0, then group 1, ...) to keep a group L2-resident; results
+ * are bit-identical for every value.  0 = automatic (default), S = all samples per launch. */
+int xy_set_schedule(xy_pt *pt, int samples_per_group);
+
+/* ---- single-colour steps (lockstep parity tests) ----
+ * Metropolis on colour class `colour` of every sample with Philox sweep index `sweep` (the handle's
+ * sweep counter is not touched); OR on one colour class. */
+int xy_metropolis_colour(xy_pt *pt, int colour, uint32_t sweep);
+int xy_overrelax_colour(xy_pt *pt, int colour);
+
+/* ---- state access (all synchronise the stream) ---- */
+int xy_get_theta(xy_pt *pt, float *theta_host /*[S][N][R]*/);
+int xy_set_theta(xy_pt *pt, const float *theta_host /*[S][N][R]*/);
+int xy_get_labels(xy_pt *pt, int32_t *temp_of_slot_host /*[S][R]*/);
+int xy_set_labels(xy_pt *pt, const int32_t *temp_of_slot_host /*[S][R], a permutation per sample*/);
+/* energies per memory slot [S][R] (recomputed if stale; accumulators untouched) */
+int xy_get_energy(xy_pt *pt, double *E_slot_host);
+/* one swap round with the caller's decisions: accept[S][R], entry [s][t] is used for pair (t,t+1) of the
+ * round's parity.  Bit-exact permutation test; round += 1. */
+int xy_swap_with_decisions(xy_pt *pt, const uint8_t *accept_host);
+/* accumulators [S][R][XY_NACC] indexed by temperature */
+int xy_read_accumulators(xy_pt *pt, double *acc_host);
+int xy_reset_accumulators(xy_pt *pt);
+/* sweep / round counters and per-pair swap statistics [S][R] (entry t = pair (t,t+1)); NULLs allowed */
+int xy_get_counters(xy_pt *pt, uint32_t *sweep, uint32_t *round, int64_t *swap_attempts_host,
+                    int64_t *swap_accepts_host);
+int xy_set_counters(xy_pt *pt, uint32_t sweep, uint32_t round);
+/* device pointer of theta (caller's or the library's) */
+int xy_theta_device(xy_pt *pt, float **theta_dev);
+/* number of kernel launches (graph kernel nodes included) issued by this handle so far */
+int xy_launch_count(xy_pt *pt, int64_t *n_launches);
+int xy_synchronize(xy_pt *pt);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,298 @@
+"""Thin Python binding of the C ABI in include/xy_b200.h: same names, argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind libxy_b200.so.  PyTorch is used for device
+memory (the theta tensor) and the CUDA stream, nothing else.  There is no CPU fallback: if the library
+cannot be built or loaded, or no CUDA device is present, the calls raise.
+"""
+import ctypes as C
+
+import numpy as np
+
+from . import _build
+
+XY_OK, XY_EINVAL, XY_ENOMEM, XY_ECUDA, XY_EGRAPH, XY_ESTATE = 0, -1, -2, -3, -4, -5
+XY_NACC = 8
+_CODES = {XY_EINVAL: "XY_EINVAL", XY_ENOMEM: "XY_ENOMEM", XY_ECUDA: "XY_ECUDA", XY_EGRAPH: "XY_EGRAPH",
+          XY_ESTATE: "XY_ESTATE"}
+
+# every symbol include/xy_b200.h declares (tests/test_abi_symbols.py checks the header against this list)
+SYMBOLS = {
+    "xy_last_error": (C.c_char_p, []),
+    "xy_abi_version": (C.c_int, []),
+    "xy_graph_load": (C.c_int, [C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p)]),
+    "xy_graph_free": (C.c_int, [C.c_void_p]),
+    "xy_graph_info": (C.c_int, [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int64),
+                                C.POINTER(C.c_int), C.POINTER(C.c_int)]),
+    "xy_pt_create": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_void_p,
+                               C.c_void_p, C.POINTER(C.c_void_p)]),
+    "xy_pt_destroy": (C.c_int, [C.c_void_p]),
+    "xy_sweep": (C.c_int, [C.c_void_p, C.c_int]),
+    "xy_overrelax": (C.c_int, [C.c_void_p, C.c_int]),
+    "xy_pt_swap": (C.c_int, [C.c_void_p]),
+    "xy_measure": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "xy_run": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]),
+    "xy_set_schedule": (C.c_int, [C.c_void_p, C.c_int]),
+    "xy_metropolis_colour": (C.c_int, [C.c_void_p, C.c_int, C.c_uint32]),
+    "xy_overrelax_colour": (C.c_int, [C.c_void_p, C.c_int]),
+    "xy_get_theta": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "xy_set_theta": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "xy_get_labels": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "xy_set_labels": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "xy_get_energy": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "xy_swap_with_decisions": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "xy_read_accumulators": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "xy_reset_accumulators": (C.c_int, [C.c_void_p]),
+    "xy_get_counters": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.c_void_p, C.c_void_p]),
+    "xy_set_counters": (C.c_int, [C.c_void_p, C.c_uint32, C.c_uint32]),
+    "xy_theta_device": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p)]),
+    "xy_launch_count": (C.c_int, [C.c_void_p, C.POINTER(C.c_int64)]),
+    "xy_synchronize": (C.c_int, [C.c_void_p]),
+}
+
+_lib = None
+
+
+class XYError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"{_CODES.get(code, code)}: {msg}")
+        self.code = code
+
+
+def lib():
+    """Load (building if stale) libxy_b200.so.  Raises if nvcc or the build fails: there is no fallback."""
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build.build_xy())
+        for name, (res, args) in SYMBOLS.items():
+            f = getattr(L, name)
+            f.restype, f.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != XY_OK:
+        raise XYError(rc, lib().xy_last_error().decode())
+
+
+def _host(a, dtype):
+    a = np.ascontiguousarray(a, dtype)
+    return a, a.ctypes.data_as(C.c_void_p)
+
+
+def xy_last_error():
+    return lib().xy_last_error().decode()
+
+
+def xy_abi_version():
+    return lib().xy_abi_version()
+
+
+def xy_graph_load(row_ptr, col_idx, colour, stream=None):
+    """row_ptr [S][N+1], col_idx [S][nnz] (or concatenated 1-D), colour [S][N] host int32 -> graph handle."""
+    row_ptr = np.ascontiguousarray(row_ptr, np.int32)
+    colour = np.ascontiguousarray(colour, np.int32)
+    if row_ptr.ndim == 1:
+        row_ptr, colour = row_ptr[None, :], colour.reshape(1, -1)
+    S, N = colour.shape
+    col = np.ascontiguousarray(col_idx, np.int32).reshape(-1)
+    out = C.c_void_p()
+    _check(lib().xy_graph_load(S, N, row_ptr.ctypes.data_as(C.c_void_p),
+                               col.ctypes.data_as(C.c_void_p) if col.size else None,
+                               colour.ctypes.data_as(C.c_void_p), stream, C.byref(out)))
+    return out
+
+
+def xy_graph_free(g):
+    _check(lib().xy_graph_free(g))
+
+
+def xy_graph_info(g):
+    S, N, q, d = C.c_int(), C.c_int(), C.c_int(), C.c_int()
+    nnz = C.c_int64()
+    _check(lib().xy_graph_info(g, C.byref(S), C.byref(N), C.byref(nnz), C.byref(q), C.byref(d)))
+    return dict(S=S.value, N=N.value, nnz_total=nnz.value, q_max=q.value, max_degree=d.value)
+
+
+def xy_pt_create(g, T, seed, width=None, sample_base=0, theta_dev=None, stream=None):
+    """theta_dev: device address (int) of a caller-owned [S][N][R] fp32 buffer, e.g. tensor.data_ptr()."""
+    T, Tp = _host(T, np.float64)
+    wp = None
+    if width is not None:
+        width, wp = _host(width, np.float64)
+    out = C.c_void_p()
+    _check(lib().xy_pt_create(g, len(T), Tp, wp, seed, sample_base, theta_dev, stream, C.byref(out)))
+    return out
+
+
+def xy_pt_destroy(pt):
+    _check(lib().xy_pt_destroy(pt))
+
+
+def xy_sweep(pt, n_sweeps=1):
+    _check(lib().xy_sweep(pt, n_sweeps))
+
+
+def xy_overrelax(pt, n_sweeps=1):
+    _check(lib().xy_overrelax(pt, n_sweeps))
+
+
+def xy_pt_swap(pt):
+    _check(lib().xy_pt_swap(pt))
+
+
+def xy_measure(pt, shape=None):
+    """shape = (S, R) to get this measurement back as a host array [S][R][3] (E, Mx, My) by temperature."""
+    if shape is None:
+        _check(lib().xy_measure(pt, None))
+        return None
+    out = np.zeros((*shape, 3), np.float64)
+    _check(lib().xy_measure(pt, out.ctypes.data_as(C.c_void_p)))
+    return out
+
+
+def xy_run(pt, n_cycles, sweeps_per_swap=10, or_per_sweep=1, measure_every=1):
+    _check(lib().xy_run(pt, n_cycles, sweeps_per_swap, or_per_sweep, measure_every))
+
+
+def xy_set_schedule(pt, samples_per_group):
+    _check(lib().xy_set_schedule(pt, samples_per_group))
+
+
+def xy_metropolis_colour(pt, colour, sweep):
+    _check(lib().xy_metropolis_colour(pt, colour, sweep))
+
+
+def xy_overrelax_colour(pt, colour):
+    _check(lib().xy_overrelax_colour(pt, colour))
+
+
+def xy_get_theta(pt, shape, out=None):
+    out = np.empty(shape, np.float32) if out is None else out
+    _check(lib().xy_get_theta(pt, out.ctypes.data_as(C.c_void_p)))
+    return out
+
+
+def xy_set_theta(pt, theta):
+    theta, p = _host(theta, np.float32)
+    _check(lib().xy_set_theta(pt, p))
+
+
+def xy_get_labels(pt, shape):
+    out = np.empty(shape, np.int32)
+    _check(lib().xy_get_labels(pt, out.ctypes.data_as(C.c_void_p)))
+    return out
+
+
+def xy_set_labels(pt, temp_of_slot):
+    a, p = _host(temp_of_slot, np.int32)
+    _check(lib().xy_set_labels(pt, p))
+
+
+def xy_get_energy(pt, shape):
+    out = np.empty(shape, np.float64)
+    _check(lib().xy_get_energy(pt, out.ctypes.data_as(C.c_void_p)))
+    return out
+
+
+def xy_swap_with_decisions(pt, accept):
+    a, p = _host(accept, np.uint8)
+    _check(lib().xy_swap_with_decisions(pt, p))
+
+
+def xy_read_accumulators(pt, shape):
+    out = np.empty((*shape, XY_NACC), np.float64)
+    _check(lib().xy_read_accumulators(pt, out.ctypes.data_as(C.c_void_p)))
+    return out
+
+
+def xy_reset_accumulators(pt):
+    _check(lib().xy_reset_accumulators(pt))
+
+
+def xy_get_counters(pt, shape):
+    sw, rd = C.c_uint32(), C.c_uint32()
+    att = np.empty(shape, np.int64)
+    acc = np.empty(shape, np.int64)
+    _check(lib().xy_get_counters(pt, C.byref(sw), C.byref(rd), att.ctypes.data_as(C.c_void_p),
+                                 acc.ctypes.data_as(C.c_void_p)))
+    return sw.value, rd.value, att, acc
+
+
+def xy_set_counters(pt, sweep, round_):
+    _check(lib().xy_set_counters(pt, sweep, round_))
+
+
+def xy_theta_device(pt):
+    p = C.c_void_p()
+    _check(lib().xy_theta_device(pt, C.byref(p)))
+    return p.value
+
+
+def xy_launch_count(pt):
+    n = C.c_int64()
+    _check(lib().xy_launch_count(pt, C.byref(n)))
+    return n.value
+
+
+def xy_synchronize(pt):
+    _check(lib().xy_synchronize(pt))
+
+
+class Ensemble:
+    """Convenience owner of one graph + PT handle; theta lives in a torch tensor on its own torch stream.
+    Still marshalling only: every method forwards to the xy_* call of the same name."""
+
+    def __init__(self, row_ptr, col_idx, colour, T, seed, width=None, sample_base=0, device="cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise XYError(XY_ECUDA, "no CUDA device: this library has no CPU fallback")
+        self.torch = torch
+        self.device = torch.device(device)
+        colour = np.ascontiguousarray(colour, np.int32)
+        if colour.ndim == 1:
+            colour = colour[None, :]
+        self.S, self.N = colour.shape
+        self.T = np.ascontiguousarray(T, np.float64)
+        self.R = len(self.T)
+        with torch.cuda.device(self.device):
+            self.stream = torch.cuda.Stream()
+            self.theta = torch.empty((self.S, self.N, self.R), dtype=torch.float32, device=self.device)
+            self.graph = xy_graph_load(row_ptr, col_idx, colour, self.stream.cuda_stream)
+            self.pt = xy_pt_create(self.graph, self.T, seed, width, sample_base, self.theta.data_ptr(),
+                                   self.stream.cuda_stream)
+
+    def close(self):
+        if getattr(self, "pt", None) is not None:
+            xy_pt_destroy(self.pt)
+            xy_graph_free(self.graph)
+            self.pt = self.graph = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # forwarding
+    def sweep(self, n=1): xy_sweep(self.pt, n)
+    def overrelax(self, n=1): xy_overrelax(self.pt, n)
+    def pt_swap(self): xy_pt_swap(self.pt)
+    def measure(self, want=False): return xy_measure(self.pt, (self.S, self.R) if want else None)
+    def run(self, n_cycles, sweeps_per_swap=10, or_per_sweep=1, measure_every=1):
+        xy_run(self.pt, n_cycles, sweeps_per_swap, or_per_sweep, measure_every)
+    def set_schedule(self, g): xy_set_schedule(self.pt, g)
+    def metropolis_colour(self, c, sweep): xy_metropolis_colour(self.pt, c, sweep)
+    def overrelax_colour(self, c): xy_overrelax_colour(self.pt, c)
+    def get_theta(self, out=None): return xy_get_theta(self.pt, (self.S, self.N, self.R), out)
+    def set_theta(self, th): xy_set_theta(self.pt, th)
+    def get_labels(self): return xy_get_labels(self.pt, (self.S, self.R))
+    def set_labels(self, lab): xy_set_labels(self.pt, lab)
+    def get_energy(self): return xy_get_energy(self.pt, (self.S, self.R))
+    def swap_with_decisions(self, acc): xy_swap_with_decisions(self.pt, acc)
+    def read_accumulators(self): return xy_read_accumulators(self.pt, (self.S, self.R))
+    def reset_accumulators(self): xy_reset_accumulators(self.pt)
+    def get_counters(self): return xy_get_counters(self.pt, (self.S, self.R))
+    def set_counters(self, sweep, round_): xy_set_counters(self.pt, sweep, round_)
+    def launch_count(self): return xy_launch_count(self.pt)
+    def synchronize(self): xy_synchronize(self.pt)

@@ -2,7 +2,7 @@
 //
 // Seeded input generator for both the CUDA path and the oracle-driven tests.  Fast data structures
 // (CDF table + binary search, open-addressing edge set, ordered-set smallest-last queue); the
-// definition-level restatement it is checked against lives in oracle/xy_oracle.c and shares no code
+// definition-level restatement it is checked against lives in the oracle directory and shares no code
 // with this file.  PAPER.md:31, :96-103 (Eq. 6), :452-456 (App. B.a), :490 (colour-sorted storage).
 #include "xy_levy.h"
 

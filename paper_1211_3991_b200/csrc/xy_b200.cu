@@ -1,0 +1,707 @@
+// xy_b200.cu -- C-ABI implementation (include/xy_b200.h): handles, validation, launches, CUDA graphs.
+// Every step of the hot path runs in the kernels of xy_kernels.cuh; nothing here computes physics.
+#include "xy_b200.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <string>
+#include <tuple>
+#include <vector>
+
+#include "xy_kernels.cuh"
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string &msg) {
+    g_err = msg;
+    return code;
+}
+
+#define XY_CUDA(call)                                                                              \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(XY_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));             \
+    } while (0)
+
+template <typename T>
+int dev_alloc(T **p, size_t n) {
+    *p = nullptr;
+    if (n == 0) n = 1;
+    cudaError_t e = cudaMalloc(reinterpret_cast<void **>(p), n * sizeof(T));
+    if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? XY_ENOMEM : XY_ECUDA,
+                                      std::string("cudaMalloc: ") + cudaGetErrorString(e));
+    return XY_OK;
+}
+
+int ceil_div(long long a, long long b) { return static_cast<int>((a + b - 1) / b); }
+
+}  // namespace
+
+struct xy_graph {
+    int S = 0, N = 0, q_max = 0, q_stride = 0, max_degree = 0;
+    long long nnz_total = 0;
+    int2 *rec = nullptr;
+    int32_t *col_idx = nullptr;
+    int32_t *class_ptr = nullptr;
+    std::vector<int32_t> h_class_ptr;  // [S][q_stride]
+    size_t bytes_per_sample = 0;       // rec + col_idx (average), for the schedule heuristic
+    cudaStream_t stream = nullptr;
+};
+
+struct CycleKey {
+    int sps, orps, me, phase, group;
+    bool operator<(const CycleKey &o) const {
+        return std::tie(sps, orps, me, phase, group) < std::tie(o.sps, o.orps, o.me, o.phase, o.group);
+    }
+};
+
+struct CycleGraph {
+    cudaGraphExec_t exec = nullptr;
+    long long launches = 0;
+};
+
+struct xy_pt {
+    const xy_graph *g = nullptr;
+    int R = 0;
+    uint32_t key0 = 0, key1 = 0, sample_base = 0;
+    cudaStream_t stream = nullptr;
+    bool owns_stream = false;
+    float *theta = nullptr;
+    bool owns_theta = false;
+    float *beta_slot = nullptr, *w_slot = nullptr, *beta_f = nullptr, *w_f = nullptr;
+    double *betaT = nullptr;
+    int32_t *temp_of_slot = nullptr, *slot_of_temp = nullptr;
+    uint32_t *counters = nullptr;
+    double *E_slot = nullptr, *M_slot = nullptr, *partial = nullptr, *acc = nullptr;
+    long long *attempts = nullptr, *accepts = nullptr;
+    uint8_t *decisions = nullptr;
+    int n_chunks = 1, chunk_sites = 1;
+    int fast_G = 0;  // lanes per site of the float2 path, 0 = generic kernel
+    int col_blocks = 1;
+    int samples_per_group = 0;  // 0 = automatic
+    // host mirrors
+    uint32_t sweep = 0, round = 0;
+    bool e_fresh = false;
+    long long launches = 0;
+    std::map<CycleKey, CycleGraph> graphs;
+};
+
+namespace {
+
+// ------------------------------------------------------------------------------------------------
+// launches
+// ------------------------------------------------------------------------------------------------
+int max_class_size(const xy_graph *g, int colour, int s0, int s1) {
+    int m = 0;
+    for (int s = s0; s < s1; ++s) {
+        const int32_t *cp = g->h_class_ptr.data() + static_cast<size_t>(s) * g->q_stride;
+        m = std::max(m, cp[colour + 1] - cp[colour]);
+    }
+    return m;
+}
+
+template <int MODE>
+int launch_class(xy_pt *pt, int colour, int s0, int s1, bool use_counter, int sweep_offset, uint32_t sweep_fixed) {
+    const xy_graph *g = pt->g;
+    const int nmax = max_class_size(g, colour, s0, s1);
+    if (nmax == 0 || s1 <= s0) return XY_OK;
+    xy::ClassArgs a;
+    a.rec = g->rec; a.col_idx = g->col_idx; a.class_ptr = g->class_ptr; a.theta = pt->theta;
+    a.beta_slot = pt->beta_slot; a.w_slot = pt->w_slot; a.counters = pt->counters;
+    a.N = g->N; a.R = pt->R; a.q_stride = g->q_stride; a.colour = colour; a.s0 = s0;
+    a.sweep_fixed = sweep_fixed; a.sweep_offset = sweep_offset; a.use_counter = use_counter ? 1 : 0;
+    a.key0 = pt->key0; a.key1 = pt->key1; a.sample_base = pt->sample_base;
+
+    const int G = pt->fast_G;
+    const int spw = G ? 32 / G : 1;
+    const long long groups = (nmax + spw - 1) / spw;                       // warp tasks per sample
+    const long long total = groups * (s1 - s0) * pt->col_blocks;
+    // enough warps for ~2 full waves of 148 SMs x 48 warps, at most 16 site groups per warp
+    int chunk = static_cast<int>(std::min<long long>(16, std::max<long long>(1, total / (148 * 48 * 2))));
+    a.chunk = chunk;
+    dim3 grid(ceil_div(ceil_div(groups, chunk), xy::kWarps), s1 - s0, pt->col_blocks);
+    dim3 block(xy::kBlock);
+    switch (G) {
+        case 32: xy::k_update_class<32, MODE><<<grid, block, 0, pt->stream>>>(a); break;
+        case 16: xy::k_update_class<16, MODE><<<grid, block, 0, pt->stream>>>(a); break;
+        case 8: xy::k_update_class<8, MODE><<<grid, block, 0, pt->stream>>>(a); break;
+        case 4: xy::k_update_class<4, MODE><<<grid, block, 0, pt->stream>>>(a); break;
+        case 2: xy::k_update_class<2, MODE><<<grid, block, 0, pt->stream>>>(a); break;
+        case 1: xy::k_update_class<1, MODE><<<grid, block, 0, pt->stream>>>(a); break;
+        default: xy::k_update_class_generic<MODE><<<grid, block, 0, pt->stream>>>(a); break;
+    }
+    XY_CUDA(cudaGetLastError());
+    pt->launches += 1;
+    return XY_OK;
+}
+
+int launch_measure(xy_pt *pt, int s0, int s1, bool accumulate) {
+    const xy_graph *g = pt->g;
+    if (s1 <= s0) return XY_OK;
+    xy::MeasureArgs m;
+    m.rec = g->rec; m.col_idx = g->col_idx; m.theta = pt->theta; m.partial = pt->partial;
+    m.N = g->N; m.R = pt->R; m.s0 = s0; m.n_chunks = pt->n_chunks; m.chunk_sites = pt->chunk_sites;
+    const size_t smem = static_cast<size_t>(xy::kWarps) * pt->R * 3 * sizeof(double);
+    xy::k_measure_partial<<<dim3(pt->n_chunks, s1 - s0), xy::kBlock, smem, pt->stream>>>(m);
+    XY_CUDA(cudaGetLastError());
+    const int n = (s1 - s0) * pt->R;
+    xy::k_measure_final<<<ceil_div(n, 128), 128, 0, pt->stream>>>(pt->partial, s0, s1, g->N, pt->R, pt->n_chunks,
+                                                               pt->temp_of_slot, pt->E_slot, pt->M_slot, pt->acc,
+                                                               accumulate ? 1 : 0);
+    XY_CUDA(cudaGetLastError());
+    pt->launches += 2;
+    return XY_OK;
+}
+
+int launch_swap(xy_pt *pt, const uint8_t *decisions_dev, uint32_t d_sweep) {
+    xy::SwapArgs a;
+    a.E_slot = pt->E_slot; a.betaT = pt->betaT; a.beta_f = pt->beta_f; a.w_f = pt->w_f;
+    a.slot_of_temp = pt->slot_of_temp; a.temp_of_slot = pt->temp_of_slot;
+    a.beta_slot = pt->beta_slot; a.w_slot = pt->w_slot; a.counters = pt->counters; a.decisions = decisions_dev;
+    a.attempts = pt->attempts; a.accepts = pt->accepts; a.R = pt->R;
+    a.key0 = pt->key0; a.key1 = pt->key1; a.sample_base = pt->sample_base;
+    xy::k_pt_swap<<<pt->g->S, 128, 0, pt->stream>>>(a);
+    XY_CUDA(cudaGetLastError());
+    xy::k_tick<<<1, 1, 0, pt->stream>>>(pt->counters, d_sweep, 1u);
+    XY_CUDA(cudaGetLastError());
+    pt->launches += 2;
+    return XY_OK;
+}
+
+int sweep_group(xy_pt *pt, int mode, int s0, int s1, bool use_counter, int sweep_offset, uint32_t sweep_fixed) {
+    for (int c = 0; c < pt->g->q_max; ++c) {
+        const int rc = mode == 0 ? launch_class<0>(pt, c, s0, s1, use_counter, sweep_offset, sweep_fixed)
+                                 : launch_class<1>(pt, c, s0, s1, false, 0, 0u);
+        if (rc != XY_OK) return rc;
+    }
+    return XY_OK;
+}
+
+int auto_group(const xy_pt *pt) {
+    const xy_graph *g = pt->g;
+    if (pt->samples_per_group > 0) return std::min(pt->samples_per_group, g->S);
+    const double per_sample = static_cast<double>(g->N) * pt->R * 4.0 + static_cast<double>(g->bytes_per_sample);
+    const double l2_budget = 96.0e6;  // of the 126 MB L2
+    if (per_sample * g->S <= l2_budget) return g->S;
+    return std::max(1, std::min(g->S, static_cast<int>(l2_budget / per_sample)));
+}
+
+// enqueue one PT cycle on the stream; `phase` = sweep counter mod measure_every at entry
+int issue_cycle(xy_pt *pt, int sps, int orps, int me, int phase, int group) {
+    const int S = pt->g->S;
+    for (int s0 = 0; s0 < S; s0 += group) {
+        const int s1 = std::min(S, s0 + group);
+        bool fresh = false;
+        for (int k = 1; k <= sps; ++k) {
+            int rc = sweep_group(pt, 0, s0, s1, true, k, 0u);
+            if (rc != XY_OK) return rc;
+            for (int o = 0; o < orps; ++o)
+                if ((rc = sweep_group(pt, 1, s0, s1, false, 0, 0u)) != XY_OK) return rc;
+            fresh = false;
+            if (me > 0 && (phase + k) % me == 0) {
+                if ((rc = launch_measure(pt, s0, s1, true)) != XY_OK) return rc;
+                fresh = true;
+            }
+        }
+        if (!fresh) {
+            const int rc = launch_measure(pt, s0, s1, false);
+            if (rc != XY_OK) return rc;
+        }
+    }
+    return launch_swap(pt, nullptr, static_cast<uint32_t>(sps));
+}
+
+void drop_graphs(xy_pt *pt) {
+    for (auto &kv : pt->graphs)
+        if (kv.second.exec) cudaGraphExecDestroy(kv.second.exec);
+    pt->graphs.clear();
+}
+
+bool check_pt(const xy_pt *pt) { return pt && pt->g; }
+
+}  // namespace
+
+// ====================================================================================================
+extern "C" {
+
+const char *xy_last_error(void) { return g_err.c_str(); }
+int xy_abi_version(void) { return 1; }
+
+int xy_graph_load(int S, int N, const int32_t *row_ptr, const int32_t *col_idx, const int32_t *colour,
+                  void *stream, xy_graph **out) {
+    if (!out) return fail(XY_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (S < 1 || N < 1 || !row_ptr || !colour) return fail(XY_EINVAL, "need S >= 1, N >= 1, non-NULL arrays");
+    try {
+        // ---- validation (host) ----
+        std::vector<long long> off(static_cast<size_t>(S) + 1, 0);
+        int q_max = 0, max_deg = 0;
+        for (int s = 0; s < S; ++s) {
+            const int32_t *rp = row_ptr + static_cast<size_t>(s) * (N + 1);
+            if (rp[0] != 0) return fail(XY_EGRAPH, "row_ptr[s][0] != 0 (sample " + std::to_string(s) + ")");
+            for (int i = 0; i < N; ++i) {
+                if (rp[i + 1] < rp[i]) return fail(XY_EGRAPH, "row_ptr not monotone (sample " + std::to_string(s) + ")");
+                max_deg = std::max(max_deg, rp[i + 1] - rp[i]);
+            }
+            off[s + 1] = off[s] + rp[N];
+        }
+        if (off[S] > 0 && !col_idx) return fail(XY_EINVAL, "col_idx is NULL");
+        if (off[S] > 0x7fffffffll) return fail(XY_EINVAL, "total nnz exceeds int32");
+        std::vector<uint64_t> fwd, rev;
+        for (int s = 0; s < S; ++s) {
+            const int32_t *rp = row_ptr + static_cast<size_t>(s) * (N + 1);
+            const int32_t *ci = col_idx + off[s];
+            const int32_t *col = colour + static_cast<size_t>(s) * N;
+            const std::string where = " (sample " + std::to_string(s) + ")";
+            for (int i = 0; i < N; ++i) {
+                if (col[i] < 0) return fail(XY_EGRAPH, "negative colour" + where);
+                if (i > 0 && col[i] < col[i - 1])
+                    return fail(XY_EGRAPH, "site numbering is not colour-major (colour must be non-decreasing)" + where);
+            }
+            q_max = std::max(q_max, col[N - 1] + 1);
+            fwd.clear(); rev.clear();
+            fwd.reserve(rp[N]); rev.reserve(rp[N]);
+            for (int i = 0; i < N; ++i)
+                for (int e = rp[i]; e < rp[i + 1]; ++e) {
+                    const int j = ci[e];
+                    if (j < 0 || j >= N) return fail(XY_EGRAPH, "neighbour id out of range" + where);
+                    if (j == i) return fail(XY_EGRAPH, "self-loop" + where);
+                    if (col[j] == col[i]) return fail(XY_EGRAPH, "monochromatic edge: colouring is not proper" + where);
+                    fwd.push_back((static_cast<uint64_t>(i) << 32) | static_cast<uint32_t>(j));
+                    rev.push_back((static_cast<uint64_t>(j) << 32) | static_cast<uint32_t>(i));
+                }
+            std::sort(fwd.begin(), fwd.end());
+            std::sort(rev.begin(), rev.end());
+            if (std::adjacent_find(fwd.begin(), fwd.end()) != fwd.end()) return fail(XY_EGRAPH, "duplicate edge" + where);
+            if (fwd != rev) return fail(XY_EGRAPH, "adjacency is not symmetric" + where);
+        }
+        // ---- device copies ----
+        int n_dev = 0;
+        if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1)
+            return fail(XY_ECUDA, "no CUDA device: this library has no CPU fallback");
+        xy_graph *g = new xy_graph();
+        g->S = S; g->N = N; g->q_max = q_max; g->q_stride = q_max + 1; g->max_degree = max_deg;
+        g->nnz_total = off[S];
+        g->stream = static_cast<cudaStream_t>(stream);
+        g->bytes_per_sample = static_cast<size_t>(off[S] / S) * 4 + static_cast<size_t>(N) * 8;
+        std::vector<int2> h_rec(static_cast<size_t>(S) * N);
+        g->h_class_ptr.assign(static_cast<size_t>(S) * g->q_stride, 0);
+        for (int s = 0; s < S; ++s) {
+            const int32_t *rp = row_ptr + static_cast<size_t>(s) * (N + 1);
+            const int32_t *col = colour + static_cast<size_t>(s) * N;
+            int32_t *cp = g->h_class_ptr.data() + static_cast<size_t>(s) * g->q_stride;
+            for (int i = 0; i < N; ++i) {
+                h_rec[static_cast<size_t>(s) * N + i] = make_int2(static_cast<int>(off[s] + rp[i]), rp[i + 1] - rp[i]);
+                cp[col[i] + 1]++;
+            }
+            for (int c = 0; c < q_max; ++c) cp[c + 1] += cp[c];
+        }
+        int rc;
+        if ((rc = dev_alloc(&g->rec, h_rec.size())) != XY_OK || (rc = dev_alloc(&g->col_idx, off[S])) != XY_OK ||
+            (rc = dev_alloc(&g->class_ptr, g->h_class_ptr.size())) != XY_OK) {
+            xy_graph_free(g);
+            return rc;
+        }
+        cudaError_t e = cudaMemcpyAsync(g->rec, h_rec.data(), h_rec.size() * sizeof(int2), cudaMemcpyHostToDevice, g->stream);
+        if (e == cudaSuccess && off[S] > 0)
+            e = cudaMemcpyAsync(g->col_idx, col_idx, off[S] * sizeof(int32_t), cudaMemcpyHostToDevice, g->stream);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(g->class_ptr, g->h_class_ptr.data(), g->h_class_ptr.size() * sizeof(int32_t),
+                                cudaMemcpyHostToDevice, g->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(g->stream);
+        if (e != cudaSuccess) {
+            xy_graph_free(g);
+            return fail(XY_ECUDA, std::string("graph upload: ") + cudaGetErrorString(e));
+        }
+        *out = g;
+        return XY_OK;
+    } catch (const std::bad_alloc &) {
+        return fail(XY_ENOMEM, "host allocation failed");
+    }
+}
+
+int xy_graph_free(xy_graph *g) {
+    if (!g) return XY_OK;
+    cudaFree(g->rec); cudaFree(g->col_idx); cudaFree(g->class_ptr);
+    delete g;
+    return XY_OK;
+}
+
+int xy_graph_info(const xy_graph *g, int *S, int *N, int64_t *nnz_total, int *q_max, int *max_degree) {
+    if (!g) return fail(XY_EINVAL, "graph is NULL");
+    if (S) *S = g->S;
+    if (N) *N = g->N;
+    if (nnz_total) *nnz_total = g->nnz_total;
+    if (q_max) *q_max = g->q_max;
+    if (max_degree) *max_degree = g->max_degree;
+    return XY_OK;
+}
+
+int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width, uint64_t seed, uint32_t sample_base,
+                 float *theta_dev, void *stream, xy_pt **out) {
+    if (!out) return fail(XY_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!g || !T) return fail(XY_EINVAL, "graph or T is NULL");
+    if (R < 1 || R > 1024) return fail(XY_EINVAL, "need 1 <= R <= 1024");
+    if (static_cast<uint64_t>(sample_base) + g->S > 65536u) return fail(XY_EINVAL, "sample_base + S must be <= 65536");
+    for (int k = 0; k < R; ++k) {
+        if (!(T[k] > 0.0)) return fail(XY_EINVAL, "temperatures must be > 0");
+        if (k > 0 && !(T[k] >= T[k - 1])) return fail(XY_EINVAL, "temperatures must be ascending");
+        if (width && !(width[k] >= 0.0 && std::isfinite(width[k]))) return fail(XY_EINVAL, "bad proposal width");
+    }
+    if (theta_dev && (reinterpret_cast<uintptr_t>(theta_dev) & 7u)) return fail(XY_EINVAL, "theta_dev must be 8-byte aligned");
+    xy_pt *pt = nullptr;
+    try {
+        pt = new xy_pt();
+    } catch (const std::bad_alloc &) {
+        return fail(XY_ENOMEM, "host allocation failed");
+    }
+    pt->g = g; pt->R = R;
+    pt->key0 = static_cast<uint32_t>(seed); pt->key1 = static_cast<uint32_t>(seed >> 32);
+    pt->sample_base = sample_base;
+    pt->stream = static_cast<cudaStream_t>(stream);
+    if (!pt->stream) {  // CUDA graphs cannot be captured on the legacy default stream
+        const cudaError_t es = cudaStreamCreateWithFlags(&pt->stream, cudaStreamNonBlocking);
+        if (es != cudaSuccess) {
+            delete pt;
+            return fail(XY_ECUDA, std::string("cudaStreamCreate: ") + cudaGetErrorString(es));
+        }
+        pt->owns_stream = true;
+    }
+    const int S = g->S, N = g->N;
+    // kernel flavour: float2 path when R = 2G with G a power of two <= 32, or R a multiple of 64
+    pt->fast_G = 0; pt->col_blocks = 1;
+    if (R % 64 == 0) { pt->fast_G = 32; pt->col_blocks = R / 64; }
+    else if (R % 2 == 0 && R / 2 <= 32 && ((R / 2) & (R / 2 - 1)) == 0) pt->fast_G = R / 2;
+    // measure partition: a function of N only, so results do not depend on the schedule
+    pt->chunk_sites = std::max(256, ((N + 127) / 128 + 7) / 8 * 8);
+    pt->n_chunks = (N + pt->chunk_sites - 1) / pt->chunk_sites;
+
+    const size_t SR = static_cast<size_t>(S) * R;
+    int rc = XY_OK;
+    auto A = [&](int r) { if (rc == XY_OK) rc = r; };
+    if (theta_dev) pt->theta = theta_dev;
+    else { A(dev_alloc(&pt->theta, SR * N)); pt->owns_theta = true; }
+    A(dev_alloc(&pt->beta_slot, SR)); A(dev_alloc(&pt->w_slot, SR));
+    A(dev_alloc(&pt->beta_f, R)); A(dev_alloc(&pt->w_f, R)); A(dev_alloc(&pt->betaT, R));
+    A(dev_alloc(&pt->temp_of_slot, SR)); A(dev_alloc(&pt->slot_of_temp, SR));
+    A(dev_alloc(&pt->counters, 2));
+    A(dev_alloc(&pt->E_slot, SR)); A(dev_alloc(&pt->M_slot, SR * 2));
+    A(dev_alloc(&pt->partial, SR * pt->n_chunks * 3)); A(dev_alloc(&pt->acc, SR * XY_NACC));
+    A(dev_alloc(&pt->attempts, SR)); A(dev_alloc(&pt->accepts, SR)); A(dev_alloc(&pt->decisions, SR));
+    if (rc != XY_OK) { xy_pt_destroy(pt); return rc; }
+    {
+        const size_t smem = static_cast<size_t>(xy::kWarps) * R * 3 * sizeof(double);
+        if (smem > 48 * 1024) {
+            const cudaError_t ea = cudaFuncSetAttribute(xy::k_measure_partial, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                        static_cast<int>(smem));
+            if (ea != cudaSuccess) {
+                xy_pt_destroy(pt);
+                return fail(XY_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(ea));
+            }
+        }
+    }
+
+    std::vector<float> hb(R), hw(R);
+    std::vector<double> hbT(R);
+    std::vector<int32_t> lab(SR);
+    for (int k = 0; k < R; ++k) {
+        hbT[k] = 1.0 / T[k];
+        hb[k] = static_cast<float>(1.0 / T[k]);
+        const double half = 0.5 * T[k];
+        hw[k] = static_cast<float>(width ? width[k] : 6.283185307179586476925286766559 * (half < 1.0 ? half : 1.0));
+    }
+    for (size_t i = 0; i < SR; ++i) lab[i] = static_cast<int32_t>(i % R);
+    cudaError_t e = cudaMemcpyAsync(pt->beta_f, hb.data(), R * sizeof(float), cudaMemcpyHostToDevice, pt->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(pt->w_f, hw.data(), R * sizeof(float), cudaMemcpyHostToDevice, pt->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(pt->betaT, hbT.data(), R * sizeof(double), cudaMemcpyHostToDevice, pt->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(pt->temp_of_slot, lab.data(), SR * sizeof(int32_t), cudaMemcpyHostToDevice, pt->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(pt->counters, 0, 2 * sizeof(uint32_t), pt->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(pt->acc, 0, SR * XY_NACC * sizeof(double), pt->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(pt->attempts, 0, SR * sizeof(long long), pt->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(pt->accepts, 0, SR * sizeof(long long), pt->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(pt->E_slot, 0, SR * sizeof(double), pt->stream);
+    if (e == cudaSuccess) {
+        xy::k_refresh_slot_params<<<ceil_div(SR, 128), 128, 0, pt->stream>>>(pt->temp_of_slot, pt->slot_of_temp, pt->beta_f,
+                                                                            pt->w_f, pt->beta_slot, pt->w_slot, S, R);
+        xy::k_init_theta<<<148 * 8, 256, 0, pt->stream>>>(pt->theta, S, N, R, pt->key0, pt->key1, pt->sample_base);
+        pt->launches += 2;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(pt->stream);
+    if (e != cudaSuccess) {
+        xy_pt_destroy(pt);
+        return fail(XY_ECUDA, std::string("xy_pt_create: ") + cudaGetErrorString(e));
+    }
+    *out = pt;
+    return XY_OK;
+}
+
+int xy_pt_destroy(xy_pt *pt) {
+    if (!pt) return XY_OK;
+    cudaStreamSynchronize(pt->stream);
+    drop_graphs(pt);
+    if (pt->owns_theta) cudaFree(pt->theta);
+    cudaFree(pt->beta_slot); cudaFree(pt->w_slot); cudaFree(pt->beta_f); cudaFree(pt->w_f); cudaFree(pt->betaT);
+    cudaFree(pt->temp_of_slot); cudaFree(pt->slot_of_temp); cudaFree(pt->counters);
+    cudaFree(pt->E_slot); cudaFree(pt->M_slot); cudaFree(pt->partial); cudaFree(pt->acc);
+    cudaFree(pt->attempts); cudaFree(pt->accepts); cudaFree(pt->decisions);
+    if (pt->owns_stream) cudaStreamDestroy(pt->stream);
+    delete pt;
+    return XY_OK;
+}
+
+int xy_sweep(xy_pt *pt, int n_sweeps) {
+    if (!check_pt(pt) || n_sweeps < 0) return fail(XY_EINVAL, "bad handle or n_sweeps < 0");
+    for (int n = 0; n < n_sweeps; ++n) {
+        const int rc = sweep_group(pt, 0, 0, pt->g->S, true, 1, 0u);
+        if (rc != XY_OK) return rc;
+        xy::k_tick<<<1, 1, 0, pt->stream>>>(pt->counters, 1u, 0u);
+        XY_CUDA(cudaGetLastError());
+        pt->launches += 1;
+        pt->sweep += 1;
+    }
+    if (n_sweeps > 0) pt->e_fresh = false;
+    return XY_OK;
+}
+
+int xy_overrelax(xy_pt *pt, int n_sweeps) {
+    if (!check_pt(pt) || n_sweeps < 0) return fail(XY_EINVAL, "bad handle or n_sweeps < 0");
+    for (int n = 0; n < n_sweeps; ++n) {
+        const int rc = sweep_group(pt, 1, 0, pt->g->S, false, 0, 0u);
+        if (rc != XY_OK) return rc;
+    }
+    if (n_sweeps > 0) pt->e_fresh = false;
+    return XY_OK;
+}
+
+int xy_metropolis_colour(xy_pt *pt, int colour, uint32_t sweep) {
+    if (!check_pt(pt) || colour < 0 || colour >= pt->g->q_max) return fail(XY_EINVAL, "bad handle or colour");
+    pt->e_fresh = false;
+    return launch_class<0>(pt, colour, 0, pt->g->S, false, 0, sweep);
+}
+
+int xy_overrelax_colour(xy_pt *pt, int colour) {
+    if (!check_pt(pt) || colour < 0 || colour >= pt->g->q_max) return fail(XY_EINVAL, "bad handle or colour");
+    pt->e_fresh = false;
+    return launch_class<1>(pt, colour, 0, pt->g->S, false, 0, 0u);
+}
+
+int xy_pt_swap(xy_pt *pt) {
+    if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    if (!pt->e_fresh) {
+        const int rc = launch_measure(pt, 0, pt->g->S, false);
+        if (rc != XY_OK) return rc;
+        pt->e_fresh = true;
+    }
+    const int rc = launch_swap(pt, nullptr, 0u);
+    if (rc == XY_OK) pt->round += 1;
+    return rc;
+}
+
+int xy_swap_with_decisions(xy_pt *pt, const uint8_t *accept_host) {
+    if (!check_pt(pt) || !accept_host) return fail(XY_EINVAL, "bad handle or NULL decisions");
+    const size_t SR = static_cast<size_t>(pt->g->S) * pt->R;
+    XY_CUDA(cudaMemcpyAsync(pt->decisions, accept_host, SR, cudaMemcpyHostToDevice, pt->stream));
+    XY_CUDA(cudaStreamSynchronize(pt->stream));  // accept_host is borrowed for the call only
+    const int rc = launch_swap(pt, pt->decisions, 0u);
+    if (rc == XY_OK) pt->round += 1;
+    return rc;
+}
+
+int xy_measure(xy_pt *pt, double *out_host) {
+    if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    const int S = pt->g->S, R = pt->R;
+    const int rc = launch_measure(pt, 0, S, true);
+    if (rc != XY_OK) return rc;
+    pt->e_fresh = true;
+    if (out_host) {
+        const size_t SR = static_cast<size_t>(S) * R;
+        try {
+            std::vector<double> E(SR), M(SR * 2);
+            std::vector<int32_t> tos(SR);
+            XY_CUDA(cudaMemcpyAsync(E.data(), pt->E_slot, SR * sizeof(double), cudaMemcpyDeviceToHost, pt->stream));
+            XY_CUDA(cudaMemcpyAsync(M.data(), pt->M_slot, SR * 2 * sizeof(double), cudaMemcpyDeviceToHost, pt->stream));
+            XY_CUDA(cudaMemcpyAsync(tos.data(), pt->temp_of_slot, SR * sizeof(int32_t), cudaMemcpyDeviceToHost, pt->stream));
+            XY_CUDA(cudaStreamSynchronize(pt->stream));
+            for (int s = 0; s < S; ++s)
+                for (int r = 0; r < R; ++r) {
+                    const size_t i = static_cast<size_t>(s) * R + r;
+                    double *o = out_host + (static_cast<size_t>(s) * R + tos[i]) * 3;
+                    o[0] = E[i]; o[1] = M[2 * i]; o[2] = M[2 * i + 1];
+                }
+        } catch (const std::bad_alloc &) {
+            return fail(XY_ENOMEM, "host allocation failed");
+        }
+    }
+    return XY_OK;
+}
+
+int xy_set_schedule(xy_pt *pt, int samples_per_group) {
+    if (!check_pt(pt) || samples_per_group < 0) return fail(XY_EINVAL, "bad handle or samples_per_group < 0");
+    pt->samples_per_group = samples_per_group;
+    return XY_OK;
+}
+
+int xy_run(xy_pt *pt, int n_cycles, int sps, int orps, int me) {
+    if (!check_pt(pt) || n_cycles < 0 || sps < 1 || orps < 0 || me < 0)
+        return fail(XY_EINVAL, "need n_cycles >= 0, sweeps_per_swap >= 1, or_per_sweep >= 0, measure_every >= 0");
+    const int group = auto_group(pt);
+    for (int c = 0; c < n_cycles; ++c) {
+        const int phase = me > 0 ? static_cast<int>(pt->sweep % static_cast<uint32_t>(me)) : 0;
+        const CycleKey key{sps, orps, me, phase, group};
+        auto it = pt->graphs.find(key);
+        if (it == pt->graphs.end()) {
+            if (pt->graphs.size() >= 32) drop_graphs(pt);
+            cudaGraph_t graph = nullptr;
+            const long long before = pt->launches;
+            XY_CUDA(cudaStreamBeginCapture(pt->stream, cudaStreamCaptureModeThreadLocal));
+            const int rc = issue_cycle(pt, sps, orps, me, phase, group);
+            const cudaError_t e = cudaStreamEndCapture(pt->stream, &graph);
+            CycleGraph cg;
+            cg.launches = pt->launches - before;
+            pt->launches = before;
+            if (rc != XY_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+            if (e != cudaSuccess) return fail(XY_ECUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(e));
+            const cudaError_t e2 = cudaGraphInstantiate(&cg.exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (e2 != cudaSuccess) return fail(XY_ECUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e2));
+            it = pt->graphs.emplace(key, cg).first;
+        }
+        XY_CUDA(cudaGraphLaunch(it->second.exec, pt->stream));
+        pt->launches += it->second.launches;
+        pt->sweep += static_cast<uint32_t>(sps);
+        pt->round += 1;
+        pt->e_fresh = false;  // labels moved; E per slot is still valid but keep the rule simple
+    }
+    return XY_OK;
+}
+
+int xy_get_theta(xy_pt *pt, float *theta_host) {
+    if (!check_pt(pt) || !theta_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
+    const size_t n = static_cast<size_t>(pt->g->S) * pt->g->N * pt->R;
+    XY_CUDA(cudaMemcpyAsync(theta_host, pt->theta, n * sizeof(float), cudaMemcpyDeviceToHost, pt->stream));
+    XY_CUDA(cudaStreamSynchronize(pt->stream));
+    return XY_OK;
+}
+
+int xy_set_theta(xy_pt *pt, const float *theta_host) {
+    if (!check_pt(pt) || !theta_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
+    const size_t n = static_cast<size_t>(pt->g->S) * pt->g->N * pt->R;
+    XY_CUDA(cudaMemcpyAsync(pt->theta, theta_host, n * sizeof(float), cudaMemcpyHostToDevice, pt->stream));
+    XY_CUDA(cudaStreamSynchronize(pt->stream));
+    pt->e_fresh = false;
+    return XY_OK;
+}
+
+int xy_get_labels(xy_pt *pt, int32_t *temp_of_slot_host) {
+    if (!check_pt(pt) || !temp_of_slot_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
+    const size_t SR = static_cast<size_t>(pt->g->S) * pt->R;
+    XY_CUDA(cudaMemcpyAsync(temp_of_slot_host, pt->temp_of_slot, SR * sizeof(int32_t), cudaMemcpyDeviceToHost, pt->stream));
+    XY_CUDA(cudaStreamSynchronize(pt->stream));
+    return XY_OK;
+}
+
+int xy_set_labels(xy_pt *pt, const int32_t *temp_of_slot_host) {
+    if (!check_pt(pt) || !temp_of_slot_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
+    const int S = pt->g->S, R = pt->R;
+    try {
+        std::vector<uint8_t> seen(R);
+        for (int s = 0; s < S; ++s) {
+            std::fill(seen.begin(), seen.end(), 0);
+            for (int r = 0; r < R; ++r) {
+                const int t = temp_of_slot_host[static_cast<size_t>(s) * R + r];
+                if (t < 0 || t >= R || seen[t]) return fail(XY_EINVAL, "labels are not a permutation of 0..R-1");
+                seen[t] = 1;
+            }
+        }
+    } catch (const std::bad_alloc &) {
+        return fail(XY_ENOMEM, "host allocation failed");
+    }
+    const size_t SR = static_cast<size_t>(S) * R;
+    XY_CUDA(cudaMemcpyAsync(pt->temp_of_slot, temp_of_slot_host, SR * sizeof(int32_t), cudaMemcpyHostToDevice, pt->stream));
+    xy::k_refresh_slot_params<<<ceil_div(SR, 128), 128, 0, pt->stream>>>(pt->temp_of_slot, pt->slot_of_temp, pt->beta_f, pt->w_f,
+                                                                        pt->beta_slot, pt->w_slot, S, R);
+    XY_CUDA(cudaGetLastError());
+    pt->launches += 1;
+    XY_CUDA(cudaStreamSynchronize(pt->stream));
+    return XY_OK;
+}
+
+int xy_get_energy(xy_pt *pt, double *E_slot_host) {
+    if (!check_pt(pt) || !E_slot_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
+    if (!pt->e_fresh) {
+        const int rc = launch_measure(pt, 0, pt->g->S, false);
+        if (rc != XY_OK) return rc;
+        pt->e_fresh = true;
+    }
+    const size_t SR = static_cast<size_t>(pt->g->S) * pt->R;
+    XY_CUDA(cudaMemcpyAsync(E_slot_host, pt->E_slot, SR * sizeof(double), cudaMemcpyDeviceToHost, pt->stream));
+    XY_CUDA(cudaStreamSynchronize(pt->stream));
+    return XY_OK;
+}
+
+int xy_read_accumulators(xy_pt *pt, double *acc_host) {
+    if (!check_pt(pt) || !acc_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
+    const size_t n = static_cast<size_t>(pt->g->S) * pt->R * XY_NACC;
+    XY_CUDA(cudaMemcpyAsync(acc_host, pt->acc, n * sizeof(double), cudaMemcpyDeviceToHost, pt->stream));
+    XY_CUDA(cudaStreamSynchronize(pt->stream));
+    return XY_OK;
+}
+
+int xy_reset_accumulators(xy_pt *pt) {
+    if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    const size_t n = static_cast<size_t>(pt->g->S) * pt->R * XY_NACC;
+    XY_CUDA(cudaMemsetAsync(pt->acc, 0, n * sizeof(double), pt->stream));
+    return XY_OK;
+}
+
+int xy_get_counters(xy_pt *pt, uint32_t *sweep, uint32_t *round, int64_t *att, int64_t *acc) {
+    if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    uint32_t c[2];
+    const size_t SR = static_cast<size_t>(pt->g->S) * pt->R;
+    XY_CUDA(cudaMemcpyAsync(c, pt->counters, sizeof(c), cudaMemcpyDeviceToHost, pt->stream));
+    if (att) XY_CUDA(cudaMemcpyAsync(att, pt->attempts, SR * sizeof(int64_t), cudaMemcpyDeviceToHost, pt->stream));
+    if (acc) XY_CUDA(cudaMemcpyAsync(acc, pt->accepts, SR * sizeof(int64_t), cudaMemcpyDeviceToHost, pt->stream));
+    XY_CUDA(cudaStreamSynchronize(pt->stream));
+    if (c[0] != pt->sweep || c[1] != pt->round) return fail(XY_ESTATE, "device counters diverged from the host mirror");
+    if (sweep) *sweep = c[0];
+    if (round) *round = c[1];
+    return XY_OK;
+}
+
+int xy_set_counters(xy_pt *pt, uint32_t sweep, uint32_t round) {
+    if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    const uint32_t c[2] = {sweep, round};
+    XY_CUDA(cudaMemcpyAsync(pt->counters, c, sizeof(c), cudaMemcpyHostToDevice, pt->stream));
+    XY_CUDA(cudaStreamSynchronize(pt->stream));
+    pt->sweep = sweep; pt->round = round;
+    return XY_OK;
+}
+
+int xy_theta_device(xy_pt *pt, float **theta_dev) {
+    if (!check_pt(pt) || !theta_dev) return fail(XY_EINVAL, "bad handle or NULL out");
+    *theta_dev = pt->theta;
+    return XY_OK;
+}
+
+int xy_launch_count(xy_pt *pt, int64_t *n) {
+    if (!check_pt(pt) || !n) return fail(XY_EINVAL, "bad handle or NULL out");
+    *n = pt->launches;
+    return XY_OK;
+}
+
+int xy_synchronize(xy_pt *pt) {
+    if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    XY_CUDA(cudaStreamSynchronize(pt->stream));
+    return XY_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,298 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI) against the oracle, element by element on the
+same seeded inputs (BASELINE.json north_star): bit-exact integer work, |dtheta| <= 1e-5 rad after one
+step from an identical state (near-threshold / ill-conditioned sites counted and reported)."""
+import numpy as np
+import pytest
+
+import graphs as G
+import gpu_util as U
+import oracle as O
+from paper_1211_3991_b200 import binding as B
+from paper_1211_3991_b200 import levy, workloads
+
+pytestmark = pytest.mark.gpu
+SEED = 0xA5A5F00D1234
+
+
+def small_levy(L, rho, S, sample_base=0):
+    return levy.build(L, rho, 6, workloads.BASE_SEED, S=S, sample_base=sample_base)
+
+
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("R", [1, 2, 3, 8, 16, 32, 64, 128, 6])
+def test_init_theta_bit_exact(R):
+    g = small_levy(8, 3.5, 3, sample_base=5)
+    T = O.geometric_temperatures(R, 1.0, 4.0)
+    ens = U.ensemble_from_levy(g, T, SEED, sample_base=5)
+    th = ens.get_theta()
+    for s in range(3):
+        assert np.array_equal(th[s], O.init_theta(64, R, SEED, 5 + s))
+    assert np.array_equal(ens.get_labels(), np.tile(np.arange(R, dtype=np.int32), (3, 1)))
+    ens.close()
+
+
+@pytest.mark.parametrize("L,rho,R,S", [(16, 3.5, 8, 1), (16, 3.5, 64, 2), (24, 2.5, 16, 3), (16, 4.5, 32, 2),
+                                        (12, 3.0, 2, 2), (12, 3.0, 4, 2), (8, 3.5, 128, 1), (12, 3.5, 3, 2),
+                                        (12, 3.5, 1, 1), (12, 3.5, 6, 2), (12, 3.5, 10, 1)])
+def test_lockstep_one_sweep_metropolis_and_overrelax(L, rho, R, S):
+    """config-0-like sizes spanning every kernel flavour (G = 1..32, column blocks, generic R)."""
+    g = small_levy(L, rho, S, sample_base=2)
+    T = O.geometric_temperatures(R, 1.0, 4.0)
+    ens = U.ensemble_from_levy(g, T, SEED, sample_base=2)
+    graphs = U.graphs_of_levy(g)
+    # scramble the labels so that slot != temperature
+    rng = np.random.default_rng(7)
+    lab = np.stack([rng.permutation(R).astype(np.int32) for _ in range(S)])
+    ens.set_labels(lab)
+    assert np.array_equal(ens.get_labels(), lab)
+    Q = int(g.n_colours.max())
+    tot_m = dict(updates=0, near=0, bad=0, accepted=0, disagree_near=0)
+    tot_o = dict(updates=0, illcond=0, bad=0)
+    for sweep in (1, 2, 3):
+        for c in range(Q):
+            st = U.lockstep_metropolis(ens, graphs, T, SEED, c, sweep, sample_base=2)
+            for k in tot_m: tot_m[k] += st[k]
+            assert st["bad"] == 0, st
+        for c in range(Q):
+            st = U.lockstep_overrelax(ens, graphs, c)
+            for k in tot_o: tot_o[k] += st[k]
+            assert st["bad"] == 0, st
+    assert tot_m["updates"] == 3 * L * L * R * S and tot_o["updates"] == 3 * L * L * R * S
+    assert 0.2 < tot_m["accepted"] / tot_m["updates"] < 0.95
+    assert tot_m["near"] <= 5 + 2e-4 * tot_m["updates"]              # expected ~2e-5 per update
+    assert tot_o["illcond"] <= 5 + 5e-3 * tot_o["updates"]           # <= 0.17 % at T = inf
+    print(f"\n[lockstep L={L} R={R} S={S}] metropolis {tot_m}  overrelax {tot_o}")
+    th = ens.get_theta()
+    assert th.min() >= 0.0 and th.max() <= np.float32(6.2831855)
+    ens.close()
+
+
+def test_metropolis_sweep_trajectory_config0():
+    """one full Metropolis sweep (all colours) from an identical state: angles are bit-identical except inside
+    the influence cone of a near-threshold site (none expected at this size)."""
+    w = workloads.CONFIGS[0]
+    g = levy.build(w.L, w.rho, w.z, w.seed, S=1)
+    T = w.temperatures()
+    ens = U.ensemble_from_levy(g, T, SEED)
+    ref = O.init_theta(w.N, w.R, SEED, 0)
+    cp = g.class_ptr(0)
+    bs, ws = O.temperature_params(T)
+    min_margin = np.inf
+    for sweep in range(1, 6):
+        ens.sweep(1)
+        for c in range(len(cp) - 1):
+            m, _ = O.metropolis_sites(g.row_ptr[0], g.col_idx[0], ref, np.arange(cp[c], cp[c + 1], dtype=np.int32), bs, ws,
+                                      SEED, sweep, 0, want_margin=True)
+            min_margin = min(min_margin, m.min())
+        if min_margin < U.BAND:
+            break
+        assert np.array_equal(ens.get_theta()[0], ref), f"sweep {sweep}"
+    assert sweep >= 2
+    assert ens.get_counters()[0] == sweep
+    ens.close()
+
+
+@pytest.mark.parametrize("L,R,S", [(16, 8, 1), (16, 64, 2), (12, 3, 2), (20, 16, 2)])
+def test_measure_matches_oracle(L, R, S):
+    g = small_levy(L, 3.5, S)
+    T = O.geometric_temperatures(R, 1.0, 4.0)
+    ens = U.ensemble_from_levy(g, T, SEED)
+    ens.sweep(2); ens.overrelax(1)
+    rng = np.random.default_rng(3)
+    lab = np.stack([rng.permutation(R).astype(np.int32) for _ in range(S)])
+    ens.set_labels(lab)
+    out = ens.measure(want=True)
+    th = ens.get_theta()
+    E_slot = ens.get_energy()
+    n_bonds = L * L * 3
+    for s in range(S):
+        E, Mx, My = O.measure(g.row_ptr[s], g.col_idx[s], th[s])
+        # fp32 angle difference (<= ulp(2pi)/2 = 2.4e-7) + cosf (1e-7): |dE| <= 4e-7 per bond, worst case
+        assert np.all(np.abs(E_slot[s] - E) <= 4e-7 * n_bonds)
+        assert np.all(np.abs(out[s, lab[s], 0] - E) <= 4e-7 * n_bonds)
+        assert np.all(np.abs(out[s, lab[s], 1] - Mx) <= 2e-7 * L * L) and np.all(np.abs(out[s, lab[s], 2] - My) <= 2e-7 * L * L)
+    acc = ens.read_accumulators()
+    ref = np.zeros((S, R, O.NACC))
+    for s in range(S):
+        O.accumulate(L * L, out[s, lab[s], 0].copy(), out[s, lab[s], 1].copy(), out[s, lab[s], 2].copy(), lab[s], ref[s])
+    assert np.allclose(acc, ref, rtol=1e-12, atol=1e-12)
+    ens.reset_accumulators()
+    assert np.all(ens.read_accumulators() == 0)
+    ens.close()
+
+
+@pytest.mark.parametrize("R,S", [(8, 1), (32, 3), (5, 2), (2, 1), (1, 1)])
+def test_pt_swap_labels_bit_exact(R, S):
+    g = small_levy(12, 3.5, S, sample_base=1)
+    T = O.geometric_temperatures(R, 1.0, 4.0)
+    ens = U.ensemble_from_levy(g, T, SEED, sample_base=1)
+    ens.sweep(3)
+    tos = ens.get_labels().copy()
+    sot = np.argsort(tos, axis=1).astype(np.int32)
+    rng = np.random.default_rng(11)
+    n_near = 0
+    for rnd in range(12):
+        E = ens.get_energy()
+        if rnd % 2 == 0:                      # free-running: decisions must coincide given the same energies
+            ens.pt_swap()
+            for s in range(S):
+                dec, mar = O.pt_swap(T, E[s], sot[s], tos[s], SEED, rnd, 1 + s)
+                n_near += int((mar < U.BAND).sum())
+        else:                                 # forced decisions: bit-exact permutation test
+            dec_in = rng.integers(0, 2, (S, R)).astype(np.uint8)
+            ens.swap_with_decisions(dec_in)
+            for s in range(S):
+                O.pt_swap(T, E[s], sot[s], tos[s], SEED, rnd, 1 + s, decisions_in=dec_in[s])
+        if n_near == 0:
+            assert np.array_equal(ens.get_labels(), tos), f"round {rnd}"
+        ens.sweep(1)
+    sw, rd, att, acc = ens.get_counters()
+    assert rd == 12 and sw == 3 + 12
+    if R >= 2:
+        assert att[:, 0].min() == 6 and np.all(acc <= att)
+    ens.close()
+
+
+def test_run_equals_stepwise_calls_and_schedule_invariance():
+    """xy_run (captured CUDA graph, device-side counters) == the same sequence issued call by call, and the
+    result does not depend on samples_per_group."""
+    g = small_levy(16, 3.5, 4)
+    T = O.geometric_temperatures(16, 1.0, 4.0)
+    a = U.ensemble_from_levy(g, T, SEED); b = U.ensemble_from_levy(g, T, SEED); c = U.ensemble_from_levy(g, T, SEED)
+    a.set_schedule(4); c.set_schedule(1)
+    n_cycles, sps, orps, me = 3, 4, 2, 2
+    a.run(n_cycles, sps, orps, me)
+    c.run(n_cycles, sps, orps, me)
+    for _ in range(n_cycles):
+        for k in range(sps):
+            b.sweep(1); b.overrelax(orps)
+            if (b.get_counters()[0]) % me == 0:
+                b.measure()
+        b.pt_swap()
+    for other in (b, c):
+        assert np.array_equal(a.get_theta(), other.get_theta())
+        assert np.array_equal(a.get_labels(), other.get_labels())
+        assert np.array_equal(a.read_accumulators(), other.read_accumulators())
+        assert a.get_counters()[:2] == other.get_counters()[:2] == (n_cycles * sps, n_cycles)
+    assert a.read_accumulators()[..., 0].min() == n_cycles * sps // me
+    # measure_every not dividing sweeps_per_swap: phase-dependent graphs
+    a.run(3, 3, 1, 2); c.run(3, 3, 1, 2)
+    assert np.array_equal(a.get_theta(), c.get_theta()) and np.array_equal(a.read_accumulators(), c.read_accumulators())
+    assert a.read_accumulators()[..., 0].min() == 6 + (21 // 2 - 6)
+    assert a.launch_count() > 0
+    for e in (a, b, c): e.close()
+
+
+def test_run_matches_oracle_protocol_short():
+    """two full cycles on config 0 against orc_run: labels, counters and accumulated observables agree as long
+    as no decision was near threshold (angles are compared in lockstep elsewhere; here the protocol order,
+    measurement cadence and swap bookkeeping are what is checked)."""
+    w = workloads.CONFIGS[0]
+    g = levy.build(w.L, w.rho, w.z, w.seed, S=1)
+    T = w.temperatures()
+    ens = U.ensemble_from_levy(g, T, SEED)
+    ch = O.Chain(g.row_ptr[0], g.col_idx[0], g.class_ptr(0), T, SEED)
+    ens.run(1, 2, 1, 1); ch.run(1, 2, 1, 1)
+    acc = ens.read_accumulators()[0]
+    assert np.array_equal(acc[:, 0], ch.acc[:, 0])
+    assert np.allclose(acc[:, 1], ch.acc[:, 1], rtol=0, atol=2e-3)            # sum of 2 energies, chaotic drift small
+    assert np.allclose(acc[:, 4], ch.acc[:, 4], rtol=0, atol=1e-4)
+    assert np.array_equal(ens.get_labels()[0], ch.temp_of_slot)
+    assert U.circ(ens.get_theta()[0], ch.theta).mean() < 1e-3
+    ens.close()
+
+
+# ---------------------------------------------------------------------------------------------------
+def test_graph_load_rejects_bad_graphs_and_accepts_odd_ones():
+    gd = G.colour_major(6, G.ring_edges(6))
+    rp, ci, col = gd["row_ptr"], gd["col_idx"], gd["colour"]
+    g = B.xy_graph_load(rp, ci, col)
+    assert B.xy_graph_info(g) == dict(S=1, N=6, nnz_total=12, q_max=2, max_degree=2)
+    B.xy_graph_free(g)
+
+    def rejected(rp_, ci_, col_):
+        with pytest.raises(B.XYError) as e:
+            B.xy_graph_load(rp_, ci_, col_)
+        assert e.value.code == B.XY_EGRAPH, str(e.value)
+        return str(e.value)
+
+    bad = col.copy(); bad[:] = 0
+    assert "monochromatic" in rejected(rp, ci, bad)
+    assert "colour-major" in rejected(rp, ci, col[::-1].copy())
+    ci2 = ci.copy(); ci2[0] = 0
+    rejected(rp, ci2, col)                                        # self loop / monochromatic
+    ci3 = ci.copy(); ci3[0] = 99
+    assert "range" in rejected(rp, ci3, col)
+    # asymmetric: drop one direction
+    e = [(0, 3), (1, 3)]
+    rp4, ci4 = G.csr_from_edges(4, e)
+    ci4 = ci4.copy(); rp4 = rp4.copy()
+    col4 = np.array([0, 0, 0, 1], np.int32)
+    ci_asym = np.array([3, 3, 0], np.int32); rp_asym = np.array([0, 1, 2, 2, 3], np.int32)
+    assert "symmetric" in rejected(rp_asym, ci_asym, col4)
+    ci_dup = np.array([3, 3, 3, 0, 0, 1], np.int32); rp_dup = np.array([0, 2, 3, 3, 6], np.int32)
+    assert "duplicate" in rejected(rp_dup, ci_dup, col4)
+    rp_bad = rp.copy(); rp_bad[0] = 1
+    rejected(rp_bad, ci, col)
+    # edgeless graph, isolated sites, single colour: fine
+    g = B.xy_graph_load(np.zeros(5, np.int32), np.zeros(0, np.int32), np.zeros(4, np.int32))
+    assert B.xy_graph_info(g)["nnz_total"] == 0
+    B.xy_graph_free(g)
+    with pytest.raises(B.XYError):
+        B.xy_pt_create(None, [1.0], 1)
+
+
+def test_pt_create_rejects_bad_arguments():
+    gd = G.colour_major(6, G.ring_edges(6))
+    g = B.xy_graph_load(gd["row_ptr"], gd["col_idx"], gd["colour"])
+    for T in ([2.0, 1.0], [0.0, 1.0], [-1.0], [float("nan")], []):
+        with pytest.raises(B.XYError) as e:
+            B.xy_pt_create(g, T, 1)
+        assert e.value.code == B.XY_EINVAL
+    with pytest.raises(B.XYError):
+        B.xy_pt_create(g, [1.0], 1, sample_base=65536)
+    pt = B.xy_pt_create(g, [1.0, np.inf], 1)            # beta = 0 allowed; library-owned theta and stream
+    B.xy_run(pt, 2, 3, 1, 1)
+    th = B.xy_get_theta(pt, (1, 6, 2))
+    assert np.isfinite(th).all() and B.xy_theta_device(pt) != 0
+    with pytest.raises(B.XYError):
+        B.xy_set_labels(pt, np.array([[0, 0]], np.int32))
+    with pytest.raises(B.XYError):
+        B.xy_metropolis_colour(pt, 7, 1)
+    with pytest.raises(B.XYError):
+        B.xy_run(pt, 1, 0, 1, 1)
+    B.xy_pt_destroy(pt); B.xy_graph_free(g)
+
+
+def test_degenerate_graphs_isolated_sites_and_unequal_colour_counts():
+    """degree-0 sites: Metropolis always accepts (dE = 0), OR leaves them unchanged (DESIGN R3, R7);
+    samples with different numbers of colours in one batch."""
+    N = 8
+    e0 = [(0, 1), (1, 2), (2, 0), (3, 4)]             # triangle + bond + 3 isolated sites: 3 colours
+    e1 = [(0, 1), (2, 3), (4, 5)]                     # 2 colours
+    g0, g1 = G.colour_major(N, e0), G.colour_major(N, e1)
+    assert len(g0["class_ptr"]) - 1 == 3 and len(g1["class_ptr"]) - 1 == 2
+    nnz = max(len(g0["col_idx"]), len(g1["col_idx"]))
+    rp = np.stack([g0["row_ptr"], g1["row_ptr"]]); col = np.stack([g0["colour"], g1["colour"]])
+    ci = np.concatenate([g0["col_idx"], g1["col_idx"]])
+    T = np.array([0.5, 1.0, 2.0, 4.0])
+    ens = B.Ensemble(rp, ci, col, T, SEED)
+    graphs = [(g0["row_ptr"], g0["col_idx"], g0["class_ptr"]), (g1["row_ptr"], g1["col_idx"], g1["class_ptr"])]
+    for sweep in (1, 2):
+        for c in range(3):
+            st = U.lockstep_metropolis(ens, graphs, T, SEED, c, sweep)
+            assert st["bad"] == 0
+        for c in range(3):
+            pre = ens.get_theta()
+            st = U.lockstep_overrelax(ens, graphs, c)
+            assert st["bad"] == 0
+            post = ens.get_theta()
+            for s, gd in enumerate((g0, g1)):
+                iso = np.where(np.diff(gd["row_ptr"]) == 0)[0]
+                assert np.array_equal(post[s, iso], pre[s, iso])
+    ens.run(3, 5, 1, 1)
+    E = ens.get_energy(); th = ens.get_theta()
+    for s, gd in enumerate((g0, g1)):
+        Eo, _, _ = O.measure(gd["row_ptr"], gd["col_idx"], th[s])
+        assert np.allclose(E[s], Eo, atol=1e-5)
+    ens.close()
