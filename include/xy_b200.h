@@ -96,6 +96,11 @@ int xy_measure(xy_pt *pt, double *out_host);
  * sweeps_per_swap >= 1, or_per_sweep >= 0. */
 int xy_run(xy_pt *pt, int n_cycles, int sweeps_per_swap, int or_per_sweep, int measure_every);
 
+/* n_blocks x [ sweeps_per_block x (one Metropolis sweep + or_per_sweep OR sweeps) ], no measurement and no
+ * swap, in the same group schedule and from the same kind of captured graph as xy_run: the bare coloured
+ * Metropolis + over-relaxation sweep of SURVEY.md 8(d) "(A)".  sweep counter += n_blocks*sweeps_per_block. */
+int xy_run_sweeps(xy_pt *pt, int n_blocks, int sweeps_per_block, int or_per_sweep);
+
 /* Samples are independent, so a cycle may be executed for groups of `samples_per_group` samples at a
  * time (all sweeps of the cycle for group 0, then group 1, ...) to keep a group L2-resident; results
  * are bit-identical for every value.  0 = automatic (default), S = all samples per launch. */

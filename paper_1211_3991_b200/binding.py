@@ -31,6 +31,7 @@ SYMBOLS = {
     "xy_pt_swap": (C.c_int, [C.c_void_p]),
     "xy_measure": (C.c_int, [C.c_void_p, C.c_void_p]),
     "xy_run": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]),
+    "xy_run_sweeps": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int]),
     "xy_set_schedule": (C.c_int, [C.c_void_p, C.c_int]),
     "xy_metropolis_colour": (C.c_int, [C.c_void_p, C.c_int, C.c_uint32]),
     "xy_overrelax_colour": (C.c_int, [C.c_void_p, C.c_int]),
@@ -153,6 +154,10 @@ def xy_measure(pt, shape=None):
 
 def xy_run(pt, n_cycles, sweeps_per_swap=10, or_per_sweep=1, measure_every=1):
     _check(lib().xy_run(pt, n_cycles, sweeps_per_swap, or_per_sweep, measure_every))
+
+
+def xy_run_sweeps(pt, n_blocks, sweeps_per_block=10, or_per_sweep=1):
+    _check(lib().xy_run_sweeps(pt, n_blocks, sweeps_per_block, or_per_sweep))
 
 
 def xy_set_schedule(pt, samples_per_group):
@@ -281,6 +286,8 @@ class Ensemble:
     def measure(self, want=False): return xy_measure(self.pt, (self.S, self.R) if want else None)
     def run(self, n_cycles, sweeps_per_swap=10, or_per_sweep=1, measure_every=1):
         xy_run(self.pt, n_cycles, sweeps_per_swap, or_per_sweep, measure_every)
+    def run_sweeps(self, n_blocks, sweeps_per_block=10, or_per_sweep=1):
+        xy_run_sweeps(self.pt, n_blocks, sweeps_per_block, or_per_sweep)
     def set_schedule(self, g): xy_set_schedule(self.pt, g)
     def metropolis_colour(self, c, sweep): xy_metropolis_colour(self.pt, c, sweep)
     def overrelax_colour(self, c): xy_overrelax_colour(self.pt, c)

@@ -218,6 +218,53 @@ int issue_cycle(xy_pt *pt, int sps, int orps, int me, int phase, int group) {
     return launch_swap(pt, nullptr, static_cast<uint32_t>(sps));
 }
 
+// enqueue `sps` bare sweeps (Metropolis + orps x OR) per sample group, then advance the sweep counter
+int issue_sweeps(xy_pt *pt, int sps, int orps, int group) {
+    const int S = pt->g->S;
+    for (int s0 = 0; s0 < S; s0 += group) {
+        const int s1 = std::min(S, s0 + group);
+        for (int k = 1; k <= sps; ++k) {
+            int rc = sweep_group(pt, 0, s0, s1, true, k, 0u);
+            if (rc != XY_OK) return rc;
+            for (int o = 0; o < orps; ++o)
+                if ((rc = sweep_group(pt, 1, s0, s1, false, 0, 0u)) != XY_OK) return rc;
+        }
+    }
+    xy::k_tick<<<1, 1, 0, pt->stream>>>(pt->counters, static_cast<uint32_t>(sps), 0u);
+    XY_CUDA(cudaGetLastError());
+    pt->launches += 1;
+    return XY_OK;
+}
+
+// capture `issue` into an executable graph stored under `key` (or fetch it from the cache)
+template <typename F>
+int cached_graph(xy_pt *pt, const CycleKey &key, F issue, CycleGraph **out) {
+    auto it = pt->graphs.find(key);
+    if (it == pt->graphs.end()) {
+        if (pt->graphs.size() >= 32) {
+            for (auto &kv : pt->graphs)
+                if (kv.second.exec) cudaGraphExecDestroy(kv.second.exec);
+            pt->graphs.clear();
+        }
+        cudaGraph_t graph = nullptr;
+        const long long before = pt->launches;
+        XY_CUDA(cudaStreamBeginCapture(pt->stream, cudaStreamCaptureModeThreadLocal));
+        const int rc = issue();
+        const cudaError_t e = cudaStreamEndCapture(pt->stream, &graph);
+        CycleGraph cg;
+        cg.launches = pt->launches - before;
+        pt->launches = before;
+        if (rc != XY_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+        if (e != cudaSuccess) return fail(XY_ECUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(e));
+        const cudaError_t e2 = cudaGraphInstantiate(&cg.exec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (e2 != cudaSuccess) return fail(XY_ECUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e2));
+        it = pt->graphs.emplace(key, cg).first;
+    }
+    *out = &it->second;
+    return XY_OK;
+}
+
 void drop_graphs(xy_pt *pt) {
     for (auto &kv : pt->graphs)
         if (kv.second.exec) cudaGraphExecDestroy(kv.second.exec);
@@ -557,29 +604,31 @@ int xy_run(xy_pt *pt, int n_cycles, int sps, int orps, int me) {
     for (int c = 0; c < n_cycles; ++c) {
         const int phase = me > 0 ? static_cast<int>(pt->sweep % static_cast<uint32_t>(me)) : 0;
         const CycleKey key{sps, orps, me, phase, group};
-        auto it = pt->graphs.find(key);
-        if (it == pt->graphs.end()) {
-            if (pt->graphs.size() >= 32) drop_graphs(pt);
-            cudaGraph_t graph = nullptr;
-            const long long before = pt->launches;
-            XY_CUDA(cudaStreamBeginCapture(pt->stream, cudaStreamCaptureModeThreadLocal));
-            const int rc = issue_cycle(pt, sps, orps, me, phase, group);
-            const cudaError_t e = cudaStreamEndCapture(pt->stream, &graph);
-            CycleGraph cg;
-            cg.launches = pt->launches - before;
-            pt->launches = before;
-            if (rc != XY_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
-            if (e != cudaSuccess) return fail(XY_ECUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(e));
-            const cudaError_t e2 = cudaGraphInstantiate(&cg.exec, graph, 0);
-            cudaGraphDestroy(graph);
-            if (e2 != cudaSuccess) return fail(XY_ECUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e2));
-            it = pt->graphs.emplace(key, cg).first;
-        }
-        XY_CUDA(cudaGraphLaunch(it->second.exec, pt->stream));
-        pt->launches += it->second.launches;
+        CycleGraph *cg = nullptr;
+        const int rc = cached_graph(pt, key, [&] { return issue_cycle(pt, sps, orps, me, phase, group); }, &cg);
+        if (rc != XY_OK) return rc;
+        XY_CUDA(cudaGraphLaunch(cg->exec, pt->stream));
+        pt->launches += cg->launches;
         pt->sweep += static_cast<uint32_t>(sps);
         pt->round += 1;
         pt->e_fresh = false;  // labels moved; E per slot is still valid but keep the rule simple
+    }
+    return XY_OK;
+}
+
+int xy_run_sweeps(xy_pt *pt, int n_blocks, int sps, int orps) {
+    if (!check_pt(pt) || n_blocks < 0 || sps < 1 || orps < 0)
+        return fail(XY_EINVAL, "need n_blocks >= 0, sweeps_per_block >= 1, or_per_sweep >= 0");
+    const int group = auto_group(pt);
+    for (int b = 0; b < n_blocks; ++b) {
+        const CycleKey key{sps, orps, -1, 0, group};
+        CycleGraph *cg = nullptr;
+        const int rc = cached_graph(pt, key, [&] { return issue_sweeps(pt, sps, orps, group); }, &cg);
+        if (rc != XY_OK) return rc;
+        XY_CUDA(cudaGraphLaunch(cg->exec, pt->stream));
+        pt->launches += cg->launches;
+        pt->sweep += static_cast<uint32_t>(sps);
+        pt->e_fresh = false;
     }
     return XY_OK;
 }
