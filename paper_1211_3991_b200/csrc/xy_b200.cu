@@ -79,12 +79,16 @@ struct xy_pt {
     double *betaT = nullptr;
     int32_t *temp_of_slot = nullptr, *slot_of_temp = nullptr;
     uint32_t *counters = nullptr;
-    double *E_slot = nullptr, *M_slot = nullptr, *partial = nullptr, *acc = nullptr;
+    double *E_slot = nullptr, *M_slot = nullptr, *acc = nullptr;
+    long long *fx = nullptr;            // [S][R][3] fixed-point measure sums (zero between launches)
+    unsigned int *ticket = nullptr;     // [S]
     long long *attempts = nullptr, *accepts = nullptr;
     uint8_t *decisions = nullptr;
-    int n_chunks = 1, chunk_sites = 1;
+    xy::PhiloxKeys keys;
     int fast_G = 0;  // lanes per site of the float2 path, 0 = generic kernel
     int col_blocks = 1;
+    int measure_tpw = 1;      // tiles per warp of the measure launch: a function of N and R only
+    int measure_chunk = 256;  // sites per CTA of the generic measure kernel
     int samples_per_group = 0;  // 0 = automatic
     // host mirrors
     uint32_t sweep = 0, round = 0;
@@ -107,36 +111,54 @@ int max_class_size(const xy_graph *g, int colour, int s0, int s1) {
     return m;
 }
 
+xy::TileArgs tile_args(const xy_pt *pt, int colour, int s0) {
+    const xy_graph *g = pt->g;
+    xy::TileArgs a;
+    a.rec = g->rec; a.col_idx = g->col_idx; a.class_ptr = g->class_ptr; a.theta = pt->theta;
+    a.beta_slot = pt->beta_slot; a.w_slot = pt->w_slot; a.counters = pt->counters;
+    a.N = g->N; a.R = pt->R; a.q_stride = g->q_stride; a.colour = colour; a.s0 = s0; a.tiles_per_warp = 1;
+    a.sweep_fixed = 0u; a.sweep_offset = 0; a.use_counter = 0;
+    a.sample_base = pt->sample_base; a.keys = pt->keys;
+    a.fx = pt->fx; a.ticket = pt->ticket; a.temp_of_slot = pt->temp_of_slot;
+    a.E_slot = pt->E_slot; a.M_slot = pt->M_slot; a.acc = pt->acc; a.accumulate = 0;
+    return a;
+}
+
+// sites per tile of the float2 path with G lanes per site (mirrors k_tile)
+int tile_sites(int G) { return (G < 8 ? G : 8) * (32 / G); }
+
+template <int MODE>
+void launch_tile_kernel(int G, int col_blocks, dim3 grid, cudaStream_t st, const xy::TileArgs &a) {
+    const dim3 block(xy::kBlock);
+    switch (G) {
+        case 32:
+            if (col_blocks == 1) xy::k_tile<32, 1, MODE><<<grid, block, 0, st>>>(a);
+            else xy::k_tile<32, 0, MODE><<<grid, block, 0, st>>>(a);
+            break;
+        case 16: xy::k_tile<16, 1, MODE><<<grid, block, 0, st>>>(a); break;
+        case 8: xy::k_tile<8, 1, MODE><<<grid, block, 0, st>>>(a); break;
+        case 4: xy::k_tile<4, 1, MODE><<<grid, block, 0, st>>>(a); break;
+        case 2: xy::k_tile<2, 1, MODE><<<grid, block, 0, st>>>(a); break;
+        default: xy::k_tile<1, 1, MODE><<<grid, block, 0, st>>>(a); break;
+    }
+}
+
 template <int MODE>
 int launch_class(xy_pt *pt, int colour, int s0, int s1, bool use_counter, int sweep_offset, uint32_t sweep_fixed) {
     const xy_graph *g = pt->g;
     const int nmax = max_class_size(g, colour, s0, s1);
     if (nmax == 0 || s1 <= s0) return XY_OK;
-    xy::ClassArgs a;
-    a.rec = g->rec; a.col_idx = g->col_idx; a.class_ptr = g->class_ptr; a.theta = pt->theta;
-    a.beta_slot = pt->beta_slot; a.w_slot = pt->w_slot; a.counters = pt->counters;
-    a.N = g->N; a.R = pt->R; a.q_stride = g->q_stride; a.colour = colour; a.s0 = s0;
+    xy::TileArgs a = tile_args(pt, colour, s0);
     a.sweep_fixed = sweep_fixed; a.sweep_offset = sweep_offset; a.use_counter = use_counter ? 1 : 0;
-    a.key0 = pt->key0; a.key1 = pt->key1; a.sample_base = pt->sample_base;
-
     const int G = pt->fast_G;
-    const int spw = G ? 32 / G : 1;
-    const long long groups = (nmax + spw - 1) / spw;                       // warp tasks per sample
-    const long long total = groups * (s1 - s0) * pt->col_blocks;
-    // enough warps for ~2 full waves of 148 SMs x 48 warps, at most 16 site groups per warp
-    int chunk = static_cast<int>(std::min<long long>(16, std::max<long long>(1, total / (148 * 48 * 2))));
-    a.chunk = chunk;
-    dim3 grid(ceil_div(ceil_div(groups, chunk), xy::kWarps), s1 - s0, pt->col_blocks);
-    dim3 block(xy::kBlock);
-    switch (G) {
-        case 32: xy::k_update_class<32, MODE><<<grid, block, 0, pt->stream>>>(a); break;
-        case 16: xy::k_update_class<16, MODE><<<grid, block, 0, pt->stream>>>(a); break;
-        case 8: xy::k_update_class<8, MODE><<<grid, block, 0, pt->stream>>>(a); break;
-        case 4: xy::k_update_class<4, MODE><<<grid, block, 0, pt->stream>>>(a); break;
-        case 2: xy::k_update_class<2, MODE><<<grid, block, 0, pt->stream>>>(a); break;
-        case 1: xy::k_update_class<1, MODE><<<grid, block, 0, pt->stream>>>(a); break;
-        default: xy::k_update_class_generic<MODE><<<grid, block, 0, pt->stream>>>(a); break;
-    }
+    const int ts = G ? tile_sites(G) : 1;
+    const long long tiles = (nmax + ts - 1) / ts;                          // warp tasks per sample
+    const long long total = tiles * (s1 - s0) * pt->col_blocks;
+    // enough warps for ~3 full waves of 148 SMs x 32 resident warps, at most 8 tiles per warp
+    a.tiles_per_warp = static_cast<int>(std::min<long long>(8, std::max<long long>(1, total / (148 * 32 * 3))));
+    const dim3 grid(ceil_div(ceil_div(tiles, a.tiles_per_warp), xy::kWarps), s1 - s0, pt->col_blocks);
+    if (G) launch_tile_kernel<MODE>(G, pt->col_blocks, grid, pt->stream, a);
+    else xy::k_update_class_generic<MODE><<<grid, xy::kBlock, 0, pt->stream>>>(a);
     XY_CUDA(cudaGetLastError());
     pt->launches += 1;
     return XY_OK;
@@ -145,18 +167,20 @@ int launch_class(xy_pt *pt, int colour, int s0, int s1, bool use_counter, int sw
 int launch_measure(xy_pt *pt, int s0, int s1, bool accumulate) {
     const xy_graph *g = pt->g;
     if (s1 <= s0) return XY_OK;
-    xy::MeasureArgs m;
-    m.rec = g->rec; m.col_idx = g->col_idx; m.theta = pt->theta; m.partial = pt->partial;
-    m.N = g->N; m.R = pt->R; m.s0 = s0; m.n_chunks = pt->n_chunks; m.chunk_sites = pt->chunk_sites;
-    const size_t smem = static_cast<size_t>(xy::kWarps) * pt->R * 3 * sizeof(double);
-    xy::k_measure_partial<<<dim3(pt->n_chunks, s1 - s0), xy::kBlock, smem, pt->stream>>>(m);
+    xy::TileArgs a = tile_args(pt, 0, s0);
+    a.accumulate = accumulate ? 1 : 0;
+    const int G = pt->fast_G;
+    if (G) {
+        const long long tiles = (g->N + tile_sites(G) - 1) / tile_sites(G);
+        a.tiles_per_warp = pt->measure_tpw;
+        const dim3 grid(ceil_div(ceil_div(tiles, a.tiles_per_warp), xy::kWarps), s1 - s0, pt->col_blocks);
+        launch_tile_kernel<xy::kModeMeasure>(G, pt->col_blocks, grid, pt->stream, a);
+    } else {
+        const dim3 grid(ceil_div(g->N, pt->measure_chunk), s1 - s0);
+        xy::k_measure_generic<<<grid, xy::kBlock, 0, pt->stream>>>(a, pt->measure_chunk);
+    }
     XY_CUDA(cudaGetLastError());
-    const int n = (s1 - s0) * pt->R;
-    xy::k_measure_final<<<ceil_div(n, 128), 128, 0, pt->stream>>>(pt->partial, s0, s1, g->N, pt->R, pt->n_chunks,
-                                                               pt->temp_of_slot, pt->E_slot, pt->M_slot, pt->acc,
-                                                               accumulate ? 1 : 0);
-    XY_CUDA(cudaGetLastError());
-    pt->launches += 2;
+    pt->launches += 1;
     return XY_OK;
 }
 
@@ -166,7 +190,7 @@ int launch_swap(xy_pt *pt, const uint8_t *decisions_dev, uint32_t d_sweep) {
     a.slot_of_temp = pt->slot_of_temp; a.temp_of_slot = pt->temp_of_slot;
     a.beta_slot = pt->beta_slot; a.w_slot = pt->w_slot; a.counters = pt->counters; a.decisions = decisions_dev;
     a.attempts = pt->attempts; a.accepts = pt->accepts; a.R = pt->R;
-    a.key0 = pt->key0; a.key1 = pt->key1; a.sample_base = pt->sample_base;
+    a.keys = pt->keys; a.sample_base = pt->sample_base;
     xy::k_pt_swap<<<pt->g->S, 128, 0, pt->stream>>>(a);
     XY_CUDA(cudaGetLastError());
     xy::k_tick<<<1, 1, 0, pt->stream>>>(pt->counters, d_sweep, 1u);
@@ -296,6 +320,7 @@ int xy_graph_load(int S, int N, const int32_t *row_ptr, const int32_t *col_idx, 
             for (int i = 0; i < N; ++i) {
                 if (rp[i + 1] < rp[i]) return fail(XY_EGRAPH, "row_ptr not monotone (sample " + std::to_string(s) + ")");
                 max_deg = std::max(max_deg, rp[i + 1] - rp[i]);
+                if (rp[i + 1] - rp[i] > 0xffff) return fail(XY_EGRAPH, "degree exceeds 65535 (sample " + std::to_string(s) + ")");
             }
             off[s + 1] = off[s] + rp[N];
         }
@@ -339,13 +364,19 @@ int xy_graph_load(int S, int N, const int32_t *row_ptr, const int32_t *col_idx, 
         g->stream = static_cast<cudaStream_t>(stream);
         g->bytes_per_sample = static_cast<size_t>(off[S] / S) * 4 + static_cast<size_t>(N) * 8;
         std::vector<int2> h_rec(static_cast<size_t>(S) * N);
+        std::vector<int32_t> h_col(static_cast<size_t>(off[S]));   // neighbour lists, ascending per site
         g->h_class_ptr.assign(static_cast<size_t>(S) * g->q_stride, 0);
         for (int s = 0; s < S; ++s) {
             const int32_t *rp = row_ptr + static_cast<size_t>(s) * (N + 1);
             const int32_t *col = colour + static_cast<size_t>(s) * N;
             int32_t *cp = g->h_class_ptr.data() + static_cast<size_t>(s) * g->q_stride;
             for (int i = 0; i < N; ++i) {
-                h_rec[static_cast<size_t>(s) * N + i] = make_int2(static_cast<int>(off[s] + rp[i]), rp[i + 1] - rp[i]);
+                int32_t *dst = h_col.data() + off[s] + rp[i];
+                const int deg = rp[i + 1] - rp[i];
+                std::copy(col_idx + off[s] + rp[i], col_idx + off[s] + rp[i + 1], dst);
+                std::sort(dst, dst + deg);
+                const int n_lower = static_cast<int>(std::lower_bound(dst, dst + deg, i) - dst);
+                h_rec[static_cast<size_t>(s) * N + i] = make_int2(static_cast<int>(off[s] + rp[i]), deg | (n_lower << 16));
                 cp[col[i] + 1]++;
             }
             for (int c = 0; c < q_max; ++c) cp[c + 1] += cp[c];
@@ -358,7 +389,7 @@ int xy_graph_load(int S, int N, const int32_t *row_ptr, const int32_t *col_idx, 
         }
         cudaError_t e = cudaMemcpyAsync(g->rec, h_rec.data(), h_rec.size() * sizeof(int2), cudaMemcpyHostToDevice, g->stream);
         if (e == cudaSuccess && off[S] > 0)
-            e = cudaMemcpyAsync(g->col_idx, col_idx, off[S] * sizeof(int32_t), cudaMemcpyHostToDevice, g->stream);
+            e = cudaMemcpyAsync(g->col_idx, h_col.data(), off[S] * sizeof(int32_t), cudaMemcpyHostToDevice, g->stream);
         if (e == cudaSuccess)
             e = cudaMemcpyAsync(g->class_ptr, g->h_class_ptr.data(), g->h_class_ptr.size() * sizeof(int32_t),
                                 cudaMemcpyHostToDevice, g->stream);
@@ -427,9 +458,19 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
     pt->fast_G = 0; pt->col_blocks = 1;
     if (R % 64 == 0) { pt->fast_G = 32; pt->col_blocks = R / 64; }
     else if (R % 2 == 0 && R / 2 <= 32 && ((R / 2) & (R / 2 - 1)) == 0) pt->fast_G = R / 2;
-    // measure partition: a function of N only, so results do not depend on the schedule
-    pt->chunk_sites = std::max(256, ((N + 127) / 128 + 7) / 8 * 8);
-    pt->n_chunks = (N + pt->chunk_sites - 1) / pt->chunk_sites;
+    if (static_cast<long long>(N) * ((R + 1) / 2) > 0x7fffffffll) {
+        if (pt->owns_stream) cudaStreamDestroy(pt->stream);
+        delete pt;
+        return fail(XY_EINVAL, "N * R / 2 must fit in int32 (offsets inside a sample are 32-bit)");
+    }
+    pt->keys = xy::philox_key_schedule(pt->key0, pt->key1);
+    // measure partition: a function of N and R only, so results do not depend on the schedule
+    {
+        const int ts = pt->fast_G ? tile_sites(pt->fast_G) : 1;
+        const long long tiles = (N + ts - 1) / ts;
+        pt->measure_tpw = static_cast<int>(std::min<long long>(16, std::max<long long>(1, tiles / 4096)));
+        pt->measure_chunk = std::max(256, ((N + 127) / 128 + 7) / 8 * 8);
+    }
 
     const size_t SR = static_cast<size_t>(S) * R;
     int rc = XY_OK;
@@ -441,21 +482,9 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
     A(dev_alloc(&pt->temp_of_slot, SR)); A(dev_alloc(&pt->slot_of_temp, SR));
     A(dev_alloc(&pt->counters, 2));
     A(dev_alloc(&pt->E_slot, SR)); A(dev_alloc(&pt->M_slot, SR * 2));
-    A(dev_alloc(&pt->partial, SR * pt->n_chunks * 3)); A(dev_alloc(&pt->acc, SR * XY_NACC));
+    A(dev_alloc(&pt->fx, SR * 3)); A(dev_alloc(&pt->ticket, S)); A(dev_alloc(&pt->acc, SR * XY_NACC));
     A(dev_alloc(&pt->attempts, SR)); A(dev_alloc(&pt->accepts, SR)); A(dev_alloc(&pt->decisions, SR));
     if (rc != XY_OK) { xy_pt_destroy(pt); return rc; }
-    {
-        const size_t smem = static_cast<size_t>(xy::kWarps) * R * 3 * sizeof(double);
-        if (smem > 48 * 1024) {
-            const cudaError_t ea = cudaFuncSetAttribute(xy::k_measure_partial, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                        static_cast<int>(smem));
-            if (ea != cudaSuccess) {
-                xy_pt_destroy(pt);
-                return fail(XY_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(ea));
-            }
-        }
-    }
-
     std::vector<float> hb(R), hw(R);
     std::vector<double> hbT(R);
     std::vector<int32_t> lab(SR);
@@ -475,10 +504,12 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
     if (e == cudaSuccess) e = cudaMemsetAsync(pt->attempts, 0, SR * sizeof(long long), pt->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(pt->accepts, 0, SR * sizeof(long long), pt->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(pt->E_slot, 0, SR * sizeof(double), pt->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(pt->fx, 0, SR * 3 * sizeof(long long), pt->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(pt->ticket, 0, S * sizeof(unsigned int), pt->stream);
     if (e == cudaSuccess) {
         xy::k_refresh_slot_params<<<ceil_div(SR, 128), 128, 0, pt->stream>>>(pt->temp_of_slot, pt->slot_of_temp, pt->beta_f,
                                                                             pt->w_f, pt->beta_slot, pt->w_slot, S, R);
-        xy::k_init_theta<<<148 * 8, 256, 0, pt->stream>>>(pt->theta, S, N, R, pt->key0, pt->key1, pt->sample_base);
+        xy::k_init_theta<<<148 * 8, 256, 0, pt->stream>>>(pt->theta, S, N, R, pt->keys, pt->sample_base);
         pt->launches += 2;
         e = cudaGetLastError();
     }
@@ -498,7 +529,7 @@ int xy_pt_destroy(xy_pt *pt) {
     if (pt->owns_theta) cudaFree(pt->theta);
     cudaFree(pt->beta_slot); cudaFree(pt->w_slot); cudaFree(pt->beta_f); cudaFree(pt->w_f); cudaFree(pt->betaT);
     cudaFree(pt->temp_of_slot); cudaFree(pt->slot_of_temp); cudaFree(pt->counters);
-    cudaFree(pt->E_slot); cudaFree(pt->M_slot); cudaFree(pt->partial); cudaFree(pt->acc);
+    cudaFree(pt->E_slot); cudaFree(pt->M_slot); cudaFree(pt->fx); cudaFree(pt->ticket); cudaFree(pt->acc);
     cudaFree(pt->attempts); cudaFree(pt->accepts); cudaFree(pt->decisions);
     if (pt->owns_stream) cudaStreamDestroy(pt->stream);
     delete pt;

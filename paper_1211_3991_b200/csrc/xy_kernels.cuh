@@ -2,9 +2,16 @@
 //
 // Layout: theta[S][N][R] fp32, replica (slot) fastest.  A lane owns TWO adjacent slots (one float2 and
 // one Philox4x32-10 call per site: words (x0,x1) feed the even slot, (x2,x3) the odd one), so a group of
-// G = R/2 lanes covers one site and a warp covers 32/G sites.  At R = 64 a warp gathers one neighbour as
-// one 256-byte coalesced request.  The neighbour ids of a site are fetched with ONE coalesced load
-// (lane l takes col_idx[start + l]) and broadcast with shuffles.
+// G = R/2 lanes covers one site and a warp covers SPW = 32/G sites at once.  At R = 64 a warp gathers one
+// neighbour as one 256-byte coalesced request.
+//
+// Work unit = a TILE of TS = CH*SPW consecutive sites of one colour class, owned by one warp:
+//   1. lane m < TS loads rec[i0+m] = {first col_idx entry, degree | n_lower<<16}      (one coalesced load)
+//   2. the tile's neighbour ids are one contiguous run of col_idx (CSR order): staged into the warp's
+//      slice of shared memory with coalesced loads, read back as broadcast LDS
+//   3. row t = sites i0 + t*SPW + sub: own float2, Philox, gather, finish, store.  When SPW == 1 the
+//      degree is warp-uniform and the gather runs exact-degree batches (no predicated-off issue slots).
+// All offsets inside a sample are 32-bit (N*R/2 < 2^31 is checked at xy_pt_create).
 //
 // PAPER.md:444,:454 (coloured single-spin Metropolis), :460 (over-relaxation, ref 66), :167-181 (E, m),
 // :460-472 (parallel tempering); readings R5-R11 in DESIGN.md.
@@ -18,26 +25,42 @@ constexpr float kTwoPiF = 6.2831855f;           // fp32(2 pi)
 constexpr float kTwoPiLo = -1.7484555e-7f;      // 2 pi - fp32(2 pi)
 constexpr float kInvTwoPiF = 0.15915494f;
 constexpr unsigned kFull = 0xffffffffu;
-constexpr int kBlock = 256;                     // threads per CTA in the class kernels
+constexpr int kBlock = 256;                     // threads per CTA in the tile kernels
 constexpr int kWarps = kBlock / 32;
+constexpr int kIdxCap = 192;                    // staged neighbour ids per warp (ints); longer runs read global
+constexpr double kFix = 68719476736.0;          // 2^36: fixed-point scale of the measure reduction
+constexpr double kInvFix = 1.0 / 68719476736.0;
 
 enum : uint32_t { kDomInit = 0u, kDomMetropolis = 1u, kDomSwap = 2u };
+enum : int { kModeMetropolis = 0, kModeOverrelax = 1, kModeMeasure = 2 };
 
 // ---- Philox4x32-10 (Salmon et al., SC'11), written from the round function -------------------------
+// ks[2r], ks[2r+1] = the round keys k0 + r W0, k1 + r W1 (W0 = 0x9E3779B9, W1 = 0xBB67AE85)
+struct PhiloxKeys { uint32_t ks[20]; };
+
+__host__ __device__ inline PhiloxKeys philox_key_schedule(uint32_t k0, uint32_t k1) {
+    PhiloxKeys k;
+    for (int r = 0; r < 10; ++r) {
+        k.ks[2 * r] = k0;
+        k.ks[2 * r + 1] = k1;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    return k;
+}
+
 __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
-                                              uint32_t k0, uint32_t k1, uint32_t (&x)[4]) {
+                                              const PhiloxKeys &k, uint32_t (&x)[4]) {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
         const unsigned long long p0 = static_cast<unsigned long long>(0xD2511F53u) * c0;
         const unsigned long long p1 = static_cast<unsigned long long>(0xCD9E8D57u) * c2;
-        const uint32_t n0 = static_cast<uint32_t>(p1 >> 32) ^ c1 ^ k0;
-        const uint32_t n2 = static_cast<uint32_t>(p0 >> 32) ^ c3 ^ k1;
+        const uint32_t n0 = static_cast<uint32_t>(p1 >> 32) ^ c1 ^ k.ks[2 * r];
+        const uint32_t n2 = static_cast<uint32_t>(p0 >> 32) ^ c3 ^ k.ks[2 * r + 1];
         c1 = static_cast<uint32_t>(p1);
         c3 = static_cast<uint32_t>(p0);
         c0 = n0;
         c2 = n2;
-        k0 += 0x9E3779B9u;
-        k1 += 0xBB67AE85u;
     }
     x[0] = c0; x[1] = c1; x[2] = c2; x[3] = c3;
 }
@@ -47,19 +70,26 @@ __device__ __forceinline__ float u01(uint32_t x) {
     return fmaf(static_cast<float>(x >> 9), 1.1920928955078125e-07f, 5.9604644775390625e-08f);
 }
 
-// ---- arguments shared by the per-colour kernels ------------------------------------------------------
-struct ClassArgs {
-    const int2 *rec;           // [S][N] {first col_idx entry (absolute), degree}
-    const int32_t *col_idx;    // concatenated neighbour ids (local to the sample)
+// ---- arguments of the tile kernels -----------------------------------------------------------------
+struct TileArgs {
+    const int2 *rec;           // [S][N] {first col_idx entry (absolute), degree | n_lower << 16}
+    const int32_t *col_idx;    // concatenated neighbour ids (local to the sample), ascending per site
     const int32_t *class_ptr;  // [S][q_stride]
     float *theta;              // [S][N][R]
     const float *beta_slot;    // [S][R]
     const float *w_slot;       // [S][R]
     const uint32_t *counters;  // device {sweep, round}
-    int N, R, q_stride, colour, s0, chunk;  // chunk = site groups per warp
+    int N, R, q_stride, colour, s0, tiles_per_warp;
     uint32_t sweep_fixed;
     int sweep_offset, use_counter;
-    uint32_t key0, key1, sample_base;
+    uint32_t sample_base;
+    PhiloxKeys keys;
+    // measure only
+    long long *fx;             // [S][R][3] fixed-point sums (E, Mx, My), zero between launches
+    unsigned int *ticket;      // [S] CTAs done, zero between launches
+    const int32_t *temp_of_slot;
+    double *E_slot, *M_slot, *acc;
+    int accumulate;
 };
 
 // Metropolis for one slot given the sum over neighbours of sin(mid - theta_j):
@@ -86,123 +116,286 @@ __device__ __forceinline__ float overrelax_finish(float own, float hx, float hy)
     return t;
 }
 
-// ---- fast path: R = 2 G (G a power of two <= 32) or R a multiple of 64 (G = 32, blockIdx.z = column block)
-// MODE 0 = Metropolis, 1 = over-relaxation.
-template <int G, int MODE>
-__global__ void __launch_bounds__(kBlock) k_update_class(const ClassArgs a) {
-    constexpr int SPW = 32 / G;              // sites per warp
-    constexpr int UNR = G < 8 ? G : 8;       // neighbour gathers issued back to back
+// ---- per-lane state of one row (two slots) ------------------------------------------------------------
+template <int MODE> struct RowAcc;
+
+template <> struct RowAcc<kModeMetropolis> {
+    float midx, midy, ax = 0.f, ay = 0.f;
+    __device__ __forceinline__ void add(const float2 t) {
+        ax += __sinf(midx - t.x);
+        ay += __sinf(midy - t.y);
+    }
+};
+template <> struct RowAcc<kModeOverrelax> {
+    float hxx = 0.f, hyx = 0.f, hxy = 0.f, hyy = 0.f;   // (hxx, hyx) = field of the .x slot
+    __device__ __forceinline__ void add(const float2 t) {
+        float sn, cs;
+        __sincosf(t.x, &sn, &cs);
+        hxx += cs; hyx += sn;
+        __sincosf(t.y, &sn, &cs);
+        hxy += cs; hyy += sn;
+    }
+};
+template <> struct RowAcc<kModeMeasure> {
+    float ownx, owny, ex = 0.f, ey = 0.f;
+    __device__ __forceinline__ void add(const float2 t) {
+        ex += __cosf(ownx - t.x);
+        ey += __cosf(owny - t.y);
+    }
+};
+
+// neighbour id k of the run: staged copy (broadcast LDS) or, for over-long runs, global
+__device__ __forceinline__ int nbr_id(const int32_t *sidx, const int32_t *gidx, bool staged, int pos) {
+    return staged ? sidx[pos] : __ldg(gidx + pos);
+}
+
+// exact-degree gather for warp-uniform degree: D loads back to back, then D accumulations
+template <int D, typename ACC>
+__device__ __forceinline__ void gather_batch(ACC &acc, const float2 *__restrict__ base_q, uint32_t stride,
+                                             const int32_t *sidx, const int32_t *gidx, bool staged, int pos) {
+    float2 t[D];
+#pragma unroll
+    for (int u = 0; u < D; ++u) {
+        const uint32_t j = static_cast<uint32_t>(nbr_id(sidx, gidx, staged, pos + u));
+        t[u] = base_q[j * stride];
+    }
+#pragma unroll
+    for (int u = 0; u < D; ++u) acc.add(t[u]);
+}
+
+template <typename ACC>
+__device__ __forceinline__ void gather_uniform(ACC &acc, const float2 *__restrict__ base_q, uint32_t stride,
+                                               const int32_t *sidx, const int32_t *gidx, bool staged, int pos,
+                                               int cnt) {
+    while (cnt >= 8) {
+        gather_batch<8>(acc, base_q, stride, sidx, gidx, staged, pos);
+        pos += 8; cnt -= 8;
+    }
+    switch (cnt) {
+        case 7: gather_batch<7>(acc, base_q, stride, sidx, gidx, staged, pos); break;
+        case 6: gather_batch<6>(acc, base_q, stride, sidx, gidx, staged, pos); break;
+        case 5: gather_batch<5>(acc, base_q, stride, sidx, gidx, staged, pos); break;
+        case 4: gather_batch<4>(acc, base_q, stride, sidx, gidx, staged, pos); break;
+        case 3: gather_batch<3>(acc, base_q, stride, sidx, gidx, staged, pos); break;
+        case 2: gather_batch<2>(acc, base_q, stride, sidx, gidx, staged, pos); break;
+        case 1: gather_batch<1>(acc, base_q, stride, sidx, gidx, staged, pos); break;
+        default: break;
+    }
+}
+
+// several sites per warp: degrees differ between the lane groups; run to the warp maximum, absent
+// neighbours are replaced by a harmless in-range load and left out of the sum
+template <typename ACC>
+__device__ __forceinline__ void gather_divergent(ACC &acc, const float2 *__restrict__ base_q, uint32_t stride,
+                                                 const int32_t *sidx, const int32_t *gidx, bool staged, int pos,
+                                                 int cnt, int cntmax, uint32_t safe_site) {
+    for (int k = 0; k < cntmax; k += 4) {
+        float2 t[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            uint32_t j = safe_site;
+            if (k + u < cnt) j = static_cast<uint32_t>(nbr_id(sidx, gidx, staged, pos + k + u));
+            t[u] = base_q[j * stride];
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            ACC trial = acc;
+            trial.add(t[u]);
+            if (k + u < cnt) acc = trial;
+        }
+    }
+}
+
+// ---- the tile kernel: MODE 0 Metropolis / 1 over-relaxation on one colour class, 2 measure on all sites ----
+// R = 2G (G a power of two <= 32, CB = 1: stride known at compile time) or R a multiple of 64 (G = 32,
+// CB = 0: blockIdx.z = block of 64 slots).
+template <int G, int CB, int MODE>
+__global__ void __launch_bounds__(kBlock) k_tile(const TileArgs a) {
+    constexpr int SPW = 32 / G;                 // sites per row
+    constexpr int CH = G < 8 ? G : 8;           // rows per tile
+    constexpr int TS = CH * SPW;                // sites per tile (<= 32)
+    __shared__ int32_t s_idx[kWarps][kIdxCap];
+    __shared__ double s_red[MODE == kModeMeasure ? kWarps * 32 * 6 : 1];
+    __shared__ int s_last;
+
     const int s = a.s0 + blockIdx.y;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int sub = lane / G, l = lane % G;
-    const int R2 = a.R >> 1;
-    const int q = blockIdx.z * G + l;        // slot pair handled by this lane
+    const uint32_t R2 = CB ? static_cast<uint32_t>(G) : static_cast<uint32_t>(a.R >> 1);
+    const int q = blockIdx.z * G + l;            // slot pair handled by this lane
 
-    const int cbeg = a.class_ptr[s * a.q_stride + a.colour];
-    const int cend = a.class_ptr[s * a.q_stride + a.colour + 1];
-    const int n_groups = (cend - cbeg + SPW - 1) / SPW;
-    const int g0 = (blockIdx.x * kWarps + warp) * a.chunk;
-    if (g0 >= n_groups) return;
-    const int g1 = min(g0 + a.chunk, n_groups);
+    int cbeg = 0, cend = a.N;
+    if constexpr (MODE != kModeMeasure) {
+        cbeg = a.class_ptr[s * a.q_stride + a.colour];
+        cend = a.class_ptr[s * a.q_stride + a.colour + 1];
+    }
+    const int n_tiles = (cend - cbeg + TS - 1) / TS;
+    const int tile0 = (blockIdx.x * kWarps + warp) * a.tiles_per_warp;
+    const int tile1 = min(tile0 + a.tiles_per_warp, n_tiles);
 
-    float2 *__restrict__ th2 = reinterpret_cast<float2 *>(a.theta) + static_cast<size_t>(s) * a.N * R2;
+    float2 *__restrict__ base_q = reinterpret_cast<float2 *>(a.theta) + static_cast<size_t>(s) * a.N * R2 + q;
     const int2 *__restrict__ rec = a.rec + static_cast<size_t>(s) * a.N;
+    int32_t *sidx = s_idx[warp];
 
     float2 beta = make_float2(0.f, 0.f), w = make_float2(0.f, 0.f);
     uint32_t sweep = 0, c2 = 0;
-    if (MODE == 0) {
+    if constexpr (MODE == kModeMetropolis) {
         beta = reinterpret_cast<const float2 *>(a.beta_slot)[static_cast<size_t>(s) * R2 + q];
         w = reinterpret_cast<const float2 *>(a.w_slot)[static_cast<size_t>(s) * R2 + q];
         sweep = a.use_counter ? a.counters[0] + static_cast<uint32_t>(a.sweep_offset) : a.sweep_fixed;
         c2 = ((a.sample_base + static_cast<uint32_t>(s)) << 16) | static_cast<uint32_t>(q);
     }
+    double dacc[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};   // measure: E, Mx, My of the .x slot, then of the .y slot
 
-    for (int g = g0; g < g1; ++g) {
-        const int i = cbeg + g * SPW + sub;
-        const bool valid = i < cend;
+    for (int tile = tile0; tile < tile1; ++tile) {
+        const int i0 = cbeg + tile * TS;
+        const int nsite = min(TS, cend - i0);
         int2 rc = make_int2(0, 0);
-        if (valid) rc = rec[i];
-        const int deg = rc.y;
-        const int degmax = (SPW == 1) ? deg : __reduce_max_sync(kFull, deg);
-        float2 own = make_float2(0.f, 0.f);
-        if (valid) own = th2[static_cast<size_t>(i) * R2 + q];
+        if (lane < nsite) rc = rec[i0 + lane];
+        const int start0 = __shfl_sync(kFull, rc.x, 0);
+        const int n_run = __shfl_sync(kFull, rc.x + (rc.y & 0xffff), nsite - 1) - start0;
+        const bool staged = n_run <= kIdxCap;
+        const int32_t *gidx = a.col_idx + start0;
+        if (staged)
+            for (int p = lane; p < n_run; p += 32) sidx[p] = gidx[p];
+        __syncwarp();
 
-        // per-slot state: Metropolis (mid-angle, half-step, sum of sines) or OR (hx, hy)
-        float midx = 0.f, midy = 0.f, halfx = 0.f, halfy = 0.f, thpx = 0.f, thpy = 0.f;
-        float u2x = 0.f, u2y = 0.f;
-        float ax = 0.f, ay = 0.f, bx = 0.f, by = 0.f;   // MET: ax, ay = sine sums; OR: (ax,bx) = h of .x slot
-        if (MODE == 0) {
-            uint32_t x[4];
-            philox4x32_10(static_cast<uint32_t>(i), sweep, c2, kDomMetropolis, a.key0, a.key1, x);
-            const float dx = __fmul_rn(w.x, u01(x[0]) - 0.5f);
-            const float dy = __fmul_rn(w.y, u01(x[2]) - 0.5f);
-            u2x = u01(x[1]);
-            u2y = u01(x[3]);
-            thpx = __fadd_rn(own.x, dx);
-            thpy = __fadd_rn(own.y, dy);
-            halfx = 0.5f * (thpx - own.x);
-            halfy = 0.5f * (thpy - own.y);
-            midx = own.x + halfx;
-            midy = own.y + halfy;
-        }
-
-        for (int base = 0; base < degmax; base += G) {
-            int myidx = -1;
-            if (base + l < deg) myidx = a.col_idx[rc.x + base + l];
+        float fe[4] = {0.f, 0.f, 0.f, 0.f};   // measure: per-tile fp32 partials ex, ey (bond sums)
+        float fm[4] = {0.f, 0.f, 0.f, 0.f};   // measure: mx.x, my.x, mx.y, my.y
+        float2 own_next = make_float2(0.f, 0.f);
+        if (sub < nsite) own_next = base_q[static_cast<uint32_t>(i0 + sub) * R2];
 #pragma unroll 1
-            for (int k0 = 0; k0 < G && base + k0 < degmax; k0 += UNR) {
-                float2 t[UNR];
-                bool ok[UNR];
-#pragma unroll
-                for (int u = 0; u < UNR; ++u) {
-                    const int j = __shfl_sync(kFull, myidx, k0 + u, G);
-                    ok[u] = j >= 0;
-                    t[u] = make_float2(0.f, 0.f);
-                    if (ok[u]) t[u] = th2[static_cast<size_t>(j) * R2 + q];
+        for (int t = 0; t < CH; ++t) {
+            const int m = t * SPW + sub;          // position of this lane's site in the tile
+            if (t * SPW >= nsite) break;          // warp-uniform
+            const bool valid = m < nsite;
+            const int i = i0 + m;
+            const float2 own = own_next;
+            if (t + 1 < CH && m + SPW < nsite) own_next = base_q[static_cast<uint32_t>(i + SPW) * R2];
+            const int ry = __shfl_sync(kFull, rc.y, m & 31);
+            const int rx = __shfl_sync(kFull, rc.x, m & 31);
+            int deg = valid ? (ry & 0xffff) : 0;
+            int pos = rx - start0;
+            if constexpr (MODE == kModeMeasure) {           // bonds counted once: neighbours j > i are the tail of the list
+                const int nlow = valid ? (ry >> 16) : 0;
+                pos += nlow;
+                deg -= nlow;
+            }
+
+            RowAcc<MODE> acc;
+            float thpx = 0.f, thpy = 0.f, halfx = 0.f, halfy = 0.f, u2x = 0.f, u2y = 0.f;
+            if constexpr (MODE == kModeMetropolis) {
+                uint32_t x[4];
+                philox4x32_10(static_cast<uint32_t>(i), sweep, c2, kDomMetropolis, a.keys, x);
+                const float dx = __fmul_rn(w.x, u01(x[0]) - 0.5f);
+                const float dy = __fmul_rn(w.y, u01(x[2]) - 0.5f);
+                u2x = u01(x[1]);
+                u2y = u01(x[3]);
+                thpx = __fadd_rn(own.x, dx);
+                thpy = __fadd_rn(own.y, dy);
+                halfx = 0.5f * (thpx - own.x);
+                halfy = 0.5f * (thpy - own.y);
+                acc.midx = own.x + halfx;
+                acc.midy = own.y + halfy;
+            }
+            if constexpr (MODE == kModeMeasure) { acc.ownx = own.x; acc.owny = own.y; }
+
+            if constexpr (SPW == 1) {
+                gather_uniform(acc, base_q, R2, sidx, gidx, staged, pos, deg);
+            } else {
+                const int degmax = __reduce_max_sync(kFull, deg);
+                gather_divergent(acc, base_q, R2, sidx, gidx, staged, pos, deg, degmax,
+                                 static_cast<uint32_t>(min(i, a.N - 1)));
+            }
+
+            if constexpr (MODE == kModeMetropolis) {
+                if (valid) {
+                    float2 out;
+                    out.x = metropolis_finish(own.x, thpx, halfx, acc.ax, beta.x, u2x);
+                    out.y = metropolis_finish(own.y, thpy, halfy, acc.ay, beta.y, u2y);
+                    base_q[static_cast<uint32_t>(i) * R2] = out;
                 }
-#pragma unroll
-                for (int u = 0; u < UNR; ++u) {
-                    if (ok[u]) {
-                        if (MODE == 0) {
-                            ax += __sinf(midx - t[u].x);
-                            ay += __sinf(midy - t[u].y);
-                        } else {
-                            float sn, cs;
-                            __sincosf(t[u].x, &sn, &cs);
-                            ax += cs; bx += sn;
-                            __sincosf(t[u].y, &sn, &cs);
-                            ay += cs; by += sn;
-                        }
-                    }
+            } else if constexpr (MODE == kModeOverrelax) {
+                if (valid) {
+                    float2 out;
+                    out.x = overrelax_finish(own.x, acc.hxx, acc.hyx);
+                    out.y = overrelax_finish(own.y, acc.hxy, acc.hyy);
+                    base_q[static_cast<uint32_t>(i) * R2] = out;
+                }
+            } else {
+                if (valid) {
+                    float sn, cs;
+                    fe[0] += acc.ex; fe[1] += acc.ey;
+                    __sincosf(own.x, &sn, &cs);
+                    fm[0] += cs; fm[1] += sn;
+                    __sincosf(own.y, &sn, &cs);
+                    fm[2] += cs; fm[3] += sn;
                 }
             }
         }
+        if constexpr (MODE == kModeMeasure) {
+            dacc[0] -= static_cast<double>(fe[0]); dacc[1] += static_cast<double>(fm[0]); dacc[2] += static_cast<double>(fm[1]);
+            dacc[3] -= static_cast<double>(fe[1]); dacc[4] += static_cast<double>(fm[2]); dacc[5] += static_cast<double>(fm[3]);
+        }
+        __syncwarp();
+    }
 
-        if (valid) {
-            float2 out;
-            if (MODE == 0) {
-                out.x = metropolis_finish(own.x, thpx, halfx, ax, beta.x, u2x);
-                out.y = metropolis_finish(own.y, thpy, halfy, ay, beta.y, u2y);
-            } else {
-                out.x = overrelax_finish(own.x, ax, bx);
-                out.y = overrelax_finish(own.y, ay, by);
+    if constexpr (MODE == kModeMeasure) {
+        // CTA reduction in a fixed order, then exact (order-independent) fixed-point accumulation
+#pragma unroll
+        for (int c = 0; c < 6; ++c) s_red[(warp * 32 + lane) * 6 + c] = dacc[c];
+        __syncthreads();
+        if (threadIdx.x < G * 6) {
+            const int ll = threadIdx.x / 6, c = threadIdx.x % 6;
+            double v = 0.0;
+            for (int wi = 0; wi < kWarps; ++wi)
+                for (int sb = 0; sb < SPW; ++sb) v += s_red[(wi * 32 + sb * G + ll) * 6 + c];
+            const int slot = 2 * (blockIdx.z * G + ll) + c / 3;
+            atomicAdd(reinterpret_cast<unsigned long long *>(a.fx) + (static_cast<size_t>(s) * a.R + slot) * 3 + c % 3,
+                      static_cast<unsigned long long>(__double2ll_rn(v * kFix)));
+        }
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const unsigned int total = gridDim.x * gridDim.z;
+            s_last = (atomicAdd(a.ticket + s, 1u) == total - 1u) ? 1 : 0;
+        }
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            for (int r = threadIdx.x; r < a.R; r += kBlock) {
+                long long *f = a.fx + (static_cast<size_t>(s) * a.R + r) * 3;
+                const double e = static_cast<double>(__ldcg(f)) * kInvFix;
+                const double mx = static_cast<double>(__ldcg(f + 1)) * kInvFix;
+                const double my = static_cast<double>(__ldcg(f + 2)) * kInvFix;
+                f[0] = 0; f[1] = 0; f[2] = 0;
+                const size_t sr = static_cast<size_t>(s) * a.R + r;
+                a.E_slot[sr] = e;
+                a.M_slot[2 * sr] = mx;
+                a.M_slot[2 * sr + 1] = my;
+                if (a.accumulate) {
+                    double *o = a.acc + (static_cast<size_t>(s) * a.R + a.temp_of_slot[sr]) * 8;
+                    const double ux = mx / a.N, uy = my / a.N, m2 = ux * ux + uy * uy;
+                    o[0] += 1.0; o[1] += e; o[2] += e * e; o[3] += sqrt(m2); o[4] += m2; o[5] += m2 * m2;
+                    o[6] += ux; o[7] += uy;
+                }
             }
-            th2[static_cast<size_t>(i) * R2 + q] = out;
+            if (threadIdx.x == 0) a.ticket[s] = 0u;
         }
     }
 }
 
 // ---- generic path: any R >= 1 (odd R, R = 6, ...): one warp per site, lanes stride over the slots ----
 template <int MODE>
-__global__ void __launch_bounds__(kBlock) k_update_class_generic(const ClassArgs a) {
+__global__ void __launch_bounds__(kBlock) k_update_class_generic(const TileArgs a) {
     const int s = a.s0 + blockIdx.y;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int cbeg = a.class_ptr[s * a.q_stride + a.colour];
     const int cend = a.class_ptr[s * a.q_stride + a.colour + 1];
     const int n_sites = cend - cbeg;
-    const int g0 = (blockIdx.x * kWarps + warp) * a.chunk;
+    const int g0 = (blockIdx.x * kWarps + warp) * a.tiles_per_warp;
     if (g0 >= n_sites) return;
-    const int g1 = min(g0 + a.chunk, n_sites);
+    const int g1 = min(g0 + a.tiles_per_warp, n_sites);
     float *__restrict__ th = a.theta + static_cast<size_t>(s) * a.N * a.R;
     const int2 *__restrict__ rec = a.rec + static_cast<size_t>(s) * a.N;
     const uint32_t sweep = a.use_counter ? a.counters[0] + static_cast<uint32_t>(a.sweep_offset) : a.sweep_fixed;
@@ -210,14 +403,15 @@ __global__ void __launch_bounds__(kBlock) k_update_class_generic(const ClassArgs
     for (int g = g0; g < g1; ++g) {
         const int i = cbeg + g;
         const int2 rc = rec[i];
+        const int deg = rc.y & 0xffff;
         for (int r = lane; r < a.R; r += 32) {
             const float own = th[static_cast<size_t>(i) * a.R + r];
             float thp = 0.f, half = 0.f, mid = 0.f, u2 = 0.f, acc0 = 0.f, acc1 = 0.f;
-            if (MODE == 0) {
+            if (MODE == kModeMetropolis) {
                 uint32_t x[4];
                 philox4x32_10(static_cast<uint32_t>(i), sweep,
                               ((a.sample_base + static_cast<uint32_t>(s)) << 16) | static_cast<uint32_t>(r >> 1),
-                              kDomMetropolis, a.key0, a.key1, x);
+                              kDomMetropolis, a.keys, x);
                 const float u1 = (r & 1) ? u01(x[2]) : u01(x[0]);
                 u2 = (r & 1) ? u01(x[3]) : u01(x[1]);
                 const float w = a.w_slot[static_cast<size_t>(s) * a.R + r];
@@ -225,9 +419,9 @@ __global__ void __launch_bounds__(kBlock) k_update_class_generic(const ClassArgs
                 half = 0.5f * (thp - own);
                 mid = own + half;
             }
-            for (int e = 0; e < rc.y; ++e) {
+            for (int e = 0; e < deg; ++e) {
                 const float t = th[static_cast<size_t>(a.col_idx[rc.x + e]) * a.R + r];
-                if (MODE == 0) {
+                if (MODE == kModeMetropolis) {
                     acc0 += __sinf(mid - t);
                 } else {
                     float sn, cs;
@@ -236,7 +430,7 @@ __global__ void __launch_bounds__(kBlock) k_update_class_generic(const ClassArgs
                 }
             }
             float out;
-            if (MODE == 0)
+            if (MODE == kModeMetropolis)
                 out = metropolis_finish(own, thp, half, acc0, a.beta_slot[static_cast<size_t>(s) * a.R + r], u2);
             else
                 out = overrelax_finish(own, acc0, acc1);
@@ -245,9 +439,60 @@ __global__ void __launch_bounds__(kBlock) k_update_class_generic(const ClassArgs
     }
 }
 
+// generic measure: grid (n_chunks, samples); thread = slot (strided), sequential over the CTA's sites
+__global__ void __launch_bounds__(kBlock) k_measure_generic(const TileArgs a, int chunk_sites) {
+    __shared__ int s_last;
+    const int s = a.s0 + blockIdx.y;
+    const int ibeg = blockIdx.x * chunk_sites;
+    const int iend = min(ibeg + chunk_sites, a.N);
+    const float *__restrict__ th = a.theta + static_cast<size_t>(s) * a.N * a.R;
+    const int2 *__restrict__ rec = a.rec + static_cast<size_t>(s) * a.N;
+    for (int r = threadIdx.x; r < a.R; r += kBlock) {
+        double e = 0.0, mx = 0.0, my = 0.0;
+        for (int i = ibeg; i < iend; ++i) {
+            const int2 rc = rec[i];
+            const int deg = rc.y & 0xffff, nlow = rc.y >> 16;
+            const float own = th[static_cast<size_t>(i) * a.R + r];
+            float sn, cs, es = 0.f;
+            __sincosf(own, &sn, &cs);
+            for (int k = nlow; k < deg; ++k)
+                es += __cosf(own - th[static_cast<size_t>(a.col_idx[rc.x + k]) * a.R + r]);
+            e -= static_cast<double>(es); mx += static_cast<double>(cs); my += static_cast<double>(sn);
+        }
+        unsigned long long *f = reinterpret_cast<unsigned long long *>(a.fx) + (static_cast<size_t>(s) * a.R + r) * 3;
+        atomicAdd(f, static_cast<unsigned long long>(__double2ll_rn(e * kFix)));
+        atomicAdd(f + 1, static_cast<unsigned long long>(__double2ll_rn(mx * kFix)));
+        atomicAdd(f + 2, static_cast<unsigned long long>(__double2ll_rn(my * kFix)));
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(a.ticket + s, 1u) == gridDim.x - 1u) ? 1 : 0;
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+        for (int r = threadIdx.x; r < a.R; r += kBlock) {
+            long long *f = a.fx + (static_cast<size_t>(s) * a.R + r) * 3;
+            const double e = static_cast<double>(__ldcg(f)) * kInvFix;
+            const double mx = static_cast<double>(__ldcg(f + 1)) * kInvFix;
+            const double my = static_cast<double>(__ldcg(f + 2)) * kInvFix;
+            f[0] = 0; f[1] = 0; f[2] = 0;
+            const size_t sr = static_cast<size_t>(s) * a.R + r;
+            a.E_slot[sr] = e;
+            a.M_slot[2 * sr] = mx;
+            a.M_slot[2 * sr + 1] = my;
+            if (a.accumulate) {
+                double *o = a.acc + (static_cast<size_t>(s) * a.R + a.temp_of_slot[sr]) * 8;
+                const double ux = mx / a.N, uy = my / a.N, m2 = ux * ux + uy * uy;
+                o[0] += 1.0; o[1] += e; o[2] += e * e; o[3] += sqrt(m2); o[4] += m2; o[5] += m2 * m2;
+                o[6] += ux; o[7] += uy;
+            }
+        }
+        if (threadIdx.x == 0) a.ticket[s] = 0u;
+    }
+}
+
 // ---- init: theta = 2 pi_f * u, Philox domain 0, sweep 0 ------------------------------------------------
-__global__ void k_init_theta(float *theta, int S, int N, int R, uint32_t key0, uint32_t key1,
-                             uint32_t sample_base) {
+__global__ void k_init_theta(float *theta, int S, int N, int R, PhiloxKeys keys, uint32_t sample_base) {
     const size_t total = static_cast<size_t>(S) * N * R;
     for (size_t idx = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; idx < total;
          idx += static_cast<size_t>(gridDim.x) * blockDim.x) {
@@ -257,87 +502,12 @@ __global__ void k_init_theta(float *theta, int S, int N, int R, uint32_t key0, u
         const int s = static_cast<int>(si / N);
         uint32_t x[4];
         philox4x32_10(static_cast<uint32_t>(i), 0u, ((sample_base + static_cast<uint32_t>(s)) << 16) | static_cast<uint32_t>(r >> 1),
-                      kDomInit, key0, key1, x);
+                      kDomInit, keys, x);
         theta[idx] = __fmul_rn(kTwoPiF, (r & 1) ? u01(x[2]) : u01(x[0]));
     }
 }
 
-// ---- measure: E = -sum_{i<j} cos(theta_i - theta_j), M = sum_i (cos, sin) per slot ---------------------
-// grid (n_chunks, samples in group); each CTA reduces a contiguous range of `chunk_sites` sites of one
-// sample and writes partial[s][chunk][r][3] (fp64).  Fixed summation order -> bit-reproducible.
-struct MeasureArgs {
-    const int2 *rec;
-    const int32_t *col_idx;
-    const float *theta;
-    double *partial;   // [S][n_chunks][R][3]
-    int N, R, s0, n_chunks, chunk_sites;
-};
-
-__global__ void __launch_bounds__(kBlock) k_measure_partial(const MeasureArgs a) {
-    extern __shared__ double sm[];   // [kWarps][R][3]
-    const int s = a.s0 + blockIdx.y;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int ibeg = blockIdx.x * a.chunk_sites;
-    const int iend = min(ibeg + a.chunk_sites, a.N);
-    const float *__restrict__ th = a.theta + static_cast<size_t>(s) * a.N * a.R;
-    const int2 *__restrict__ rec = a.rec + static_cast<size_t>(s) * a.N;
-
-    for (int r0 = 0; r0 < a.R; r0 += 32) {
-        const int r = r0 + lane;
-        double e = 0.0, mx = 0.0, my = 0.0;
-        if (r < a.R) {
-            for (int i = ibeg + warp; i < iend; i += kWarps) {
-                const int2 rc = rec[i];
-                const float own = th[static_cast<size_t>(i) * a.R + r];
-                float sn, cs;
-                sincosf(own, &sn, &cs);
-                mx += static_cast<double>(cs);
-                my += static_cast<double>(sn);
-                float esite = 0.f;
-                for (int q = 0; q < rc.y; ++q) {
-                    const int j = a.col_idx[rc.x + q];
-                    if (j > i) esite += cosf(own - th[static_cast<size_t>(j) * a.R + r]);
-                }
-                e -= static_cast<double>(esite);
-            }
-            double *row = sm + (static_cast<size_t>(warp) * a.R + r) * 3;
-            row[0] = e; row[1] = mx; row[2] = my;
-        }
-    }
-    __syncthreads();
-    double *out = a.partial + (static_cast<size_t>(s) * a.n_chunks + blockIdx.x) * a.R * 3;
-    for (int idx = threadIdx.x; idx < a.R * 3; idx += kBlock) {
-        double acc = 0.0;
-        for (int wi = 0; wi < kWarps; ++wi) acc += sm[static_cast<size_t>(wi) * a.R * 3 + idx];
-        out[idx] = acc;
-    }
-}
-
-// one thread per (sample, slot): sum the chunk partials in order, publish E/M per slot and (optionally)
-// add Eq. 13-16 moments to the accumulators of the slot's temperature.
-__global__ void k_measure_final(const double *partial, int s0, int s1, int N, int R, int n_chunks,
-                                const int32_t *temp_of_slot, double *E_slot, double *M_slot, double *acc,
-                                int accumulate) {
-    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-    const int s = s0 + idx / R, r = idx % R;
-    if (s >= s1) return;
-    double e = 0.0, mx = 0.0, my = 0.0;
-    for (int c = 0; c < n_chunks; ++c) {
-        const double *p = partial + ((static_cast<size_t>(s) * n_chunks + c) * R + r) * 3;
-        e += p[0]; mx += p[1]; my += p[2];
-    }
-    E_slot[static_cast<size_t>(s) * R + r] = e;
-    M_slot[(static_cast<size_t>(s) * R + r) * 2] = mx;
-    M_slot[(static_cast<size_t>(s) * R + r) * 2 + 1] = my;
-    if (accumulate) {
-        double *a = acc + (static_cast<size_t>(s) * R + temp_of_slot[static_cast<size_t>(s) * R + r]) * 8;
-        const double ux = mx / N, uy = my / N, m2 = ux * ux + uy * uy;
-        a[0] += 1.0; a[1] += e; a[2] += e * e; a[3] += sqrt(m2); a[4] += m2; a[5] += m2 * m2;
-        a[6] += ux; a[7] += uy;
-    }
-}
-
-// ---- parallel-tempering swap round: one CTA per sample -------------------------------------------------
+// ---- parallel-tempering swap round: one CTA per sample; thread 0 of block 0 also advances the counters ----
 struct SwapArgs {
     const double *E_slot;       // [S][R]
     const double *betaT;        // [R] 1/T fp64
@@ -350,7 +520,8 @@ struct SwapArgs {
     const uint8_t *decisions;   // [S][R] or nullptr
     long long *attempts, *accepts;  // [S][R]
     int R;
-    uint32_t key0, key1, sample_base;
+    PhiloxKeys keys;
+    uint32_t sample_base;
 };
 
 __global__ void k_pt_swap(const SwapArgs a) {
@@ -367,7 +538,7 @@ __global__ void k_pt_swap(const SwapArgs a) {
         } else {
             uint32_t x[4];
             philox4x32_10(static_cast<uint32_t>(t), round, (a.sample_base + static_cast<uint32_t>(s)) << 16, kDomSwap,
-                          a.key0, a.key1, x);
+                          a.keys, x);
             const double u = static_cast<double>(u01(x[0]));
             const double arg = (a.betaT[t] - a.betaT[t + 1]) *
                                (a.E_slot[static_cast<size_t>(s) * a.R + sa] - a.E_slot[static_cast<size_t>(s) * a.R + sb]);
