@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "xy_kernels.cuh"
+#include "xy_w32.cuh"
 
 namespace {
 
@@ -41,6 +42,8 @@ int dev_alloc(T **p, size_t n) {
 }
 
 int ceil_div(long long a, long long b) { return static_cast<int>((a + b - 1) / b); }
+
+constexpr int kSMs = 148;  // B200: grids are sized in multiples of the SM count
 
 }  // namespace
 
@@ -132,8 +135,8 @@ void launch_tile_kernel(int G, int col_blocks, dim3 grid, cudaStream_t st, const
     const dim3 block(xy::kBlock);
     switch (G) {
         case 32:
-            if (col_blocks == 1) xy::k_tile<32, 1, MODE><<<grid, block, 0, st>>>(a);
-            else xy::k_tile<32, 0, MODE><<<grid, block, 0, st>>>(a);
+            if (col_blocks == 1) xy::k_w32<1, MODE><<<grid, block, 0, st>>>(a);
+            else xy::k_w32<0, MODE><<<grid, block, 0, st>>>(a);
             break;
         case 16: xy::k_tile<16, 1, MODE><<<grid, block, 0, st>>>(a); break;
         case 8: xy::k_tile<8, 1, MODE><<<grid, block, 0, st>>>(a); break;
@@ -151,12 +154,21 @@ int launch_class(xy_pt *pt, int colour, int s0, int s1, bool use_counter, int sw
     xy::TileArgs a = tile_args(pt, colour, s0);
     a.sweep_fixed = sweep_fixed; a.sweep_offset = sweep_offset; a.use_counter = use_counter ? 1 : 0;
     const int G = pt->fast_G;
-    const int ts = G ? tile_sites(G) : 1;
-    const long long tiles = (nmax + ts - 1) / ts;                          // warp tasks per sample
-    const long long total = tiles * (s1 - s0) * pt->col_blocks;
-    // enough warps for ~3 full waves of 148 SMs x 32 resident warps, at most 8 tiles per warp
-    a.tiles_per_warp = static_cast<int>(std::min<long long>(8, std::max<long long>(1, total / (148 * 32 * 3))));
-    const dim3 grid(ceil_div(ceil_div(tiles, a.tiles_per_warp), xy::kWarps), s1 - s0, pt->col_blocks);
+    dim3 grid;
+    if (G == 32) {
+        // k_w32: persistent-style grid, one wave of resident CTAs shared by the group's samples and column
+        // blocks; every warp takes an equal contiguous share of the class (no tail wave)
+        const int capacity = kSMs * xy::kW32MinBlocks;
+        const int gx = std::max(1, std::min(ceil_div(nmax, xy::kWarps), capacity / ((s1 - s0) * pt->col_blocks)));
+        grid = dim3(gx, s1 - s0, pt->col_blocks);
+    } else {
+        const int ts = G ? tile_sites(G) : 1;
+        const long long tiles = (nmax + ts - 1) / ts;                          // warp tasks per sample
+        const long long total = tiles * (s1 - s0) * pt->col_blocks;
+        // enough warps for ~3 full waves of 148 SMs x 32 resident warps, at most 8 tiles per warp
+        a.tiles_per_warp = static_cast<int>(std::min<long long>(8, std::max<long long>(1, total / (148 * 32 * 3))));
+        grid = dim3(ceil_div(ceil_div(tiles, a.tiles_per_warp), xy::kWarps), s1 - s0, pt->col_blocks);
+    }
     if (G) launch_tile_kernel<MODE>(G, pt->col_blocks, grid, pt->stream, a);
     else xy::k_update_class_generic<MODE><<<grid, xy::kBlock, 0, pt->stream>>>(a);
     XY_CUDA(cudaGetLastError());
@@ -170,7 +182,11 @@ int launch_measure(xy_pt *pt, int s0, int s1, bool accumulate) {
     xy::TileArgs a = tile_args(pt, 0, s0);
     a.accumulate = accumulate ? 1 : 0;
     const int G = pt->fast_G;
-    if (G) {
+    if (G == 32) {
+        // the partition (hence the fp32 summation order) is a function of N only: schedule-independent results
+        const dim3 grid(std::max(1, std::min(ceil_div(g->N, xy::kWarps * 16), kSMs * xy::kW32MinBlocks)), s1 - s0, pt->col_blocks);
+        launch_tile_kernel<xy::kModeMeasure>(G, pt->col_blocks, grid, pt->stream, a);
+    } else if (G) {
         const long long tiles = (g->N + tile_sites(G) - 1) / tile_sites(G);
         a.tiles_per_warp = pt->measure_tpw;
         const dim3 grid(ceil_div(ceil_div(tiles, a.tiles_per_warp), xy::kWarps), s1 - s0, pt->col_blocks);

@@ -92,12 +92,43 @@ struct TileArgs {
     int accumulate;
 };
 
+// last CTA of a sample: fixed-point sums -> E, M per slot; optional accumulation under the slot's temperature
+// (Eq. 13-16); leaves fx and the ticket zeroed for the next launch
+__device__ __forceinline__ void measure_finalize(const TileArgs &a, int s) {
+    for (int r = threadIdx.x; r < a.R; r += blockDim.x) {
+        long long *f = a.fx + (static_cast<size_t>(s) * a.R + r) * 3;
+        const double e = static_cast<double>(__ldcg(f)) * kInvFix;
+        const double mx = static_cast<double>(__ldcg(f + 1)) * kInvFix;
+        const double my = static_cast<double>(__ldcg(f + 2)) * kInvFix;
+        f[0] = 0; f[1] = 0; f[2] = 0;
+        const size_t sr = static_cast<size_t>(s) * a.R + r;
+        a.E_slot[sr] = e;
+        a.M_slot[2 * sr] = mx;
+        a.M_slot[2 * sr + 1] = my;
+        if (a.accumulate) {
+            double *o = a.acc + (static_cast<size_t>(s) * a.R + a.temp_of_slot[sr]) * 8;
+            const double ux = mx / a.N, uy = my / a.N, m2 = ux * ux + uy * uy;
+            o[0] += 1.0; o[1] += e; o[2] += e * e; o[3] += sqrt(m2); o[4] += m2; o[5] += m2 * m2;
+            o[6] += ux; o[7] += uy;
+        }
+    }
+    if (threadIdx.x == 0) a.ticket[s] = 0u;
+}
+
 // Metropolis for one slot given the sum over neighbours of sin(mid - theta_j):
 //   dE = -sum_j[cos(th' - th_j) - cos(th - th_j)] = 2 sin((th'-th)/2) sum_j sin((th'+th)/2 - th_j)
 __device__ __forceinline__ float metropolis_finish(float own, float thp, float half, float ssum, float beta,
                                                    float u2) {
     const float dE = 2.0f * __sinf(half) * ssum;
     const float p = __expf(-beta * dE);
+    float wrapped = thp;
+    if (thp >= kTwoPiF) wrapped = thp - kTwoPiF;
+    else if (thp < 0.0f) wrapped = thp + kTwoPiF;
+    return (u2 < p) ? wrapped : own;
+}
+
+// wrap the proposal once by +-2 pi_f (R5) and keep it iff u2 < p (R6, strict)
+__device__ __forceinline__ float metropolis_select(float own, float thp, float u2, float p) {
     float wrapped = thp;
     if (thp >= kTwoPiF) wrapped = thp - kTwoPiF;
     else if (thp < 0.0f) wrapped = thp + kTwoPiF;
@@ -363,24 +394,7 @@ __global__ void __launch_bounds__(kBlock) k_tile(const TileArgs a) {
         __syncthreads();
         if (s_last) {
             __threadfence();
-            for (int r = threadIdx.x; r < a.R; r += kBlock) {
-                long long *f = a.fx + (static_cast<size_t>(s) * a.R + r) * 3;
-                const double e = static_cast<double>(__ldcg(f)) * kInvFix;
-                const double mx = static_cast<double>(__ldcg(f + 1)) * kInvFix;
-                const double my = static_cast<double>(__ldcg(f + 2)) * kInvFix;
-                f[0] = 0; f[1] = 0; f[2] = 0;
-                const size_t sr = static_cast<size_t>(s) * a.R + r;
-                a.E_slot[sr] = e;
-                a.M_slot[2 * sr] = mx;
-                a.M_slot[2 * sr + 1] = my;
-                if (a.accumulate) {
-                    double *o = a.acc + (static_cast<size_t>(s) * a.R + a.temp_of_slot[sr]) * 8;
-                    const double ux = mx / a.N, uy = my / a.N, m2 = ux * ux + uy * uy;
-                    o[0] += 1.0; o[1] += e; o[2] += e * e; o[3] += sqrt(m2); o[4] += m2; o[5] += m2 * m2;
-                    o[6] += ux; o[7] += uy;
-                }
-            }
-            if (threadIdx.x == 0) a.ticket[s] = 0u;
+            measure_finalize(a, s);
         }
     }
 }
@@ -470,24 +484,7 @@ __global__ void __launch_bounds__(kBlock) k_measure_generic(const TileArgs a, in
     __syncthreads();
     if (s_last) {
         __threadfence();
-        for (int r = threadIdx.x; r < a.R; r += kBlock) {
-            long long *f = a.fx + (static_cast<size_t>(s) * a.R + r) * 3;
-            const double e = static_cast<double>(__ldcg(f)) * kInvFix;
-            const double mx = static_cast<double>(__ldcg(f + 1)) * kInvFix;
-            const double my = static_cast<double>(__ldcg(f + 2)) * kInvFix;
-            f[0] = 0; f[1] = 0; f[2] = 0;
-            const size_t sr = static_cast<size_t>(s) * a.R + r;
-            a.E_slot[sr] = e;
-            a.M_slot[2 * sr] = mx;
-            a.M_slot[2 * sr + 1] = my;
-            if (a.accumulate) {
-                double *o = a.acc + (static_cast<size_t>(s) * a.R + a.temp_of_slot[sr]) * 8;
-                const double ux = mx / a.N, uy = my / a.N, m2 = ux * ux + uy * uy;
-                o[0] += 1.0; o[1] += e; o[2] += e * e; o[3] += sqrt(m2); o[4] += m2; o[5] += m2 * m2;
-                o[6] += ux; o[7] += uy;
-            }
-        }
-        if (threadIdx.x == 0) a.ticket[s] = 0u;
+        measure_finalize(a, s);
     }
 }
 
