@@ -130,9 +130,21 @@ xy::TileArgs tile_args(const xy_pt *pt, int colour, int s0) {
 // sites per tile of the float2 path with G lanes per site (mirrors k_tile)
 int tile_sites(int G) { return (G < 8 ? G : 8) * (32 / G); }
 
+// k_w32 keeps kW32MinBlocks CTAs x 45 KB of shared memory resident per SM: ask for the largest carve-out
+template <int CB, int MODE>
+void w32_prefer_shared() {
+    static const cudaError_t once = cudaFuncSetAttribute(xy::k_w32<CB, MODE>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                                         static_cast<int>(cudaSharedmemCarveoutMaxShared));
+    (void)once;
+}
+
 template <int MODE>
 void launch_tile_kernel(int G, int col_blocks, dim3 grid, cudaStream_t st, const xy::TileArgs &a) {
     const dim3 block(xy::kBlock);
+    if (G == 32) {
+        if (col_blocks == 1) w32_prefer_shared<1, MODE>();
+        else w32_prefer_shared<0, MODE>();
+    }
     switch (G) {
         case 32:
             if (col_blocks == 1) xy::k_w32<1, MODE><<<grid, block, 0, st>>>(a);

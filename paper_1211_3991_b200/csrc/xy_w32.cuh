@@ -1,29 +1,43 @@
 // xy_w32.cuh -- the R % 64 == 0 flavour of the colour-class kernels (config 4: R = 64): one warp = one site,
-// one lane = two adjacent slots (float2), software-pipelined across sites.
+// one lane = two adjacent slots (float2), software-pipelined across sites through shared memory.
 //
-// Why a second kernel (profiles/r1a_full.md): the tile kernel issues a site's gathers and
-// then waits for them (long_scoreboard 7 of 11 stall cycles per issue, issue slots 50 % busy).  Same-colour
-// sites share no bond, so the gathers of site t+1 never read what site t stores: they are
-// issued BEFORE site t is computed, into a second register buffer, and the Philox / sin / exp work of
-// site t covers their latency.  Per neighbour a lane issues one broadcast LDS (pre-scaled id), one
-// IMAD.WIDE address, one 8-byte LDG (a 256-byte request per warp), and packed fp32x2 arithmetic
-// (add/mul.rn.f32x2 -> FADD2/FMUL2 on sm_100a) for its two slots.
+// Why a second kernel (profiles/r1a_full.md, r1b_full.md): the path is bound by instruction
+// issue and latency, not by bytes.  The tile kernel issues a site's gathers and then waits for them
+// (long_scoreboard 7 of 11 stall cycles per issue, issue slots 50 % busy); holding the in-flight gathers of
+// the next site in registers costs 120 registers and leaves 16 warps per SM.  Same-colour sites share no
+// bond, so the gathers of site t+1 never read what site t stores: they are issued BEFORE site
+// t is computed, as cp.async (LDGSTS) copies of the lane's own 8 bytes into a per-warp ring in shared
+// memory.  In-flight data then costs no registers (<= 64 per thread, 32 warps per SM), each lane reads back
+// only what it copied itself (no cross-lane synchronisation, cp.async.wait_group only), and the Philox /
+// sin / exp work of site t covers the latency of site t+1.
+// Per neighbour a lane issues: one broadcast LDS (pre-scaled id), one IMAD.WIDE address, one LDGSTS (a
+// 256-byte request per warp), one LDS.64, and packed fp32x2 arithmetic (add/mul.rn.f32x2 -> FADD2/FMUL2 on
+// sm_100a) for its two slots.
 //
 // A warp owns a contiguous, equal share of the colour class and walks it in chunks of <= 32 sites: one
 // coalesced load of the chunk's rec[], the chunk's neighbour ids (one contiguous CSR run) staged in the
-// warp's slice of shared memory.  Degrees above kDB use a short non-pipelined tail loop; a single site
-// whose degree exceeds the staging capacity is walked straight from global memory.
+// warp's slice of shared memory.  Neighbours beyond kDB per site use a short non-pipelined tail loop; a
+// single site whose degree exceeds the staging capacity is walked in blocks.
 #pragma once
 #include "xy_kernels.cuh"
 
 namespace xy {
 
-constexpr int kDB = 8;            // pipelined gathers per site and buffer
-constexpr int kStageCap = 352;    // staged neighbour ids per warp and chunk (ints)
+constexpr int kDB = 8;            // pipelined gathers per site
+constexpr int kDepth = 2;         // ring slots per warp (sites in flight)
+constexpr int kStageCap = 256;    // staged neighbour ids per warp and chunk (ints)
 #ifndef XY_W32_MIN_BLOCKS
-#define XY_W32_MIN_BLOCKS 2
+#define XY_W32_MIN_BLOCKS 4
 #endif
-constexpr int kW32MinBlocks = XY_W32_MIN_BLOCKS;  // resident CTAs per SM the register budget is sized for
+constexpr int kW32MinBlocks = XY_W32_MIN_BLOCKS;  // resident CTAs per SM the register / shared budget is sized for
+
+// per warp: ring[kDepth][kDB + 1][32] float2 (row kDB = the site's own angle) + staged ids
+struct __align__(16) W32Warp {
+    float2 ring[kDepth][kDB + 1][32];
+    uint32_t idx[kStageCap];
+};
+static_assert(sizeof(W32Warp) * kWarps <= 48 * 1024 - 64, "static shared memory limit");
+static_assert(sizeof(W32Warp) * kWarps >= sizeof(double) * kWarps * 32 * 6, "measure reduction reuses the ring");
 
 // ---- packed fp32x2 helpers (IEEE rn per component: bit-identical to the scalar operations) ----------
 __device__ __forceinline__ float2 add2(const float2 a, const float2 b) {
@@ -42,6 +56,14 @@ __device__ __forceinline__ float2 mul2(const float2 a, const float2 b) {
 
 // as_float((x >> 9) | 0x3f800000) = 1 + k 2^-23, k = x >> 9
 __device__ __forceinline__ float mant12(uint32_t x) { return __uint_as_float((x >> 9) | 0x3f800000u); }
+
+// ---- cp.async (LDGSTS): 8 bytes per lane, global -> shared, no register staging ---------------------------
+__device__ __forceinline__ void cp_async8(uint32_t smem_addr, const void *gptr) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_addr), "l"(gptr));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // ---- per-lane state of one site (two slots) ----------------------------------------------------------
 template <int MODE> struct PairAcc;
@@ -72,53 +94,61 @@ template <> struct PairAcc<kModeMeasure> {
 
 struct W32Site { int i, deg, pos; };   // warp-uniform: site id, neighbours to visit, first staged id
 
-// gather of neighbour with pre-scaled id `sid` (float2 units): one IMAD.WIDE.U32 + one LDG.64
-__device__ __forceinline__ float2 w32_ld(const float2 *__restrict__ lb, uint32_t sid) {
+// direct gather of the neighbour with pre-scaled id `sid` (float2 units): one IMAD.WIDE.U32 + one LDG.64
+__device__ __forceinline__ float2 w32_ld(const float2 *lb, uint32_t sid) {
     return __ldcg(lb + static_cast<unsigned long long>(sid));
 }
 
 template <int D>
-__device__ __forceinline__ void w32_issue_n(float2 (&v)[kDB], const float2 *__restrict__ lb, const uint32_t *sidx, int pos) {
+__device__ __forceinline__ void w32_issue_n(uint32_t row0, const float2 *lb, const uint32_t *sidx, int pos) {
+    uint32_t sid[D];
 #pragma unroll
-    for (int u = 0; u < D; ++u) v[u] = w32_ld(lb, sidx[pos + u]);
+    for (int u = 0; u < D; ++u) sid[u] = sidx[pos + u];      // all id loads first: LDS -> LDGSTS hazards are paid once
+#pragma unroll
+    for (int u = 0; u < D; ++u) cp_async8(row0 + u * 256u, lb + static_cast<unsigned long long>(sid[u]));
 }
 
-// issue min(deg, kDB) gathers back to back (deg is warp-uniform: exact count, nothing predicated off)
-__device__ __forceinline__ void w32_issue(float2 (&v)[kDB], const float2 *__restrict__ lb, const uint32_t *sidx, int pos, int deg) {
+// issue min(deg, kDB) async gathers back to back (deg is warp-uniform: exact count, nothing predicated off);
+// row0 = shared address of this lane's 8 bytes in row 0 of the ring slot
+__device__ __forceinline__ void w32_issue(uint32_t row0, const float2 *lb, const uint32_t *sidx, int pos, int deg) {
     switch (deg < kDB ? deg : kDB) {
-        case 8: w32_issue_n<8>(v, lb, sidx, pos); break;
-        case 7: w32_issue_n<7>(v, lb, sidx, pos); break;
-        case 6: w32_issue_n<6>(v, lb, sidx, pos); break;
-        case 5: w32_issue_n<5>(v, lb, sidx, pos); break;
-        case 4: w32_issue_n<4>(v, lb, sidx, pos); break;
-        case 3: w32_issue_n<3>(v, lb, sidx, pos); break;
-        case 2: w32_issue_n<2>(v, lb, sidx, pos); break;
-        case 1: w32_issue_n<1>(v, lb, sidx, pos); break;
+        case 8: w32_issue_n<8>(row0, lb, sidx, pos); break;
+        case 7: w32_issue_n<7>(row0, lb, sidx, pos); break;
+        case 6: w32_issue_n<6>(row0, lb, sidx, pos); break;
+        case 5: w32_issue_n<5>(row0, lb, sidx, pos); break;
+        case 4: w32_issue_n<4>(row0, lb, sidx, pos); break;
+        case 3: w32_issue_n<3>(row0, lb, sidx, pos); break;
+        case 2: w32_issue_n<2>(row0, lb, sidx, pos); break;
+        case 1: w32_issue_n<1>(row0, lb, sidx, pos); break;
         default: break;
     }
 }
 
 template <int D, typename ACC>
-__device__ __forceinline__ void w32_consume_n(ACC &acc, const float2 (&v)[kDB]) {
+__device__ __forceinline__ void w32_consume_n(ACC &acc, const float2 *row0) {
+    float2 v[D];
+#pragma unroll
+    for (int u = 0; u < D; ++u) v[u] = row0[u * 32];
 #pragma unroll
     for (int u = 0; u < D; ++u) acc.add(v[u]);
 }
 
+// row0 = pointer to this lane's float2 in row 0 of the ring slot
 template <typename ACC>
-__device__ __forceinline__ void w32_consume(ACC &acc, const float2 (&v)[kDB], const float2 *__restrict__ lb,
-                                            const uint32_t *sidx, int pos, int deg) {
+__device__ __forceinline__ void w32_consume(ACC &acc, const float2 *row0, const float2 *lb, const uint32_t *sidx,
+                                            int pos, int deg) {
     switch (deg < kDB ? deg : kDB) {
-        case 8: w32_consume_n<8>(acc, v); break;
-        case 7: w32_consume_n<7>(acc, v); break;
-        case 6: w32_consume_n<6>(acc, v); break;
-        case 5: w32_consume_n<5>(acc, v); break;
-        case 4: w32_consume_n<4>(acc, v); break;
-        case 3: w32_consume_n<3>(acc, v); break;
-        case 2: w32_consume_n<2>(acc, v); break;
-        case 1: w32_consume_n<1>(acc, v); break;
+        case 8: w32_consume_n<8>(acc, row0); break;
+        case 7: w32_consume_n<7>(acc, row0); break;
+        case 6: w32_consume_n<6>(acc, row0); break;
+        case 5: w32_consume_n<5>(acc, row0); break;
+        case 4: w32_consume_n<4>(acc, row0); break;
+        case 3: w32_consume_n<3>(acc, row0); break;
+        case 2: w32_consume_n<2>(acc, row0); break;
+        case 1: w32_consume_n<1>(acc, row0); break;
         default: break;
     }
-    for (int k = kDB; k < deg; k += 4) {   // rare tail (degree > kDB), not pipelined
+    for (int k = kDB; k < deg; k += 4) {   // rare tail (more than kDB neighbours), not pipelined
         float2 t[4];
 #pragma unroll
         for (int u = 0; u < 4; ++u)
@@ -134,8 +164,7 @@ __device__ __forceinline__ void w32_consume(ACC &acc, const float2 (&v)[kDB], co
 // CB = 1: R == 64 (stride known at compile time).  MODE as in k_tile.
 template <int CB, int MODE>
 __global__ void __launch_bounds__(kBlock, kW32MinBlocks) k_w32(const TileArgs a) {
-    __shared__ uint32_t s_idx[kWarps][kStageCap];
-    __shared__ double s_red[MODE == kModeMeasure ? kWarps * 32 * 6 : 1];
+    __shared__ W32Warp s_w[kWarps];
     __shared__ int s_last;
 
     const int s = a.s0 + blockIdx.y;
@@ -156,7 +185,11 @@ __global__ void __launch_bounds__(kBlock, kW32MinBlocks) k_w32(const TileArgs a)
     float2 *lb = reinterpret_cast<float2 *>(a.theta) + static_cast<size_t>(s) * a.N * R2 + q;
     asm volatile("" : "+l"(lb));   // keep the lane's base as one materialised pointer: gather address = one IMAD.WIDE.U32
     const int2 *__restrict__ rec = a.rec + static_cast<size_t>(s) * a.N;
-    uint32_t *sidx = s_idx[warp];
+    uint32_t *sidx = s_w[warp].idx;
+    const float2 *ring_l = &s_w[warp].ring[0][0][lane];                       // this lane's column of the ring
+    const uint32_t ring_s = static_cast<uint32_t>(__cvta_generic_to_shared(ring_l));
+    constexpr uint32_t kSlotBytes = (kDB + 1) * 32 * sizeof(float2);
+    constexpr int kSlotElems = (kDB + 1) * 32;
 
     float2 nbeta = make_float2(0.f, 0.f), w = make_float2(0.f, 0.f);
     uint32_t sweep = 0, c2 = 0;
@@ -169,37 +202,39 @@ __global__ void __launch_bounds__(kBlock, kW32MinBlocks) k_w32(const TileArgs a)
     }
     double dacc[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};   // measure: E, Mx, My of the .x slot, then of the .y slot
 
-    // one site, its own angle and first kDB neighbours already in (own, v)
-    auto process = [&](const W32Site st, const float2 own, const float2 (&v)[kDB], float2 &fe, float2 &fmx, float2 &fmy) {
-        PairAcc<MODE> acc;
+    // Metropolis proposal of site i (both slots of the lane): th' = th + w (u1 - 1/2), half = (th' - th)/2
+    auto begin = [&](int i, const float2 own, PairAcc<MODE> &acc, float2 &thp, float2 &half, float2 &u2) {
         if constexpr (MODE == kModeMetropolis) {
             uint32_t x[4];
-            philox4x32_10(static_cast<uint32_t>(st.i), sweep, c2, kDomMetropolis, a.keys, x);
+            philox4x32_10(static_cast<uint32_t>(i), sweep, c2, kDomMetropolis, a.keys, x);
             // u = (k + 1/2) 2^-23 with k = x >> 9 (R11), every step exact:
             //   u1 - 1/2 = ((1 + k 2^-23) - 3/2) + 2^-24,   u2 = (1 + k 2^-23) - (1 - 2^-24)
             const float2 u1mh = add2(add2(make_float2(mant12(x[0]), mant12(x[2])), make_float2(-1.5f, -1.5f)),
                                      make_float2(5.9604644775390625e-08f, 5.9604644775390625e-08f));
-            const float2 u2 = add2(make_float2(mant12(x[1]), mant12(x[3])), make_float2(-0.99999994f, -0.99999994f));
-            const float2 thp = add2(own, mul2(w, u1mh));                      // R5: fp32 mul, fp32 add
-            const float2 half = mul2(sub2(thp, own), make_float2(0.5f, 0.5f));
+            u2 = add2(make_float2(mant12(x[1]), mant12(x[3])), make_float2(-0.99999994f, -0.99999994f));
+            thp = add2(own, mul2(w, u1mh));                      // R5: fp32 mul, fp32 add
+            half = mul2(sub2(thp, own), make_float2(0.5f, 0.5f));
             acc.mid = add2(own, half);
-            w32_consume(acc, v, lb, sidx, st.pos, st.deg);
+        } else if constexpr (MODE == kModeMeasure) {
+            acc.own = own;
+        }
+    };
+    auto finish = [&](int i, const float2 own, const PairAcc<MODE> &acc, const float2 thp, const float2 half,
+                      const float2 u2, float2 &fe, float2 &fmx, float2 &fmy) {
+        if constexpr (MODE == kModeMetropolis) {
             // dE = 2 sin((th'-th)/2) sum_j sin((th'+th)/2 - th_j)
             const float2 sh = make_float2(__sinf(half.x), __sinf(half.y));
             const float2 arg = mul2(nbeta, mul2(add2(sh, sh), acc.s));
             float2 out;
             out.x = metropolis_select(own.x, thp.x, u2.x, __expf(arg.x));
             out.y = metropolis_select(own.y, thp.y, u2.y, __expf(arg.y));
-            lb[static_cast<unsigned long long>(static_cast<uint32_t>(st.i) * R2)] = out;
+            lb[static_cast<unsigned long long>(static_cast<uint32_t>(i) * R2)] = out;
         } else if constexpr (MODE == kModeOverrelax) {
-            w32_consume(acc, v, lb, sidx, st.pos, st.deg);
             float2 out;
             out.x = overrelax_finish(own.x, acc.hx.x, acc.hy.x);
             out.y = overrelax_finish(own.y, acc.hx.y, acc.hy.y);
-            lb[static_cast<unsigned long long>(static_cast<uint32_t>(st.i) * R2)] = out;
+            lb[static_cast<unsigned long long>(static_cast<uint32_t>(i) * R2)] = out;
         } else {
-            acc.own = own;
-            w32_consume(acc, v, lb, sidx, st.pos, st.deg);
             float sx, cx, sy, cy;
             __sincosf(own.x, &sx, &cx);
             __sincosf(own.y, &sy, &cy);
@@ -217,12 +252,11 @@ __global__ void __launch_bounds__(kBlock, kW32MinBlocks) k_w32(const TileArgs a)
         const int start0 = __shfl_sync(kFull, rc.x, 0);
         const int endl = rc.x + (rc.y & 0xffff) - start0;
         const unsigned fits = __ballot_sync(kFull, lane < nsite && endl <= kStageCap);
-        const int m = __ffs(~fits) - 1;            // leading sites that fit (ffs(0) = 0 -> m = -1 means all 32)
-        const int msite = m < 0 ? 32 : m;
+        const int msite = fits == kFull ? 32 : __ffs(~fits) - 1;      // leading sites that fit
         float2 fe = make_float2(0.f, 0.f), fmx = make_float2(0.f, 0.f), fmy = make_float2(0.f, 0.f);
 
         if (msite == 0) {
-            // a single site with more neighbours than the staging slice: ids straight from global memory
+            // a single site with more neighbours than the staging slice: walk its ids in blocks
             const int ry = __shfl_sync(kFull, rc.y, 0);
             int deg = ry & 0xffff, pos = 0;
             if constexpr (MODE == kModeMeasure) { pos = ry >> 16; deg -= pos; }
@@ -230,17 +264,7 @@ __global__ void __launch_bounds__(kBlock, kW32MinBlocks) k_w32(const TileArgs a)
             const float2 own = lb[static_cast<unsigned long long>(static_cast<uint32_t>(i0) * R2)];
             float2 thp = make_float2(0.f, 0.f), half = thp, u2 = thp;
             PairAcc<MODE> acc;
-            if constexpr (MODE == kModeMetropolis) {
-                uint32_t x[4];
-                philox4x32_10(static_cast<uint32_t>(i0), sweep, c2, kDomMetropolis, a.keys, x);
-                const float2 u1mh = add2(add2(make_float2(mant12(x[0]), mant12(x[2])), make_float2(-1.5f, -1.5f)),
-                                         make_float2(5.9604644775390625e-08f, 5.9604644775390625e-08f));
-                u2 = add2(make_float2(mant12(x[1]), mant12(x[3])), make_float2(-0.99999994f, -0.99999994f));
-                thp = add2(own, mul2(w, u1mh));
-                half = mul2(sub2(thp, own), make_float2(0.5f, 0.5f));
-                acc.mid = add2(own, half);
-            }
-            if constexpr (MODE == kModeMeasure) acc.own = own;
+            begin(i0, own, acc, thp, half, u2);
             for (int k0 = 0; k0 < deg; k0 += kStageCap) {
                 const int nb = min(kStageCap, deg - k0);
                 __syncwarp();
@@ -256,24 +280,7 @@ __global__ void __launch_bounds__(kBlock, kW32MinBlocks) k_w32(const TileArgs a)
                         if (k + u < nb) acc.add(t[u]);
                 }
             }
-            if constexpr (MODE == kModeMetropolis) {
-                const float2 sh = make_float2(__sinf(half.x), __sinf(half.y));
-                const float2 arg = mul2(nbeta, mul2(add2(sh, sh), acc.s));
-                float2 out;
-                out.x = metropolis_select(own.x, thp.x, u2.x, __expf(arg.x));
-                out.y = metropolis_select(own.y, thp.y, u2.y, __expf(arg.y));
-                lb[static_cast<unsigned long long>(static_cast<uint32_t>(i0) * R2)] = out;
-            } else if constexpr (MODE == kModeOverrelax) {
-                float2 out;
-                out.x = overrelax_finish(own.x, acc.hx.x, acc.hy.x);
-                out.y = overrelax_finish(own.y, acc.hx.y, acc.hy.y);
-                lb[static_cast<unsigned long long>(static_cast<uint32_t>(i0) * R2)] = out;
-            } else {
-                float sx, cx, sy, cy;
-                __sincosf(own.x, &sx, &cx);
-                __sincosf(own.y, &sy, &cy);
-                fe = acc.e; fmx = make_float2(cx, cy); fmy = make_float2(sx, sy);
-            }
+            finish(i0, own, acc, thp, half, u2, fe, fmx, fmy);
             __syncwarp();
             i0 += 1;
         } else {
@@ -299,28 +306,34 @@ __global__ void __launch_bounds__(kBlock, kW32MinBlocks) k_w32(const TileArgs a)
                 }
                 return st;
             };
-            auto own_of = [&](const W32Site st) { return lb[static_cast<unsigned long long>(static_cast<uint32_t>(st.i) * R2)]; };
+            // async copies of site st (own angle -> row kDB, first kDB neighbours -> rows 0..) into ring slot `slot`
+            auto issue = [&](const W32Site st, int slot) {
+                const uint32_t row0 = ring_s + static_cast<uint32_t>(slot) * kSlotBytes;
+                cp_async8(row0 + kDB * 256u, lb + static_cast<unsigned long long>(static_cast<uint32_t>(st.i) * R2));
+                w32_issue(row0, lb, sidx, st.pos, st.deg);
+                cp_async_commit();
+            };
 
-            // software pipeline, two register buffers: the gathers of site t+1 fly while site t is computed
-            float2 va[kDB], vb[kDB], owna, ownb = make_float2(0.f, 0.f);
-            W32Site sa = site_of(0), sb = sa;
-            owna = own_of(sa);
-            w32_issue(va, lb, sidx, sa.pos, sa.deg);
-            for (int t = 0; t < msite; t += 2) {
-                const bool hb = t + 1 < msite;
-                if (hb) {
-                    sb = site_of(t + 1);
-                    ownb = own_of(sb);
-                    w32_issue(vb, lb, sidx, sb.pos, sb.deg);
+            // software pipeline over the chunk: the copies of site t+1 fly while site t is computed
+            W32Site cur = site_of(0);
+            issue(cur, 0);
+            for (int t = 0; t < msite; ++t) {
+                W32Site nxt = cur;
+                if (t + 1 < msite) {
+                    nxt = site_of(t + 1);
+                    issue(nxt, (t + 1) & 1);
+                    cp_async_wait<1>();
+                } else {
+                    cp_async_wait<0>();
                 }
-                process(sa, owna, va, fe, fmx, fmy);
-                if (!hb) break;
-                if (t + 2 < msite) {
-                    sa = site_of(t + 2);
-                    owna = own_of(sa);
-                    w32_issue(va, lb, sidx, sa.pos, sa.deg);
-                }
-                process(sb, ownb, vb, fe, fmx, fmy);
+                const float2 *row0 = ring_l + (t & 1) * kSlotElems;
+                const float2 own = row0[kDB * 32];
+                float2 thp = make_float2(0.f, 0.f), half = thp, u2 = thp;
+                PairAcc<MODE> acc;
+                begin(cur.i, own, acc, thp, half, u2);
+                w32_consume(acc, row0, lb, sidx, cur.pos, cur.deg);
+                finish(cur.i, own, acc, thp, half, u2, fe, fmx, fmy);
+                cur = nxt;
             }
             __syncwarp();
             i0 += msite;
@@ -332,7 +345,9 @@ __global__ void __launch_bounds__(kBlock, kW32MinBlocks) k_w32(const TileArgs a)
     }
 
     if constexpr (MODE == kModeMeasure) {
-        // CTA reduction in a fixed order, then exact (order-independent) fixed-point accumulation
+        // CTA reduction in a fixed order (the ring is free now), then exact order-independent fixed-point accumulation
+        __syncthreads();
+        double *s_red = reinterpret_cast<double *>(&s_w[0]);
 #pragma unroll
         for (int c = 0; c < 6; ++c) s_red[(warp * 32 + lane) * 6 + c] = dacc[c];
         __syncthreads();
