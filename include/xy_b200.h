@@ -108,7 +108,8 @@ int xy_set_schedule(xy_pt *pt, int samples_per_group);
 
 /* ---- single-colour steps (lockstep parity tests) ----
  * Metropolis on colour class `colour` of every sample with Philox sweep index `sweep` (the handle's
- * sweep counter is not touched); OR on one colour class. */
+ * sweep counter is not touched); OR on one colour class.  Launched sample group by sample group with the
+ * same grids as xy_run (xy_set_schedule), so a lockstep check exercises the timed launch configuration. */
 int xy_metropolis_colour(xy_pt *pt, int colour, uint32_t sweep);
 int xy_overrelax_colour(xy_pt *pt, int colour);
 

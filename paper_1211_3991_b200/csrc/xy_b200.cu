@@ -591,13 +591,23 @@ int xy_overrelax(xy_pt *pt, int n_sweeps) {
 int xy_metropolis_colour(xy_pt *pt, int colour, uint32_t sweep) {
     if (!check_pt(pt) || colour < 0 || colour >= pt->g->q_max) return fail(XY_EINVAL, "bad handle or colour");
     pt->e_fresh = false;
-    return launch_class<0>(pt, colour, 0, pt->g->S, false, 0, sweep);
+    const int group = auto_group(pt);   // same sample groups, hence the same grids, as xy_run / xy_run_sweeps
+    for (int s0 = 0; s0 < pt->g->S; s0 += group) {
+        const int rc = launch_class<0>(pt, colour, s0, std::min(pt->g->S, s0 + group), false, 0, sweep);
+        if (rc != XY_OK) return rc;
+    }
+    return XY_OK;
 }
 
 int xy_overrelax_colour(xy_pt *pt, int colour) {
     if (!check_pt(pt) || colour < 0 || colour >= pt->g->q_max) return fail(XY_EINVAL, "bad handle or colour");
     pt->e_fresh = false;
-    return launch_class<1>(pt, colour, 0, pt->g->S, false, 0, 0u);
+    const int group = auto_group(pt);
+    for (int s0 = 0; s0 < pt->g->S; s0 += group) {
+        const int rc = launch_class<1>(pt, colour, s0, std::min(pt->g->S, s0 + group), false, 0, 0u);
+        if (rc != XY_OK) return rc;
+    }
+    return XY_OK;
 }
 
 int xy_pt_swap(xy_pt *pt) {

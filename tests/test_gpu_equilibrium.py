@@ -1,0 +1,163 @@
+"""-m gpu equilibrium parity (BASELINE.json north_star: E, <|m|> and the Binder cumulant within 3 combined
+jackknife sigma), R13.
+
+(1) CUDA path vs exact physics (the same pins that hold the oracle: ring closed form, quadrature on small
+    graphs, beta = 0 moments) -- so an error common to both implementations cannot hide.
+(2) CUDA path vs oracle on all five BASELINE configs.  The GPU runs every config at its FULL size and sweep
+    count; the oracle (2.5e6 updates/s/core) runs sample 0 of the same graphs under the same protocol for a
+    shortened run, on a subset of the temperature ladder where the config is too large (a PT ladder leaves
+    each temperature's Gibbs measure unchanged, so the subset compares like with like; high temperatures
+    are chosen because they equilibrate within the shortened run).  Different Philox seeds on the two sides.
+"""
+import concurrent.futures as cf
+import os
+import time
+
+import numpy as np
+import pytest
+
+import closed_forms as CF
+import graphs as G
+import gpu_util as U
+import oracle as O
+import stats as S
+from paper_1211_3991_b200 import levy, workloads
+
+pytestmark = pytest.mark.gpu
+SEED_GPU, SEED_CPU = 0x9B200E01, 0x0CAC1E02
+NSIG = 4.5
+
+
+def gpu_blocks(ens, n_blocks, cycles_per_block, burn_cycles, sps=10, orps=1, me=1):
+    """accumulator increments per block, [B][S][R][8]"""
+    ens.run(burn_cycles, sps, orps, me)
+    prev = ens.read_accumulators()
+    out = []
+    for _ in range(n_blocks):
+        ens.run(cycles_per_block, sps, orps, me)
+        cur = ens.read_accumulators()
+        out.append(cur - prev)
+        prev = cur
+    return np.array(out)
+
+
+def pooled(blocks):
+    """independent samples of the SAME graph: pool them (sum of accumulators) -> [B][R][8]"""
+    return blocks.sum(axis=1)
+
+
+def check_exact(blocks, fn, exact, what):
+    est, sig = S.jackknife(blocks, fn)
+    exact = np.broadcast_to(np.asarray(exact, np.float64), est.shape)
+    z = np.abs(est - exact) / sig
+    assert np.all(z < NSIG), f"{what}: est {est} exact {exact} sigma {sig} z {z}"
+    assert np.all(sig < 0.05 * np.maximum(np.abs(exact), 0.02)), f"{what}: error bars too wide {sig}"
+
+
+# ---- (1) exact physics on the CUDA path --------------------------------------------------------------
+@pytest.mark.parametrize("N", [8, 16])
+def test_gpu_ring_closed_form(N):
+    T = np.array([0.5, 1.0, 2.0, 4.0])
+    ens = U.ensemble_from_graph(G.colour_major(N, G.ring_edges(N)), T, SEED_GPU, S=8)
+    blocks = pooled(gpu_blocks(ens, 40, 40, 40))
+    exact = np.array([CF.ring(N, 1 / t) for t in T])
+    check_exact(blocks, S.obs_energy(N), exact[:, 0], f"gpu ring N={N} e")
+    check_exact(blocks, S.obs_m2(), exact[:, 1], f"gpu ring N={N} m2")
+    sw, rd, att, acc = ens.get_counters()
+    assert 0.05 < acc.sum() / att.sum() < 0.95
+    ens.close()
+
+
+@pytest.mark.parametrize("name", ["P3", "K3", "star", "paw", "diamond", "K4"])
+def test_gpu_small_graph_quadrature(name):
+    N, edges = CF.SMALL_GRAPHS[name]
+    betas = np.array([2.0, 1.0, 0.5])
+    ens = U.ensemble_from_graph(G.colour_major(N, edges), 1 / betas, SEED_GPU, S=16)
+    blocks = pooled(gpu_blocks(ens, 40, 50, 50))
+    q = [CF.quadrature(N, edges, b) for b in betas]
+    check_exact(blocks, lambda m: m[..., S.E_], [x["E"] for x in q], f"gpu {name} E")
+    check_exact(blocks, S.obs_var_e(), [x["varE"] for x in q], f"gpu {name} varE")
+    check_exact(blocks, S.obs_absm(), [x["absm"] for x in q], f"gpu {name} |m|")
+    check_exact(blocks, S.obs_m2(), [x["m2"] for x in q], f"gpu {name} m2")
+    check_exact(blocks, S.obs_m4(), [x["m4"] for x in q], f"gpu {name} m4")
+    check_exact(blocks, S.obs_u4(), [x["m4"] / x["m2"] ** 2 - 1 for x in q], f"gpu {name} U4")
+    ens.close()
+
+
+def test_gpu_beta_zero_moments():
+    g = levy.build(8, 3.5, 6, workloads.BASE_SEED, S=4)
+    N = 64
+    ens = U.ensemble_from_levy(g, np.array([np.inf, np.inf]), SEED_GPU)
+    blocks = gpu_blocks(ens, 40, 20, 5)
+    ex = CF.beta0_moments(N, N * 3)
+    for fn, want in [(S.obs_m2(), ex["m2"]), (S.obs_m4(), ex["m4"]), (lambda m: m[..., S.E_], 0.0),
+                     (S.obs_var_e(), ex["varE"]), (S.obs_u4(), 1 - 1 / N)]:
+        est, sig = S.jackknife(blocks, fn)
+        assert np.all(np.abs(est - want) < NSIG * sig), (est, want, sig)
+    ens.close()
+
+
+# ---- (2) CUDA path vs oracle, all five configs ------------------------------------------------------------
+# cfg -> (oracle temperature indices (None = all), oracle cycles, gpu cycles); a cycle = 10 sweeps + 1 swap round.
+# GPU cycles = the config's full sweep count (BASELINE.json); oracle cycles sized to <= ~2 min of one core each.
+PLAN = {
+    0: (None, 1000, 1000),
+    1: (None, 200, 2000),
+    2: ([28, 29, 30, 31], 100, 1000),
+    3: ([28, 29, 30, 31], 40, 500),
+    4: ([62, 63], 20, 200),
+}
+N_BLOCKS = 10
+
+
+def oracle_blocks(cfg):
+    w = workloads.CONFIGS[cfg]
+    tidx, n_cycles, _ = PLAN[cfg]
+    g = levy.build(w.L, w.rho, w.z, w.seed, S=1)
+    T = w.temperatures() if tidx is None else w.temperatures()[tidx]
+    ch = O.Chain(g.row_ptr[0], g.col_idx[0], g.class_ptr(0), T, SEED_CPU + cfg)
+    t0 = time.time()
+    ch.run(n_cycles // 2, w.sweeps_per_swap, w.or_per_sweep, 1)          # burn-in: first half (R13)
+    per = max(1, (n_cycles - n_cycles // 2) // N_BLOCKS)
+    blocks = []
+    for _ in range(N_BLOCKS):
+        ch.reset_acc()
+        ch.run(per, w.sweeps_per_swap, w.or_per_sweep, 1)
+        blocks.append(ch.acc.copy())
+    return np.array(blocks), time.time() - t0
+
+
+def test_equilibrium_all_configs_vs_oracle():
+    cores = os.cpu_count() or 1
+    pool = cf.ThreadPoolExecutor(max_workers=max(1, min(5, cores - 1)))     # ctypes releases the GIL
+    # longest oracle chains first
+    futs = {cfg: pool.submit(oracle_blocks, cfg) for cfg in (1, 4, 3, 2, 0)}
+    rows, zs = [], []
+    for cfg in (0, 1, 2, 3, 4):
+        w = workloads.CONFIGS[cfg]
+        tidx, _, n_cycles = PLAN[cfg]
+        g = levy.build(w.L, w.rho, w.z, w.seed, S=w.S)
+        ens = U.ensemble_from_levy(g, w.temperatures(), SEED_GPU + cfg)
+        per = (n_cycles - n_cycles // 2) // (2 * N_BLOCKS)
+        gb = gpu_blocks(ens, 2 * N_BLOCKS, per, n_cycles // 2, w.sweeps_per_swap, w.or_per_sweep, 1)[:, 0]   # sample 0
+        ens.close()
+        if tidx is not None:
+            gb = gb[:, tidx]
+        ob, secs = futs[cfg].result()
+        for name, fn in (("E/N", S.obs_energy(w.N)), ("|m|", S.obs_absm()), ("U4", S.obs_u4())):
+            eg, sg = S.jackknife(gb, fn)
+            eo, so = S.jackknife(ob, fn)
+            z = (eg - eo) / np.sqrt(sg ** 2 + so ** 2)
+            zs.append(z)
+            k = int(np.argmax(np.abs(z)))
+            rows.append(f"cfg{cfg} {name:4s} n_T={len(z):2d} max|z|={np.abs(z).max():.2f} at T#{k}: gpu {eg[k]:.6f}+-{sg[k]:.1e} "
+                        f"oracle {eo[k]:.6f}+-{so[k]:.1e}  (oracle {secs:.0f} s)")
+    pool.shutdown()
+    z = np.abs(np.concatenate(zs))
+    print("\n" + "\n".join(rows))
+    print(f"comparisons {z.size}: >3 sigma {int((z > 3).sum())}, max {z.max():.2f}, chi2/dof {np.mean(z ** 2):.2f}")
+    # R13: 10-block jackknife errors are t-distributed (9 dof: P(|t|>3) = 1.5 %, P(|t|>4.5) = 0.15 %); with
+    # ~110 simultaneous comparisons allow the expected tail beyond 3 sigma and nothing beyond 4.5 sigma
+    assert z.max() < NSIG
+    assert (z > 3).sum() <= max(2, int(0.04 * z.size))
+    assert np.mean(z ** 2) < 2.0

@@ -1,0 +1,82 @@
+"""-m gpu parity at BASELINE.json's FULL sizes (configs 1-4), in the launch configuration bench.py times
+(same sample groups / grids as the captured xy_run graph): after a few captured PT cycles, every colour
+class is stepped in lockstep and SAMPLED sites are compared with the oracle one by one (all replicas of
+the site); energies of sampled samples are compared with the oracle's fp64 sum; and properties that hold
+at any size are checked on the whole state (range, untouched classes, OR energy conservation, labels)."""
+import numpy as np
+import pytest
+
+import gpu_util as U
+import oracle as O
+from paper_1211_3991_b200 import levy, workloads
+
+pytestmark = pytest.mark.gpu
+SEED = 0xF0115123
+SITES_PER_CLASS = 96          # sampled sites per (sample, colour class): x R replicas each
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
+def test_full_size_lockstep_sampled_sites_and_invariants(cfg):
+    w = workloads.CONFIGS[cfg]
+    g = levy.build(w.L, w.rho, w.z, w.seed, S=w.S)
+    T = w.temperatures()
+    ens = U.ensemble_from_levy(g, T, SEED)
+    graphs = U.graphs_of_levy(g)
+    rng = np.random.default_rng(cfg)
+    # the timed path first: two captured PT cycles (labels get permuted, angles decorrelate from the init)
+    ens.run(2, w.sweeps_per_swap, w.or_per_sweep, 1)
+    sw, rd, att, acc = ens.get_counters()
+    assert (sw, rd) == (2 * w.sweeps_per_swap, 2)
+    labels = ens.get_labels()
+    assert np.array_equal(np.sort(labels, axis=1), np.tile(np.arange(w.R, dtype=np.int32), (w.S, 1)))
+    assert acc.sum() > 0 and np.all(acc <= att)                       # some swaps were accepted
+    n_acc = ens.read_accumulators()[..., 0]
+    assert np.all(n_acc == 2 * w.sweeps_per_swap)
+
+    samples = sorted(rng.choice(w.S, size=min(2, w.S), replace=False).tolist())
+    Q = int(g.n_colours.max())
+    tm = dict(updates=0, near=0, bad=0, accepted=0, disagree_near=0)
+    to = dict(updates=0, illcond=0, bad=0)
+    sweep = sw + 1
+    for c in range(Q):
+        st = U.lockstep_metropolis(ens, graphs, T, SEED, c, sweep, samples=samples, site_subset=SITES_PER_CLASS, rng=rng)
+        assert st["bad"] == 0, (cfg, c, st)
+        for k in tm: tm[k] += st[k]
+    E_before = ens.get_energy()
+    for c in range(Q):
+        st = U.lockstep_overrelax(ens, graphs, c, samples=samples, site_subset=SITES_PER_CLASS, rng=rng)
+        assert st["bad"] == 0, (cfg, c, st)
+        for k in to: to[k] += st[k]
+    E_after = ens.get_energy()
+    print(f"\n[full size cfg {cfg}] metropolis {tm}  overrelax {to}")
+    assert tm["updates"] >= 0.9 * len(samples) * (Q - 1) * SITES_PER_CLASS * w.R
+    assert 0.2 < tm["accepted"] / tm["updates"] < 0.95
+    assert tm["near"] <= 5 + 2e-4 * tm["updates"]
+    assert to["illcond"] <= 5 + 5e-3 * to["updates"]
+
+    # OR sweep conserves the energy of every replica (ref 66 via PAPER.md:460): fp32 round-off only
+    assert np.all(np.abs(E_after - E_before) <= 1e-6 * w.N * 3), np.abs(E_after - E_before).max()
+
+    # energies / magnetisation of one whole sample against the oracle's fp64 sums (all R slots)
+    th = ens.get_theta()
+    assert th.min() >= 0.0 and th.max() <= np.float32(6.2831855)
+    s = samples[0]
+    Eo, Mxo, Myo = O.measure(g.row_ptr[s], g.col_idx[s], th[s])
+    assert np.all(np.abs(E_after[s] - Eo) <= 4e-7 * 3 * w.N), np.abs(E_after[s] - Eo).max()
+    out = ens.measure(want=True)
+    lab = ens.get_labels()
+    assert np.all(np.abs(out[s, lab[s], 0] - Eo) <= 4e-7 * 3 * w.N)
+    assert np.all(np.abs(out[s, lab[s], 1] - Mxo) <= 2e-7 * w.N) and np.all(np.abs(out[s, lab[s], 2] - Myo) <= 2e-7 * w.N)
+    ens.close()
+
+
+def test_full_size_graph_structure_of_all_configs():
+    """integer work at full size: the builder's graphs that the bench loads are proper, symmetric, E_b = N z / 2."""
+    for cfg in (1, 2, 3, 4):
+        w = workloads.CONFIGS[cfg]
+        g = levy.build(w.L, w.rho, w.z, w.seed, S=min(w.S, 4))
+        for s in range(g.S):
+            rp, ci, col = g.row_ptr[s], g.col_idx[s], g.colour[s]
+            assert rp[-1] == w.N * w.z
+            assert O.colouring_is_proper(rp, ci, col)
+            assert np.all(np.diff(col) >= 0)
