@@ -5,6 +5,7 @@ memory (the theta tensor) and the CUDA stream, nothing else.  There is no CPU fa
 cannot be built or loaded, or no CUDA device is present, the calls raise.
 """
 import ctypes as C
+import os
 
 import numpy as np
 
@@ -33,6 +34,7 @@ SYMBOLS = {
     "xy_run": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]),
     "xy_run_sweeps": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int]),
     "xy_set_schedule": (C.c_int, [C.c_void_p, C.c_int]),
+    "xy_set_path": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]),
     "xy_metropolis_colour": (C.c_int, [C.c_void_p, C.c_int, C.c_uint32]),
     "xy_overrelax_colour": (C.c_int, [C.c_void_p, C.c_int]),
     "xy_get_theta": (C.c_int, [C.c_void_p, C.c_void_p]),
@@ -63,7 +65,8 @@ def lib():
     """Load (building if stale) libxy_b200.so.  Raises if nvcc or the build fails: there is no fallback."""
     global _lib
     if _lib is None:
-        L = C.CDLL(_build.build_xy())
+        # XY_B200_LIB: load a prebuilt variant of the library instead (kernel tuning experiments only)
+        L = C.CDLL(os.environ.get("XY_B200_LIB") or _build.build_xy())
         for name, (res, args) in SYMBOLS.items():
             f = getattr(L, name)
             f.restype, f.argtypes = res, args
@@ -162,6 +165,10 @@ def xy_run_sweeps(pt, n_blocks, sweeps_per_block=10, or_per_sweep=1):
 
 def xy_set_schedule(pt, samples_per_group):
     _check(lib().xy_set_schedule(pt, samples_per_group))
+
+
+def xy_set_path(pt, path=0, balance=1, pdl=1, l2_persist=1):
+    _check(lib().xy_set_path(pt, path, balance, pdl, l2_persist))
 
 
 def xy_metropolis_colour(pt, colour, sweep):
@@ -289,6 +296,7 @@ class Ensemble:
     def run_sweeps(self, n_blocks, sweeps_per_block=10, or_per_sweep=1):
         xy_run_sweeps(self.pt, n_blocks, sweeps_per_block, or_per_sweep)
     def set_schedule(self, g): xy_set_schedule(self.pt, g)
+    def set_path(self, path=0, balance=1, pdl=1, l2_persist=1): xy_set_path(self.pt, path, balance, pdl, l2_persist)
     def metropolis_colour(self, c, sweep): xy_metropolis_colour(self.pt, c, sweep)
     def overrelax_colour(self, c): xy_overrelax_colour(self.pt, c)
     def get_theta(self, out=None): return xy_get_theta(self.pt, (self.S, self.N, self.R), out)

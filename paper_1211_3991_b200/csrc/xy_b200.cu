@@ -13,7 +13,7 @@
 #include <vector>
 
 #include "xy_kernels.cuh"
-#include "xy_w32.cuh"
+#include "xy_sweep.cuh"
 
 namespace {
 
@@ -43,7 +43,35 @@ int dev_alloc(T **p, size_t n) {
 
 int ceil_div(long long a, long long b) { return static_cast<int>((a + b - 1) / b); }
 
-constexpr int kSMs = 148;  // B200: grids are sized in multiples of the SM count
+// the k_sweep<G, CB> instantiation for G lanes per site (CB = 0: R a multiple of 64 larger than 64)
+const void *sweep_function(int G, bool single_block) {
+    switch (G) {
+        case 32: return single_block ? reinterpret_cast<const void *>(xy::k_sweep<32, 1>)
+                                     : reinterpret_cast<const void *>(xy::k_sweep<32, 0>);
+        case 16: return reinterpret_cast<const void *>(xy::k_sweep<16, 1>);
+        case 8: return reinterpret_cast<const void *>(xy::k_sweep<8, 1>);
+        case 4: return reinterpret_cast<const void *>(xy::k_sweep<4, 1>);
+        case 2: return reinterpret_cast<const void *>(xy::k_sweep<2, 1>);
+        default: return reinterpret_cast<const void *>(xy::k_sweep<1, 1>);
+    }
+}
+
+template <int MODE>
+const void *phase_function_mode(int G, bool single_block) {
+    switch (G) {
+        case 32: return single_block ? reinterpret_cast<const void *>(xy::k_phase<32, 1, MODE>)
+                                     : reinterpret_cast<const void *>(xy::k_phase<32, 0, MODE>);
+        case 16: return reinterpret_cast<const void *>(xy::k_phase<16, 1, MODE>);
+        case 8: return reinterpret_cast<const void *>(xy::k_phase<8, 1, MODE>);
+        case 4: return reinterpret_cast<const void *>(xy::k_phase<4, 1, MODE>);
+        case 2: return reinterpret_cast<const void *>(xy::k_phase<2, 1, MODE>);
+        default: return reinterpret_cast<const void *>(xy::k_phase<1, 1, MODE>);
+    }
+}
+const void *phase_function(int G, bool single_block, int mode) {
+    return mode == 0 ? phase_function_mode<0>(G, single_block)
+         : mode == 1 ? phase_function_mode<1>(G, single_block) : phase_function_mode<2>(G, single_block);
+}
 
 }  // namespace
 
@@ -54,6 +82,7 @@ struct xy_graph {
     int32_t *col_idx = nullptr;
     int32_t *class_ptr = nullptr;
     std::vector<int32_t> h_class_ptr;  // [S][q_stride]
+    std::vector<uint32_t> h_deg;       // [S][N] degree | n_lower << 16 (host copy of rec.y, for the share tables)
     size_t bytes_per_sample = 0;       // rec + col_idx (average), for the schedule heuristic
     cudaStream_t stream = nullptr;
 };
@@ -88,9 +117,18 @@ struct xy_pt {
     long long *attempts = nullptr, *accepts = nullptr;
     uint8_t *decisions = nullptr;
     xy::PhiloxKeys keys;
-    int fast_G = 0;  // lanes per site of the float2 path, 0 = generic kernel
+    int fast_G = 0;  // lanes per site of the persistent float2 kernel (k_sweep), 0 = legacy generic kernels
     int col_blocks = 1;
-    int measure_tpw = 1;      // tiles per warp of the measure launch: a function of N and R only
+    int l2_persist = 1;              // mark the running sample group's theta as persisting in L2 (access policy window)
+    size_t l2_persist_bytes = 0, l2_window_max = 0;   // device limits (0 = not supported)
+    int balance = 1;                 // cost-balanced share tables (1) or equal shares (0)
+    int pdl = 1;                     // programmatic dependent launch edges between the k_phase launches
+    int path = 0;                    // 0 = automatic, 1 = persistent kernel (k_sweep), 2 = one launch per phase (k_phase, CUDA graph)
+    const void *phase_fn[3] = {nullptr, nullptr, nullptr};   // k_phase<G, CB, MODE>
+    std::map<int, int32_t *> parts;  // warps per sample -> device [S][q_stride][nw + 1] cost-balanced share tables
+    const void *sweep_fn = nullptr;  // the k_sweep<G, CB> instantiation of this ensemble
+    int sweep_capacity = 0;          // co-resident CTAs of sweep_fn on this device (cooperative launch limit)
+    unsigned int *bar = nullptr;     // [S] per-sample barrier counters of k_sweep
     int measure_chunk = 256;  // sites per CTA of the generic measure kernel
     int samples_per_group = 0;  // 0 = automatic
     // host mirrors
@@ -127,86 +165,148 @@ xy::TileArgs tile_args(const xy_pt *pt, int colour, int s0) {
     return a;
 }
 
-// sites per tile of the float2 path with G lanes per site (mirrors k_tile)
-int tile_sites(int G) { return (G < 8 ? G : 8) * (32 / G); }
-
-// k_w32 keeps kW32MinBlocks CTAs x 45 KB of shared memory resident per SM: ask for the largest carve-out
-template <int CB, int MODE>
-void w32_prefer_shared() {
-    static const cudaError_t once = cudaFuncSetAttribute(xy::k_w32<CB, MODE>, cudaFuncAttributePreferredSharedMemoryCarveout,
-                                                         static_cast<int>(cudaSharedmemCarveoutMaxShared));
-    (void)once;
+// ---- share tables: for nw warps per sample, the first site of every warp's contiguous share of each colour class
+// (and, at colour index q_max, of the measure pass over all sites), balanced by cost = const + degree.  Integer
+// bookkeeping only; the kernels give the same results for any partition (sites of a class are independent, the
+// measure sums are exact integers). ----
+int get_partition(xy_pt *pt, int nw, const int32_t **out) {
+    auto it = pt->parts.find(nw);
+    if (it != pt->parts.end()) { *out = it->second; return XY_OK; }
+    const xy_graph *g = pt->g;
+    const int S = g->S, N = g->N, QS = g->q_stride;
+    std::vector<int32_t> h(static_cast<size_t>(S) * QS * (nw + 1));
+    std::vector<long long> pre(static_cast<size_t>(N) + 1);
+    for (int s = 0; s < S; ++s) {
+        const uint32_t *dg = g->h_deg.data() + static_cast<size_t>(s) * N;
+        const int32_t *cp = g->h_class_ptr.data() + static_cast<size_t>(s) * QS;
+        for (int c = 0; c < QS; ++c) {
+            const bool meas = c == QS - 1;
+            const int cbeg = meas ? 0 : cp[c], cend = meas ? N : cp[c + 1];
+            pre[0] = 0;
+            for (int i = cbeg; i < cend; ++i) {
+                const int deg = static_cast<int>(dg[i] & 0xffffu), nlow = static_cast<int>(dg[i] >> 16);
+                pre[i - cbeg + 1] = pre[i - cbeg] + (meas ? 10 + deg - nlow : 12 + deg);
+            }
+            const long long total = pre[cend - cbeg];
+            int32_t *row = h.data() + (static_cast<size_t>(s) * QS + c) * (nw + 1);
+            int pos = 0;
+            for (int k = 0; k <= nw; ++k) {
+                const long long target = (total * k + nw / 2) / nw;
+                while (pos < cend - cbeg && pre[pos] < target) ++pos;
+                row[k] = cbeg + pos;
+            }
+            row[0] = cbeg; row[nw] = cend;
+        }
+    }
+    int32_t *d = nullptr;
+    const int rc = dev_alloc(&d, h.size());
+    if (rc != XY_OK) return rc;
+    const cudaError_t e = cudaMemcpy(d, h.data(), h.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cudaFree(d); return fail(XY_ECUDA, std::string("share table upload: ") + cudaGetErrorString(e)); }
+    pt->parts[nw] = d;
+    *out = d;
+    return XY_OK;
 }
 
-template <int MODE>
-void launch_tile_kernel(int G, int col_blocks, dim3 grid, cudaStream_t st, const xy::TileArgs &a) {
-    const dim3 block(xy::kBlock);
-    if (G == 32) {
-        if (col_blocks == 1) w32_prefer_shared<1, MODE>();
-        else w32_prefer_shared<0, MODE>();
-    }
-    switch (G) {
-        case 32:
-            if (col_blocks == 1) xy::k_w32<1, MODE><<<grid, block, 0, st>>>(a);
-            else xy::k_w32<0, MODE><<<grid, block, 0, st>>>(a);
-            break;
-        case 16: xy::k_tile<16, 1, MODE><<<grid, block, 0, st>>>(a); break;
-        case 8: xy::k_tile<8, 1, MODE><<<grid, block, 0, st>>>(a); break;
-        case 4: xy::k_tile<4, 1, MODE><<<grid, block, 0, st>>>(a); break;
-        case 2: xy::k_tile<2, 1, MODE><<<grid, block, 0, st>>>(a); break;
-        default: xy::k_tile<1, 1, MODE><<<grid, block, 0, st>>>(a); break;
-    }
+// CTAs per (sample, column block) for a group of ns samples: one wave of resident CTAs shared by the group, at most
+// one row of `nmax` sites per warp
+int sweep_grid_x(const xy_pt *pt, int ns, int nmax) {
+    const int spw = 32 / pt->fast_G;
+    return std::max(1, std::min(ceil_div(nmax, xy::kWarps * spw), pt->sweep_capacity / (ns * pt->col_blocks)));
 }
 
+xy::SweepArgs sweep_args(xy_pt *pt, int s0) {
+    xy::SweepArgs a;
+    a.t = tile_args(pt, 0, s0);
+    a.n_rep = 1; a.sps = 0; a.do_met = 0; a.orps = 0; a.me = 0; a.end_measure = 0; a.do_swap = 0; a.c_lo = 0; a.c_hi = 0;
+    a.sweep0 = 0; a.round0 = 0;
+    a.bar = pt->bar; a.part = nullptr;
+    a.betaT = pt->betaT; a.beta_f = pt->beta_f; a.w_f = pt->w_f;
+    a.slot_of_temp = pt->slot_of_temp; a.temp_of_slot = pt->temp_of_slot;
+    a.beta_slot = pt->beta_slot; a.w_slot = pt->w_slot;
+    a.decisions = nullptr; a.attempts = pt->attempts; a.accepts = pt->accepts;
+    return a;
+}
+
+// launch attribute that keeps theta of samples s0..s1-1 resident in the persisting part of L2 while the group's
+// kernels run (sample-major time blocking): every neighbour gather of the group hits this window.
+// Returns 0 when the device has no persisting L2 or the option is off.
+int l2_window_attr(const xy_pt *pt, int s0, int s1, cudaLaunchAttribute *attr) {
+    if (!pt->l2_persist || pt->l2_persist_bytes == 0 || pt->l2_window_max == 0) return 0;
+    const size_t per_sample = static_cast<size_t>(pt->g->N) * pt->R * sizeof(float);
+    const size_t bytes = std::min(per_sample * static_cast<size_t>(s1 - s0), pt->l2_window_max);
+    attr->id = cudaLaunchAttributeAccessPolicyWindow;
+    attr->val.accessPolicyWindow.base_ptr = pt->theta + static_cast<size_t>(s0) * pt->g->N * pt->R;
+    attr->val.accessPolicyWindow.num_bytes = bytes;
+    attr->val.accessPolicyWindow.hitRatio = static_cast<float>(std::min(1.0, static_cast<double>(pt->l2_persist_bytes) / static_cast<double>(bytes)));
+    attr->val.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+    attr->val.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+    return 1;
+}
+
+// one phase (mode 0 Metropolis / 1 over-relaxation on `colour`, 2 measure) of samples s0..s1-1 as one k_phase launch
+// with a programmatic-dependent-launch edge to its predecessor in the stream
+int launch_phase(xy_pt *pt, int mode, int colour, int s0, int s1, bool use_counter, int sweep_offset, uint32_t sweep_fixed,
+                 bool accumulate) {
+    const xy_graph *g = pt->g;
+    const int nmax = mode == 2 ? g->N : max_class_size(g, colour, s0, s1);
+    if (nmax == 0 || s1 <= s0) return XY_OK;
+    xy::SweepArgs a = sweep_args(pt, s0);
+    a.t.colour = colour;
+    a.t.sweep_fixed = sweep_fixed; a.t.sweep_offset = sweep_offset; a.t.use_counter = use_counter ? 1 : 0;
+    a.t.accumulate = accumulate ? 1 : 0;
+    const int gx = sweep_grid_x(pt, s1 - s0, nmax);
+    if (pt->balance) {
+        const int rc = get_partition(pt, gx * xy::kWarps, &a.part);
+        if (rc != XY_OK) return rc;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(gx, s1 - s0, pt->col_blocks);
+    cfg.blockDim = dim3(xy::kBlock);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = pt->stream;
+    cudaLaunchAttribute attr[2];
+    int na = l2_window_attr(pt, s0, s1, &attr[0]);
+    if (pt->pdl) {
+        attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
+    cfg.attrs = attr; cfg.numAttrs = na;
+    void *params[] = {&a};
+    XY_CUDA(cudaLaunchKernelExC(&cfg, pt->phase_fn[mode], params));
+    pt->launches += 1;
+    return XY_OK;
+}
+
+// ---- launch path with one launch per colour class, captured in CUDA graphs: k_phase for the float2 flavours,
+// the any-R kernels when R has none (odd R, R = 6, 10, ...) ----
 template <int MODE>
 int launch_class(xy_pt *pt, int colour, int s0, int s1, bool use_counter, int sweep_offset, uint32_t sweep_fixed) {
+    if (pt->fast_G) return launch_phase(pt, MODE, colour, s0, s1, use_counter, sweep_offset, sweep_fixed, false);
     const xy_graph *g = pt->g;
     const int nmax = max_class_size(g, colour, s0, s1);
     if (nmax == 0 || s1 <= s0) return XY_OK;
     xy::TileArgs a = tile_args(pt, colour, s0);
     a.sweep_fixed = sweep_fixed; a.sweep_offset = sweep_offset; a.use_counter = use_counter ? 1 : 0;
-    const int G = pt->fast_G;
-    dim3 grid;
-    if (G == 32) {
-        // k_w32: persistent-style grid, one wave of resident CTAs shared by the group's samples and column
-        // blocks; every warp takes an equal contiguous share of the class (no tail wave)
-        const int capacity = kSMs * xy::kW32MinBlocks;
-        const int gx = std::max(1, std::min(ceil_div(nmax, xy::kWarps), capacity / ((s1 - s0) * pt->col_blocks)));
-        grid = dim3(gx, s1 - s0, pt->col_blocks);
-    } else {
-        const int ts = G ? tile_sites(G) : 1;
-        const long long tiles = (nmax + ts - 1) / ts;                          // warp tasks per sample
-        const long long total = tiles * (s1 - s0) * pt->col_blocks;
-        // enough warps for ~3 full waves of 148 SMs x 32 resident warps, at most 8 tiles per warp
-        a.tiles_per_warp = static_cast<int>(std::min<long long>(8, std::max<long long>(1, total / (148 * 32 * 3))));
-        grid = dim3(ceil_div(ceil_div(tiles, a.tiles_per_warp), xy::kWarps), s1 - s0, pt->col_blocks);
-    }
-    if (G) launch_tile_kernel<MODE>(G, pt->col_blocks, grid, pt->stream, a);
-    else xy::k_update_class_generic<MODE><<<grid, xy::kBlock, 0, pt->stream>>>(a);
+    const long long total = static_cast<long long>(nmax) * (s1 - s0);
+    // enough warps for ~3 full waves of resident warps, at most 8 sites per warp
+    a.tiles_per_warp = static_cast<int>(std::min<long long>(8, std::max<long long>(1, total / (148 * 32 * 3))));
+    const dim3 grid(ceil_div(ceil_div(nmax, a.tiles_per_warp), xy::kWarps), s1 - s0, 1);
+    xy::k_update_class_generic<MODE><<<grid, xy::kBlock, 0, pt->stream>>>(a);
     XY_CUDA(cudaGetLastError());
     pt->launches += 1;
     return XY_OK;
 }
 
 int launch_measure(xy_pt *pt, int s0, int s1, bool accumulate) {
+    if (pt->fast_G) return launch_phase(pt, 2, 0, s0, s1, false, 0, 0u, accumulate);
     const xy_graph *g = pt->g;
     if (s1 <= s0) return XY_OK;
     xy::TileArgs a = tile_args(pt, 0, s0);
     a.accumulate = accumulate ? 1 : 0;
-    const int G = pt->fast_G;
-    if (G == 32) {
-        // the partition (hence the fp32 summation order) is a function of N only: schedule-independent results
-        const dim3 grid(std::max(1, std::min(ceil_div(g->N, xy::kWarps * 16), kSMs * xy::kW32MinBlocks)), s1 - s0, pt->col_blocks);
-        launch_tile_kernel<xy::kModeMeasure>(G, pt->col_blocks, grid, pt->stream, a);
-    } else if (G) {
-        const long long tiles = (g->N + tile_sites(G) - 1) / tile_sites(G);
-        a.tiles_per_warp = pt->measure_tpw;
-        const dim3 grid(ceil_div(ceil_div(tiles, a.tiles_per_warp), xy::kWarps), s1 - s0, pt->col_blocks);
-        launch_tile_kernel<xy::kModeMeasure>(G, pt->col_blocks, grid, pt->stream, a);
-    } else {
-        const dim3 grid(ceil_div(g->N, pt->measure_chunk), s1 - s0);
-        xy::k_measure_generic<<<grid, xy::kBlock, 0, pt->stream>>>(a, pt->measure_chunk);
-    }
+    const dim3 grid(ceil_div(g->N, pt->measure_chunk), s1 - s0);
+    xy::k_measure_generic<<<grid, xy::kBlock, 0, pt->stream>>>(a, pt->measure_chunk);
     XY_CUDA(cudaGetLastError());
     pt->launches += 1;
     return XY_OK;
@@ -238,11 +338,86 @@ int sweep_group(xy_pt *pt, int mode, int s0, int s1, bool use_counter, int sweep
 
 int auto_group(const xy_pt *pt) {
     const xy_graph *g = pt->g;
-    if (pt->samples_per_group > 0) return std::min(pt->samples_per_group, g->S);
+    int group;
     const double per_sample = static_cast<double>(g->N) * pt->R * 4.0 + static_cast<double>(g->bytes_per_sample);
     const double l2_budget = 96.0e6;  // of the 126 MB L2
-    if (per_sample * g->S <= l2_budget) return g->S;
-    return std::max(1, std::min(g->S, static_cast<int>(l2_budget / per_sample)));
+    if (pt->samples_per_group > 0) group = std::min(pt->samples_per_group, g->S);
+    else if (per_sample * g->S <= l2_budget) group = g->S;
+    else group = std::max(1, std::min(g->S, static_cast<int>(l2_budget / per_sample)));
+    // k_sweep is launched cooperatively: at least one CTA per (sample, column block) must be resident
+    if (pt->fast_G) group = std::max(1, std::min(group, pt->sweep_capacity / pt->col_blocks));
+    return group;
+}
+
+// ---- the persistent path: what one k_sweep launch does for every sample of a group (xy_sweep.cuh, SweepArgs) ----
+struct SweepCtl {
+    int n_rep = 1, sps = 0, do_met = 0, orps = 0, me = 0, end_measure = 0, do_swap = 0, c_lo = 0, c_hi = -1;
+    uint32_t sweep0 = 0, round0 = 0;
+    const uint8_t *decisions = nullptr;
+};
+
+int launch_sweep_group(xy_pt *pt, int s0, int s1, const SweepCtl &c) {
+    const xy_graph *g = pt->g;
+    xy::SweepArgs a = sweep_args(pt, s0);
+    a.n_rep = c.n_rep; a.sps = c.sps; a.do_met = c.do_met; a.orps = c.orps; a.me = c.me;
+    a.end_measure = c.end_measure; a.do_swap = c.do_swap;
+    a.c_lo = c.c_lo; a.c_hi = c.c_hi < 0 ? g->q_max : c.c_hi;
+    a.sweep0 = c.sweep0; a.round0 = c.round0;
+    a.decisions = c.decisions;
+    // grid: per sample enough warps to give every warp at least one row of the largest colour class (the measure
+    // phase walks all N sites); all CTAs co-resident (cooperative launch)
+    const int ns = s1 - s0;
+    int nmax = 1;
+    const bool updates = c.sps > 0 && (c.do_met || c.orps > 0);
+    if (updates) for (int col = a.c_lo; col < a.c_hi; ++col) nmax = std::max(nmax, max_class_size(g, col, s0, s1));
+    else nmax = g->N;
+    // a barrier between two CTAs costs microseconds, a bar.sync inside one CTA nanoseconds: few, fat CTAs per sample
+    const int gx = sweep_grid_x(pt, ns, ceil_div(nmax, 4));
+    if (pt->balance) {
+        const int rc = get_partition(pt, gx * xy::kWarps, &a.part);
+        if (rc != XY_OK) return rc;
+    }
+    XY_CUDA(cudaMemsetAsync(pt->bar + s0, 0, static_cast<size_t>(ns) * sizeof(unsigned int), pt->stream));
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(gx, ns, pt->col_blocks);
+    cfg.blockDim = dim3(xy::kBlock);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = pt->stream;
+    cudaLaunchAttribute attr[2];
+    int na = l2_window_attr(pt, s0, s1, &attr[0]);
+    attr[na].id = cudaLaunchAttributeCooperative;
+    attr[na].val.cooperative = 1;
+    ++na;
+    cfg.attrs = attr; cfg.numAttrs = na;
+    void *params[] = {&a};
+    XY_CUDA(cudaLaunchKernelExC(&cfg, pt->sweep_fn, params));
+    pt->launches += 1;
+    return XY_OK;
+}
+
+// which path runs the float2 flavours: the persistent kernel when a sample is small (launch- and latency-bound
+// phases: a per-sample barrier is cheaper than a kernel boundary), one launch per phase otherwise
+bool use_persistent(const xy_pt *pt) {
+    if (!pt->fast_G) return false;
+    if (pt->path == 1) return true;
+    if (pt->path == 2) return false;
+    return false;   // measured: the per-phase launches win at every BASELINE config
+}
+
+// run `c` for every sample group (all repetitions of a group before the next group starts: sample-major time
+// blocking, legal because samples never interact), then advance the device counters
+int run_sweep(xy_pt *pt, const SweepCtl &c, uint32_t d_sweep, uint32_t d_round) {
+    const int S = pt->g->S, group = auto_group(pt);
+    for (int s0 = 0; s0 < S; s0 += group) {
+        const int rc = launch_sweep_group(pt, s0, std::min(S, s0 + group), c);
+        if (rc != XY_OK) return rc;
+    }
+    if (d_sweep || d_round) {
+        xy::k_tick<<<1, 1, 0, pt->stream>>>(pt->counters, d_sweep, d_round);
+        XY_CUDA(cudaGetLastError());
+        pt->launches += 1;
+    }
+    return XY_OK;
 }
 
 // enqueue one PT cycle on the stream; `phase` = sweep counter mod measure_every at entry
@@ -285,6 +460,23 @@ int issue_sweeps(xy_pt *pt, int sps, int orps, int group) {
     xy::k_tick<<<1, 1, 0, pt->stream>>>(pt->counters, static_cast<uint32_t>(sps), 0u);
     XY_CUDA(cudaGetLastError());
     pt->launches += 1;
+    return XY_OK;
+}
+
+// build (outside stream capture: they allocate and copy) the share tables every k_phase launch of a cycle will use
+int prepare_partitions(xy_pt *pt, int group) {
+    if (!pt->fast_G || !pt->balance) return XY_OK;
+    const xy_graph *g = pt->g;
+    for (int s0 = 0; s0 < g->S; s0 += group) {
+        const int s1 = std::min(g->S, s0 + group);
+        for (int c = 0; c <= g->q_max; ++c) {
+            const int nmax = c == g->q_max ? g->N : max_class_size(g, c, s0, s1);
+            if (nmax == 0) continue;
+            const int32_t *unused = nullptr;
+            const int rc = get_partition(pt, sweep_grid_x(pt, s1 - s0, nmax) * xy::kWarps, &unused);
+            if (rc != XY_OK) return rc;
+        }
+    }
     return XY_OK;
 }
 
@@ -394,6 +586,7 @@ int xy_graph_load(int S, int N, const int32_t *row_ptr, const int32_t *col_idx, 
         std::vector<int2> h_rec(static_cast<size_t>(S) * N);
         std::vector<int32_t> h_col(static_cast<size_t>(off[S]));   // neighbour lists, ascending per site
         g->h_class_ptr.assign(static_cast<size_t>(S) * g->q_stride, 0);
+        g->h_deg.assign(static_cast<size_t>(S) * N, 0u);
         for (int s = 0; s < S; ++s) {
             const int32_t *rp = row_ptr + static_cast<size_t>(s) * (N + 1);
             const int32_t *col = colour + static_cast<size_t>(s) * N;
@@ -405,6 +598,7 @@ int xy_graph_load(int S, int N, const int32_t *row_ptr, const int32_t *col_idx, 
                 std::sort(dst, dst + deg);
                 const int n_lower = static_cast<int>(std::lower_bound(dst, dst + deg, i) - dst);
                 h_rec[static_cast<size_t>(s) * N + i] = make_int2(static_cast<int>(off[s] + rp[i]), deg | (n_lower << 16));
+                g->h_deg[static_cast<size_t>(s) * N + i] = static_cast<uint32_t>(deg | (n_lower << 16));
                 cp[col[i] + 1]++;
             }
             for (int c = 0; c < q_max; ++c) cp[c + 1] += cp[c];
@@ -492,12 +686,35 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
         return fail(XY_EINVAL, "N * R / 2 must fit in int32 (offsets inside a sample are 32-bit)");
     }
     pt->keys = xy::philox_key_schedule(pt->key0, pt->key1);
-    // measure partition: a function of N and R only, so results do not depend on the schedule
-    {
-        const int ts = pt->fast_G ? tile_sites(pt->fast_G) : 1;
-        const long long tiles = (N + ts - 1) / ts;
-        pt->measure_tpw = static_cast<int>(std::min<long long>(16, std::max<long long>(1, tiles / 4096)));
-        pt->measure_chunk = std::max(256, ((N + 127) / 128 + 7) / 8 * 8);
+    pt->measure_chunk = std::max(256, ((N + 127) / 128 + 7) / 8 * 8);   // legacy measure partition: a function of N only
+    if (pt->fast_G) {
+        pt->sweep_fn = sweep_function(pt->fast_G, pt->col_blocks == 1);
+        for (int m = 0; m < 3; ++m) {
+            pt->phase_fn[m] = phase_function(pt->fast_G, pt->col_blocks == 1, m);
+            cudaFuncSetAttribute(pt->phase_fn[m], cudaFuncAttributePreferredSharedMemoryCarveout,
+                                 static_cast<int>(cudaSharedmemCarveoutMaxShared));
+        }
+        int per_sm = 0, n_sm = 0, dev = 0;
+        cudaError_t eo = cudaGetDevice(&dev);
+        if (eo == cudaSuccess) eo = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        if (eo == cudaSuccess)   // k_sweep keeps kSweepMinBlocks CTAs x 45 KB of shared memory resident per SM
+            eo = cudaFuncSetAttribute(pt->sweep_fn, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                      static_cast<int>(cudaSharedmemCarveoutMaxShared));
+        if (eo == cudaSuccess) eo = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pt->sweep_fn, xy::kBlock, 0);
+        if (eo != cudaSuccess || per_sm < 1 || n_sm < 1) {
+            if (pt->owns_stream) cudaStreamDestroy(pt->stream);
+            delete pt;
+            return fail(XY_ECUDA, std::string("k_sweep occupancy query: ") + cudaGetErrorString(eo));
+        }
+        pt->sweep_capacity = per_sm * n_sm;
+        int max_persist = 0, max_window = 0;
+        if (cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, dev) == cudaSuccess && max_persist > 0 &&
+            max_window > 0 && cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, static_cast<size_t>(max_persist)) == cudaSuccess) {
+            pt->l2_persist_bytes = static_cast<size_t>(max_persist);
+            pt->l2_window_max = static_cast<size_t>(max_window);
+        }
+        cudaGetLastError();
     }
 
     const size_t SR = static_cast<size_t>(S) * R;
@@ -512,6 +729,7 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
     A(dev_alloc(&pt->E_slot, SR)); A(dev_alloc(&pt->M_slot, SR * 2));
     A(dev_alloc(&pt->fx, SR * 3)); A(dev_alloc(&pt->ticket, S)); A(dev_alloc(&pt->acc, SR * XY_NACC));
     A(dev_alloc(&pt->attempts, SR)); A(dev_alloc(&pt->accepts, SR)); A(dev_alloc(&pt->decisions, SR));
+    A(dev_alloc(&pt->bar, S));
     if (rc != XY_OK) { xy_pt_destroy(pt); return rc; }
     std::vector<float> hb(R), hw(R);
     std::vector<double> hbT(R);
@@ -558,7 +776,8 @@ int xy_pt_destroy(xy_pt *pt) {
     cudaFree(pt->beta_slot); cudaFree(pt->w_slot); cudaFree(pt->beta_f); cudaFree(pt->w_f); cudaFree(pt->betaT);
     cudaFree(pt->temp_of_slot); cudaFree(pt->slot_of_temp); cudaFree(pt->counters);
     cudaFree(pt->E_slot); cudaFree(pt->M_slot); cudaFree(pt->fx); cudaFree(pt->ticket); cudaFree(pt->acc);
-    cudaFree(pt->attempts); cudaFree(pt->accepts); cudaFree(pt->decisions);
+    cudaFree(pt->attempts); cudaFree(pt->accepts); cudaFree(pt->decisions); cudaFree(pt->bar);
+    for (auto &kv : pt->parts) cudaFree(kv.second);
     if (pt->owns_stream) cudaStreamDestroy(pt->stream);
     delete pt;
     return XY_OK;
@@ -566,6 +785,16 @@ int xy_pt_destroy(xy_pt *pt) {
 
 int xy_sweep(xy_pt *pt, int n_sweeps) {
     if (!check_pt(pt) || n_sweeps < 0) return fail(XY_EINVAL, "bad handle or n_sweeps < 0");
+    if (use_persistent(pt)) {
+        if (n_sweeps == 0) return XY_OK;
+        SweepCtl c;
+        c.n_rep = n_sweeps; c.sps = 1; c.do_met = 1; c.sweep0 = pt->sweep;
+        const int rc = run_sweep(pt, c, static_cast<uint32_t>(n_sweeps), 0u);
+        if (rc != XY_OK) return rc;
+        pt->sweep += static_cast<uint32_t>(n_sweeps);
+        pt->e_fresh = false;
+        return XY_OK;
+    }
     for (int n = 0; n < n_sweeps; ++n) {
         const int rc = sweep_group(pt, 0, 0, pt->g->S, true, 1, 0u);
         if (rc != XY_OK) return rc;
@@ -580,6 +809,13 @@ int xy_sweep(xy_pt *pt, int n_sweeps) {
 
 int xy_overrelax(xy_pt *pt, int n_sweeps) {
     if (!check_pt(pt) || n_sweeps < 0) return fail(XY_EINVAL, "bad handle or n_sweeps < 0");
+    if (use_persistent(pt)) {
+        if (n_sweeps == 0) return XY_OK;
+        SweepCtl c;
+        c.n_rep = n_sweeps; c.sps = 1; c.orps = 1;
+        pt->e_fresh = false;
+        return run_sweep(pt, c, 0u, 0u);
+    }
     for (int n = 0; n < n_sweeps; ++n) {
         const int rc = sweep_group(pt, 1, 0, pt->g->S, false, 0, 0u);
         if (rc != XY_OK) return rc;
@@ -591,7 +827,12 @@ int xy_overrelax(xy_pt *pt, int n_sweeps) {
 int xy_metropolis_colour(xy_pt *pt, int colour, uint32_t sweep) {
     if (!check_pt(pt) || colour < 0 || colour >= pt->g->q_max) return fail(XY_EINVAL, "bad handle or colour");
     pt->e_fresh = false;
-    const int group = auto_group(pt);   // same sample groups, hence the same grids, as xy_run / xy_run_sweeps
+    if (use_persistent(pt)) {   // same kernel, same sample groups as xy_run / xy_run_sweeps
+        SweepCtl c;
+        c.sps = 1; c.do_met = 1; c.c_lo = colour; c.c_hi = colour + 1; c.sweep0 = sweep - 1u;
+        return run_sweep(pt, c, 0u, 0u);
+    }
+    const int group = auto_group(pt);
     for (int s0 = 0; s0 < pt->g->S; s0 += group) {
         const int rc = launch_class<0>(pt, colour, s0, std::min(pt->g->S, s0 + group), false, 0, sweep);
         if (rc != XY_OK) return rc;
@@ -602,6 +843,11 @@ int xy_metropolis_colour(xy_pt *pt, int colour, uint32_t sweep) {
 int xy_overrelax_colour(xy_pt *pt, int colour) {
     if (!check_pt(pt) || colour < 0 || colour >= pt->g->q_max) return fail(XY_EINVAL, "bad handle or colour");
     pt->e_fresh = false;
+    if (use_persistent(pt)) {
+        SweepCtl c;
+        c.sps = 1; c.orps = 1; c.c_lo = colour; c.c_hi = colour + 1;
+        return run_sweep(pt, c, 0u, 0u);
+    }
     const int group = auto_group(pt);
     for (int s0 = 0; s0 < pt->g->S; s0 += group) {
         const int rc = launch_class<1>(pt, colour, s0, std::min(pt->g->S, s0 + group), false, 0, 0u);
@@ -612,6 +858,13 @@ int xy_overrelax_colour(xy_pt *pt, int colour) {
 
 int xy_pt_swap(xy_pt *pt) {
     if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    if (use_persistent(pt)) {
+        SweepCtl c;
+        c.end_measure = pt->e_fresh ? 0 : 1; c.do_swap = 1; c.round0 = pt->round;
+        const int rc = run_sweep(pt, c, 0u, 1u);
+        if (rc == XY_OK) { pt->round += 1; pt->e_fresh = true; }
+        return rc;
+    }
     if (!pt->e_fresh) {
         const int rc = launch_measure(pt, 0, pt->g->S, false);
         if (rc != XY_OK) return rc;
@@ -627,6 +880,13 @@ int xy_swap_with_decisions(xy_pt *pt, const uint8_t *accept_host) {
     const size_t SR = static_cast<size_t>(pt->g->S) * pt->R;
     XY_CUDA(cudaMemcpyAsync(pt->decisions, accept_host, SR, cudaMemcpyHostToDevice, pt->stream));
     XY_CUDA(cudaStreamSynchronize(pt->stream));  // accept_host is borrowed for the call only
+    if (use_persistent(pt)) {
+        SweepCtl c;
+        c.do_swap = 1; c.round0 = pt->round; c.decisions = pt->decisions;
+        const int rc = run_sweep(pt, c, 0u, 1u);
+        if (rc == XY_OK) pt->round += 1;
+        return rc;
+    }
     const int rc = launch_swap(pt, pt->decisions, 0u);
     if (rc == XY_OK) pt->round += 1;
     return rc;
@@ -635,7 +895,14 @@ int xy_swap_with_decisions(xy_pt *pt, const uint8_t *accept_host) {
 int xy_measure(xy_pt *pt, double *out_host) {
     if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
     const int S = pt->g->S, R = pt->R;
-    const int rc = launch_measure(pt, 0, S, true);
+    int rc;
+    if (use_persistent(pt)) {
+        SweepCtl c;
+        c.end_measure = 2;
+        rc = run_sweep(pt, c, 0u, 0u);
+    } else {
+        rc = launch_measure(pt, 0, S, true);
+    }
     if (rc != XY_OK) return rc;
     pt->e_fresh = true;
     if (out_host) {
@@ -666,10 +933,34 @@ int xy_set_schedule(xy_pt *pt, int samples_per_group) {
     return XY_OK;
 }
 
+int xy_set_path(xy_pt *pt, int path, int balance, int pdl, int l2_persist) {
+    if (!check_pt(pt) || path < 0 || path > 2) return fail(XY_EINVAL, "bad handle or path not in {0, 1, 2}");
+    XY_CUDA(cudaStreamSynchronize(pt->stream));
+    pt->path = path; pt->balance = balance ? 1 : 0; pt->pdl = pdl ? 1 : 0; pt->l2_persist = l2_persist ? 1 : 0;
+    drop_graphs(pt);
+    return XY_OK;
+}
+
 int xy_run(xy_pt *pt, int n_cycles, int sps, int orps, int me) {
     if (!check_pt(pt) || n_cycles < 0 || sps < 1 || orps < 0 || me < 0)
         return fail(XY_EINVAL, "need n_cycles >= 0, sweeps_per_swap >= 1, or_per_sweep >= 0, measure_every >= 0");
+    if (use_persistent(pt)) {   // one persistent launch per sample group runs all n_cycles cycles of the group
+        if (n_cycles == 0) return XY_OK;
+        SweepCtl c;
+        c.n_rep = n_cycles; c.sps = sps; c.do_met = 1; c.orps = orps; c.me = me; c.end_measure = 1; c.do_swap = 1;
+        c.sweep0 = pt->sweep; c.round0 = pt->round;
+        const int rc = run_sweep(pt, c, static_cast<uint32_t>(n_cycles) * static_cast<uint32_t>(sps), static_cast<uint32_t>(n_cycles));
+        if (rc != XY_OK) return rc;
+        pt->sweep += static_cast<uint32_t>(n_cycles) * static_cast<uint32_t>(sps);
+        pt->round += static_cast<uint32_t>(n_cycles);
+        pt->e_fresh = false;
+        return XY_OK;
+    }
     const int group = auto_group(pt);
+    {
+        const int rc = prepare_partitions(pt, group);
+        if (rc != XY_OK) return rc;
+    }
     for (int c = 0; c < n_cycles; ++c) {
         const int phase = me > 0 ? static_cast<int>(pt->sweep % static_cast<uint32_t>(me)) : 0;
         const CycleKey key{sps, orps, me, phase, group};
@@ -688,7 +979,21 @@ int xy_run(xy_pt *pt, int n_cycles, int sps, int orps, int me) {
 int xy_run_sweeps(xy_pt *pt, int n_blocks, int sps, int orps) {
     if (!check_pt(pt) || n_blocks < 0 || sps < 1 || orps < 0)
         return fail(XY_EINVAL, "need n_blocks >= 0, sweeps_per_block >= 1, or_per_sweep >= 0");
+    if (use_persistent(pt)) {
+        if (n_blocks == 0) return XY_OK;
+        SweepCtl c;
+        c.n_rep = n_blocks; c.sps = sps; c.do_met = 1; c.orps = orps; c.sweep0 = pt->sweep;
+        const int rc = run_sweep(pt, c, static_cast<uint32_t>(n_blocks) * static_cast<uint32_t>(sps), 0u);
+        if (rc != XY_OK) return rc;
+        pt->sweep += static_cast<uint32_t>(n_blocks) * static_cast<uint32_t>(sps);
+        pt->e_fresh = false;
+        return XY_OK;
+    }
     const int group = auto_group(pt);
+    {
+        const int rc = prepare_partitions(pt, group);
+        if (rc != XY_OK) return rc;
+    }
     for (int b = 0; b < n_blocks; ++b) {
         const CycleKey key{sps, orps, -1, 0, group};
         CycleGraph *cg = nullptr;
@@ -755,6 +1060,13 @@ int xy_set_labels(xy_pt *pt, const int32_t *temp_of_slot_host) {
 
 int xy_get_energy(xy_pt *pt, double *E_slot_host) {
     if (!check_pt(pt) || !E_slot_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
+    if (!pt->e_fresh && use_persistent(pt)) {
+        SweepCtl c;
+        c.end_measure = 1;
+        const int rc = run_sweep(pt, c, 0u, 0u);
+        if (rc != XY_OK) return rc;
+        pt->e_fresh = true;
+    }
     if (!pt->e_fresh) {
         const int rc = launch_measure(pt, 0, pt->g->S, false);
         if (rc != XY_OK) return rc;

@@ -1,17 +1,8 @@
-// xy_kernels.cuh -- sm_100a kernels of the XY / Levy-graph hot path (see include/xy_b200.h).
-//
-// Layout: theta[S][N][R] fp32, replica (slot) fastest.  A lane owns TWO adjacent slots (one float2 and
-// one Philox4x32-10 call per site: words (x0,x1) feed the even slot, (x2,x3) the odd one), so a group of
-// G = R/2 lanes covers one site and a warp covers SPW = 32/G sites at once.  At R = 64 a warp gathers one
-// neighbour as one 256-byte coalesced request.
-//
-// Work unit = a TILE of TS = CH*SPW consecutive sites of one colour class, owned by one warp:
-//   1. lane m < TS loads rec[i0+m] = {first col_idx entry, degree | n_lower<<16}      (one coalesced load)
-//   2. the tile's neighbour ids are one contiguous run of col_idx (CSR order): staged into the warp's
-//      slice of shared memory with coalesced loads, read back as broadcast LDS
-//   3. row t = sites i0 + t*SPW + sub: own float2, Philox, gather, finish, store.  When SPW == 1 the
-//      degree is warp-uniform and the gather runs exact-degree batches (no predicated-off issue slots).
-// All offsets inside a sample are 32-bit (N*R/2 < 2^31 is checked at xy_pt_create).
+// xy_kernels.cuh -- shared device pieces of the XY / Levy-graph hot path (see include/xy_b200.h):
+// Philox4x32-10, the Metropolis / over-relaxation finishing arithmetic, the angle initialisation, and the LEGACY
+// any-R kernels (one warp per site, lanes stride over the slots; one launch per colour class) that serve replica
+// counts without a float2 flavour (odd R, R = 6, 10, ...).  The product path for R = 2 * 2^k <= 64 and R % 64 == 0
+// is the persistent kernel in xy_sweep.cuh.
 //
 // PAPER.md:444,:454 (coloured single-spin Metropolis), :460 (over-relaxation, ref 66), :167-181 (E, m),
 // :460-472 (parallel tempering); readings R5-R11 in DESIGN.md.
@@ -25,9 +16,8 @@ constexpr float kTwoPiF = 6.2831855f;           // fp32(2 pi)
 constexpr float kTwoPiLo = -1.7484555e-7f;      // 2 pi - fp32(2 pi)
 constexpr float kInvTwoPiF = 0.15915494f;
 constexpr unsigned kFull = 0xffffffffu;
-constexpr int kBlock = 256;                     // threads per CTA in the tile kernels
+constexpr int kBlock = 256;                     // threads per CTA
 constexpr int kWarps = kBlock / 32;
-constexpr int kIdxCap = 192;                    // staged neighbour ids per warp (ints); longer runs read global
 constexpr double kFix = 68719476736.0;          // 2^36: fixed-point scale of the measure reduction
 constexpr double kInvFix = 1.0 / 68719476736.0;
 
@@ -70,7 +60,7 @@ __device__ __forceinline__ float u01(uint32_t x) {
     return fmaf(static_cast<float>(x >> 9), 1.1920928955078125e-07f, 5.9604644775390625e-08f);
 }
 
-// ---- arguments of the tile kernels -----------------------------------------------------------------
+// ---- arguments shared by the update / measure kernels -----------------------------------------------------------------
 struct TileArgs {
     const int2 *rec;           // [S][N] {first col_idx entry (absolute), degree | n_lower << 16}
     const int32_t *col_idx;    // concatenated neighbour ids (local to the sample), ascending per site
@@ -166,258 +156,6 @@ __device__ __forceinline__ float overrelax_finish(float own, float hx, float hy)
     if (t < 0.0f) t += kTwoPiF;
     if (t >= kTwoPiF) t -= kTwoPiF;
     return t;
-}
-
-// ---- per-lane state of one row (two slots) ------------------------------------------------------------
-template <int MODE> struct RowAcc;
-
-template <> struct RowAcc<kModeMetropolis> {
-    float midx, midy, ax = 0.f, ay = 0.f;
-    __device__ __forceinline__ void add(const float2 t) {
-        ax += __sinf(midx - t.x);
-        ay += __sinf(midy - t.y);
-    }
-};
-template <> struct RowAcc<kModeOverrelax> {
-    float hxx = 0.f, hyx = 0.f, hxy = 0.f, hyy = 0.f;   // (hxx, hyx) = field of the .x slot
-    __device__ __forceinline__ void add(const float2 t) {
-        float sn, cs;
-        __sincosf(t.x, &sn, &cs);
-        hxx += cs; hyx += sn;
-        __sincosf(t.y, &sn, &cs);
-        hxy += cs; hyy += sn;
-    }
-};
-template <> struct RowAcc<kModeMeasure> {
-    float ownx, owny, ex = 0.f, ey = 0.f;
-    __device__ __forceinline__ void add(const float2 t) {
-        ex += __cosf(ownx - t.x);
-        ey += __cosf(owny - t.y);
-    }
-};
-
-// neighbour id k of the run: staged copy (broadcast LDS) or, for over-long runs, global
-__device__ __forceinline__ int nbr_id(const int32_t *sidx, const int32_t *gidx, bool staged, int pos) {
-    return staged ? sidx[pos] : __ldg(gidx + pos);
-}
-
-// exact-degree gather for warp-uniform degree: D loads back to back, then D accumulations
-template <int D, typename ACC>
-__device__ __forceinline__ void gather_batch(ACC &acc, const float2 *__restrict__ base_q, uint32_t stride,
-                                             const int32_t *sidx, const int32_t *gidx, bool staged, int pos) {
-    float2 t[D];
-#pragma unroll
-    for (int u = 0; u < D; ++u) {
-        const uint32_t j = static_cast<uint32_t>(nbr_id(sidx, gidx, staged, pos + u));
-        t[u] = base_q[j * stride];
-    }
-#pragma unroll
-    for (int u = 0; u < D; ++u) acc.add(t[u]);
-}
-
-template <typename ACC>
-__device__ __forceinline__ void gather_uniform(ACC &acc, const float2 *__restrict__ base_q, uint32_t stride,
-                                               const int32_t *sidx, const int32_t *gidx, bool staged, int pos,
-                                               int cnt) {
-    while (cnt >= 8) {
-        gather_batch<8>(acc, base_q, stride, sidx, gidx, staged, pos);
-        pos += 8; cnt -= 8;
-    }
-    switch (cnt) {
-        case 7: gather_batch<7>(acc, base_q, stride, sidx, gidx, staged, pos); break;
-        case 6: gather_batch<6>(acc, base_q, stride, sidx, gidx, staged, pos); break;
-        case 5: gather_batch<5>(acc, base_q, stride, sidx, gidx, staged, pos); break;
-        case 4: gather_batch<4>(acc, base_q, stride, sidx, gidx, staged, pos); break;
-        case 3: gather_batch<3>(acc, base_q, stride, sidx, gidx, staged, pos); break;
-        case 2: gather_batch<2>(acc, base_q, stride, sidx, gidx, staged, pos); break;
-        case 1: gather_batch<1>(acc, base_q, stride, sidx, gidx, staged, pos); break;
-        default: break;
-    }
-}
-
-// several sites per warp: degrees differ between the lane groups; run to the warp maximum, absent
-// neighbours are replaced by a harmless in-range load and left out of the sum
-template <typename ACC>
-__device__ __forceinline__ void gather_divergent(ACC &acc, const float2 *__restrict__ base_q, uint32_t stride,
-                                                 const int32_t *sidx, const int32_t *gidx, bool staged, int pos,
-                                                 int cnt, int cntmax, uint32_t safe_site) {
-    for (int k = 0; k < cntmax; k += 4) {
-        float2 t[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            uint32_t j = safe_site;
-            if (k + u < cnt) j = static_cast<uint32_t>(nbr_id(sidx, gidx, staged, pos + k + u));
-            t[u] = base_q[j * stride];
-        }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            ACC trial = acc;
-            trial.add(t[u]);
-            if (k + u < cnt) acc = trial;
-        }
-    }
-}
-
-// ---- the tile kernel: MODE 0 Metropolis / 1 over-relaxation on one colour class, 2 measure on all sites ----
-// R = 2G (G a power of two <= 32, CB = 1: stride known at compile time) or R a multiple of 64 (G = 32,
-// CB = 0: blockIdx.z = block of 64 slots).
-template <int G, int CB, int MODE>
-__global__ void __launch_bounds__(kBlock) k_tile(const TileArgs a) {
-    constexpr int SPW = 32 / G;                 // sites per row
-    constexpr int CH = G < 8 ? G : 8;           // rows per tile
-    constexpr int TS = CH * SPW;                // sites per tile (<= 32)
-    __shared__ int32_t s_idx[kWarps][kIdxCap];
-    __shared__ double s_red[MODE == kModeMeasure ? kWarps * 32 * 6 : 1];
-    __shared__ int s_last;
-
-    const int s = a.s0 + blockIdx.y;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int sub = lane / G, l = lane % G;
-    const uint32_t R2 = CB ? static_cast<uint32_t>(G) : static_cast<uint32_t>(a.R >> 1);
-    const int q = blockIdx.z * G + l;            // slot pair handled by this lane
-
-    int cbeg = 0, cend = a.N;
-    if constexpr (MODE != kModeMeasure) {
-        cbeg = a.class_ptr[s * a.q_stride + a.colour];
-        cend = a.class_ptr[s * a.q_stride + a.colour + 1];
-    }
-    const int n_tiles = (cend - cbeg + TS - 1) / TS;
-    const int tile0 = (blockIdx.x * kWarps + warp) * a.tiles_per_warp;
-    const int tile1 = min(tile0 + a.tiles_per_warp, n_tiles);
-
-    float2 *__restrict__ base_q = reinterpret_cast<float2 *>(a.theta) + static_cast<size_t>(s) * a.N * R2 + q;
-    const int2 *__restrict__ rec = a.rec + static_cast<size_t>(s) * a.N;
-    int32_t *sidx = s_idx[warp];
-
-    float2 beta = make_float2(0.f, 0.f), w = make_float2(0.f, 0.f);
-    uint32_t sweep = 0, c2 = 0;
-    if constexpr (MODE == kModeMetropolis) {
-        beta = reinterpret_cast<const float2 *>(a.beta_slot)[static_cast<size_t>(s) * R2 + q];
-        w = reinterpret_cast<const float2 *>(a.w_slot)[static_cast<size_t>(s) * R2 + q];
-        sweep = a.use_counter ? a.counters[0] + static_cast<uint32_t>(a.sweep_offset) : a.sweep_fixed;
-        c2 = ((a.sample_base + static_cast<uint32_t>(s)) << 16) | static_cast<uint32_t>(q);
-    }
-    double dacc[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};   // measure: E, Mx, My of the .x slot, then of the .y slot
-
-    for (int tile = tile0; tile < tile1; ++tile) {
-        const int i0 = cbeg + tile * TS;
-        const int nsite = min(TS, cend - i0);
-        int2 rc = make_int2(0, 0);
-        if (lane < nsite) rc = rec[i0 + lane];
-        const int start0 = __shfl_sync(kFull, rc.x, 0);
-        const int n_run = __shfl_sync(kFull, rc.x + (rc.y & 0xffff), nsite - 1) - start0;
-        const bool staged = n_run <= kIdxCap;
-        const int32_t *gidx = a.col_idx + start0;
-        if (staged)
-            for (int p = lane; p < n_run; p += 32) sidx[p] = gidx[p];
-        __syncwarp();
-
-        float fe[4] = {0.f, 0.f, 0.f, 0.f};   // measure: per-tile fp32 partials ex, ey (bond sums)
-        float fm[4] = {0.f, 0.f, 0.f, 0.f};   // measure: mx.x, my.x, mx.y, my.y
-        float2 own_next = make_float2(0.f, 0.f);
-        if (sub < nsite) own_next = base_q[static_cast<uint32_t>(i0 + sub) * R2];
-#pragma unroll 1
-        for (int t = 0; t < CH; ++t) {
-            const int m = t * SPW + sub;          // position of this lane's site in the tile
-            if (t * SPW >= nsite) break;          // warp-uniform
-            const bool valid = m < nsite;
-            const int i = i0 + m;
-            const float2 own = own_next;
-            if (t + 1 < CH && m + SPW < nsite) own_next = base_q[static_cast<uint32_t>(i + SPW) * R2];
-            const int ry = __shfl_sync(kFull, rc.y, m & 31);
-            const int rx = __shfl_sync(kFull, rc.x, m & 31);
-            int deg = valid ? (ry & 0xffff) : 0;
-            int pos = rx - start0;
-            if constexpr (MODE == kModeMeasure) {           // bonds counted once: neighbours j > i are the tail of the list
-                const int nlow = valid ? (ry >> 16) : 0;
-                pos += nlow;
-                deg -= nlow;
-            }
-
-            RowAcc<MODE> acc;
-            float thpx = 0.f, thpy = 0.f, halfx = 0.f, halfy = 0.f, u2x = 0.f, u2y = 0.f;
-            if constexpr (MODE == kModeMetropolis) {
-                uint32_t x[4];
-                philox4x32_10(static_cast<uint32_t>(i), sweep, c2, kDomMetropolis, a.keys, x);
-                const float dx = __fmul_rn(w.x, u01(x[0]) - 0.5f);
-                const float dy = __fmul_rn(w.y, u01(x[2]) - 0.5f);
-                u2x = u01(x[1]);
-                u2y = u01(x[3]);
-                thpx = __fadd_rn(own.x, dx);
-                thpy = __fadd_rn(own.y, dy);
-                halfx = 0.5f * (thpx - own.x);
-                halfy = 0.5f * (thpy - own.y);
-                acc.midx = own.x + halfx;
-                acc.midy = own.y + halfy;
-            }
-            if constexpr (MODE == kModeMeasure) { acc.ownx = own.x; acc.owny = own.y; }
-
-            if constexpr (SPW == 1) {
-                gather_uniform(acc, base_q, R2, sidx, gidx, staged, pos, deg);
-            } else {
-                const int degmax = __reduce_max_sync(kFull, deg);
-                gather_divergent(acc, base_q, R2, sidx, gidx, staged, pos, deg, degmax,
-                                 static_cast<uint32_t>(min(i, a.N - 1)));
-            }
-
-            if constexpr (MODE == kModeMetropolis) {
-                if (valid) {
-                    float2 out;
-                    out.x = metropolis_finish(own.x, thpx, halfx, acc.ax, beta.x, u2x);
-                    out.y = metropolis_finish(own.y, thpy, halfy, acc.ay, beta.y, u2y);
-                    base_q[static_cast<uint32_t>(i) * R2] = out;
-                }
-            } else if constexpr (MODE == kModeOverrelax) {
-                if (valid) {
-                    float2 out;
-                    out.x = overrelax_finish(own.x, acc.hxx, acc.hyx);
-                    out.y = overrelax_finish(own.y, acc.hxy, acc.hyy);
-                    base_q[static_cast<uint32_t>(i) * R2] = out;
-                }
-            } else {
-                if (valid) {
-                    float sn, cs;
-                    fe[0] += acc.ex; fe[1] += acc.ey;
-                    __sincosf(own.x, &sn, &cs);
-                    fm[0] += cs; fm[1] += sn;
-                    __sincosf(own.y, &sn, &cs);
-                    fm[2] += cs; fm[3] += sn;
-                }
-            }
-        }
-        if constexpr (MODE == kModeMeasure) {
-            dacc[0] -= static_cast<double>(fe[0]); dacc[1] += static_cast<double>(fm[0]); dacc[2] += static_cast<double>(fm[1]);
-            dacc[3] -= static_cast<double>(fe[1]); dacc[4] += static_cast<double>(fm[2]); dacc[5] += static_cast<double>(fm[3]);
-        }
-        __syncwarp();
-    }
-
-    if constexpr (MODE == kModeMeasure) {
-        // CTA reduction in a fixed order, then exact (order-independent) fixed-point accumulation
-#pragma unroll
-        for (int c = 0; c < 6; ++c) s_red[(warp * 32 + lane) * 6 + c] = dacc[c];
-        __syncthreads();
-        if (threadIdx.x < G * 6) {
-            const int ll = threadIdx.x / 6, c = threadIdx.x % 6;
-            double v = 0.0;
-            for (int wi = 0; wi < kWarps; ++wi)
-                for (int sb = 0; sb < SPW; ++sb) v += s_red[(wi * 32 + sb * G + ll) * 6 + c];
-            const int slot = 2 * (blockIdx.z * G + ll) + c / 3;
-            atomicAdd(reinterpret_cast<unsigned long long *>(a.fx) + (static_cast<size_t>(s) * a.R + slot) * 3 + c % 3,
-                      static_cast<unsigned long long>(__double2ll_rn(v * kFix)));
-        }
-        __threadfence();
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            const unsigned int total = gridDim.x * gridDim.z;
-            s_last = (atomicAdd(a.ticket + s, 1u) == total - 1u) ? 1 : 0;
-        }
-        __syncthreads();
-        if (s_last) {
-            __threadfence();
-            measure_finalize(a, s);
-        }
-    }
 }
 
 // ---- generic path: any R >= 1 (odd R, R = 6, ...): one warp per site, lanes stride over the slots ----

@@ -1,0 +1,751 @@
+// xy_sweep.cuh -- the persistent sweep kernel: every step of the hot path (Metropolis and over-relaxation colour
+// classes, E / M reductions with accumulation, parallel-tempering swap) for one group of samples in ONE launch.
+//
+// Why one kernel (profiles/r1c_full.md): with one launch per colour class the ramp-up (four
+// dependent global latencies before the first update) and the tail of the slowest warp were paid 100 times per
+// PT cycle and sample: 21 % of the cycles had no resident warp.  Here a cooperative grid stays resident and the
+// colour classes are PHASES separated by a per-sample barrier (samples never interact, so CTAs of
+// different samples never wait for one another).  The whole of xy_run(n_cycles) for a sample group is one launch.
+//
+// Work layout inside a phase: theta[S][N][R] fp32, replica fastest.  A lane owns TWO adjacent slots (one float2,
+// one Philox4x32-10 call per site: words (x0,x1) feed the even slot, (x2,x3) the odd one), G = R/2 lanes cover a
+// site (G = 32 and column blocks of 64 slots when R % 64 == 0) and a warp works on SPW = 32/G sites at once
+// ("row").  At R = 64 one neighbour gather is one fully used 256-byte request.  A warp owns a contiguous share of
+// the colour class and walks it in chunks of <= 32 sites: one coalesced load of the chunk's rec[], the chunk's
+// neighbour ids (one contiguous CSR run) staged in the warp's slice of shared memory, pre-scaled by the site
+// stride.  Same-colour sites share no bond, so the gathers of row t+1 never read what row t stores:
+// they are issued BEFORE row t is computed, as cp.async (LDGSTS) copies of the lane's own 8 bytes into a per-warp
+// ring in shared memory -- in-flight data costs no registers, each lane reads back only what it copied itself
+// (cp.async.wait_group, no cross-lane synchronisation), and the Philox / sin / exp work of row t covers the
+// latency of row t+1.  When SPW > 1 the sites of a row have different degrees: the loops run to the row maximum
+// and lanes whose site has fewer neighbours are predicated off (no memory request is made for them).
+//
+// PAPER.md:444,:454 (coloured single-spin Metropolis), :460 (over-relaxation, ref 66), :167-181 (E, m),
+// :460-472 (parallel tempering); readings R5-R11 in DESIGN.md.
+#pragma once
+#include "xy_kernels.cuh"
+
+namespace xy {
+
+constexpr int kDB = 8;            // pipelined gathers per site
+constexpr int kDepth = 2;         // ring slots per warp (rows in flight)
+constexpr int kStageCap = 256;    // staged neighbour ids per warp and chunk (ints)
+#ifndef XY_SWEEP_MIN_BLOCKS
+#define XY_SWEEP_MIN_BLOCKS 4
+#endif
+constexpr int kSweepMinBlocks = XY_SWEEP_MIN_BLOCKS;   // resident CTAs per SM the register / shared budget is sized for
+
+// fixed-point scales of the measure reduction (exact, order-independent integer sums; see quant8 / quant1)
+constexpr double kInvScaleE = 1.0 / 524288.0;      // 2^-19
+constexpr double kInvScaleM = 1.0 / 4194304.0;     // 2^-22
+
+// per warp: ring[kDepth][kDB + 1][32] float2 (row kDB = the site's own angle) + staged ids
+struct __align__(16) SweepWarp {
+    float2 ring[kDepth][kDB + 1][32];
+    uint32_t idx[kStageCap];
+};
+static_assert(sizeof(SweepWarp) * kWarps <= 48 * 1024 - 64, "static shared memory limit");
+static_assert(sizeof(SweepWarp) * kWarps >= sizeof(long long) * kWarps * 32 * 6, "measure reduction reuses the ring");
+
+// ---- packed fp32x2 helpers (IEEE rn per component: bit-identical to the scalar operations) ----------
+__device__ __forceinline__ float2 add2(const float2 a, const float2 b) {
+    float2 r;
+    asm("{ .reg .b64 ra, rb, rc; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; add.rn.f32x2 rc, ra, rb; mov.b64 {%0,%1}, rc; }"
+        : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+__device__ __forceinline__ float2 sub2(const float2 a, const float2 b) { return add2(a, make_float2(-b.x, -b.y)); }
+__device__ __forceinline__ float2 mul2(const float2 a, const float2 b) {
+    float2 r;
+    asm("{ .reg .b64 ra, rb, rc; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; mul.rn.f32x2 rc, ra, rb; mov.b64 {%0,%1}, rc; }"
+        : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+
+// as_float((x >> 9) | 0x3f800000) = 1 + k 2^-23, k = x >> 9
+__device__ __forceinline__ float mant12(uint32_t x) { return __uint_as_float((x >> 9) | 0x3f800000u); }
+
+// float -> fixed point by the magic-number add (one FADD.rn + one IADD, deterministic):
+//   |x| <= 8:  x + 24 lies in [16, 32], ulp 2^-19, so bits(x + 24) - bits(24) = rn(x 2^19)
+//   |x| <= 1:  x + 3  lies in [2, 4],   ulp 2^-22, so bits(x + 3)  - bits(3)  = rn(x 2^22)
+__device__ __forceinline__ int quant8(float x) { return __float_as_int(__fadd_rn(x, 24.0f)) - 0x41C00000; }
+__device__ __forceinline__ int quant1(float x) { return __float_as_int(__fadd_rn(x, 3.0f)) - 0x40400000; }
+
+// ---- cp.async (LDGSTS): 8 bytes per lane, global -> shared, no register staging ---------------------------
+__device__ __forceinline__ void cp_async8(uint32_t smem_addr, const void *gptr) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_addr), "l"(gptr) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+__device__ __forceinline__ unsigned ld_relaxed_gpu(const unsigned *p) {
+    unsigned v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// ---- per-lane state of one site (two slots) ----------------------------------------------------------
+template <int MODE> struct PairAcc;
+template <> struct PairAcc<kModeMetropolis> {
+    float2 mid, s = make_float2(0.f, 0.f);
+    __device__ __forceinline__ void add(const float2 t) {
+        const float2 d = sub2(mid, t);
+        s = add2(s, make_float2(__sinf(d.x), __sinf(d.y)));
+    }
+};
+template <> struct PairAcc<kModeOverrelax> {
+    float2 hx = make_float2(0.f, 0.f), hy = make_float2(0.f, 0.f);   // hx = (h_x of slot .x, h_x of slot .y)
+    __device__ __forceinline__ void add(const float2 t) {
+        float sx, cx, sy, cy;
+        __sincosf(t.x, &sx, &cx);
+        __sincosf(t.y, &sy, &cy);
+        hx = add2(hx, make_float2(cx, cy));
+        hy = add2(hy, make_float2(sx, sy));
+    }
+};
+template <> struct PairAcc<kModeMeasure> {
+    float2 own, e = make_float2(0.f, 0.f);
+    __device__ __forceinline__ void add(const float2 t) {
+        const float2 d = sub2(own, t);
+        e = add2(e, make_float2(__cosf(d.x), __cosf(d.y)));
+    }
+    // fixed-point flush after every batch of <= 8 bonds (|e| <= 8): the integer sums do not depend on who adds them
+    __device__ __forceinline__ void flush(long long &ex, long long &ey) {
+        ex += quant8(e.x); ey += quant8(e.y);
+        e = make_float2(0.f, 0.f);
+    }
+};
+
+// per-lane description of the site a lane works on in the current row (warp-uniform when SPW == 1)
+struct RowSite { int i, deg, pos; bool valid; };
+
+// direct gather of the neighbour with pre-scaled id `sid` (float2 units), L2 only: one IMAD.WIDE.U32 + one LDG.64
+__device__ __forceinline__ float2 sweep_ld(const float2 *lb, uint32_t sid) {
+    return __ldcg(lb + static_cast<unsigned long long>(sid));
+}
+
+// issue D async gathers back to back; UNI: every lane has at least D neighbours (nothing predicated off)
+template <int D, bool UNI>
+__device__ __forceinline__ void sweep_issue_n(uint32_t row0, const float2 *lb, const uint32_t *sidx, int pos, int deg) {
+    uint32_t sid[D];
+#pragma unroll
+    for (int u = 0; u < D; ++u) {      // all id loads first: LDS -> LDGSTS hazards are paid once
+        sid[u] = 0u;
+        if (UNI || u < deg) sid[u] = sidx[pos + u];
+    }
+#pragma unroll
+    for (int u = 0; u < D; ++u)
+        if (UNI || u < deg) cp_async8(row0 + u * 256u, lb + static_cast<unsigned long long>(sid[u]));
+}
+
+// row0 = shared address of this lane's 8 bytes in row 0 of the ring slot; dmax = warp maximum of deg
+template <bool UNI>
+__device__ __forceinline__ void sweep_issue(uint32_t row0, const float2 *lb, const uint32_t *sidx, int pos, int deg, int dmax) {
+    switch (dmax < kDB ? dmax : kDB) {
+        case 8: sweep_issue_n<8, UNI>(row0, lb, sidx, pos, deg); break;
+        case 7: sweep_issue_n<7, UNI>(row0, lb, sidx, pos, deg); break;
+        case 6: sweep_issue_n<6, UNI>(row0, lb, sidx, pos, deg); break;
+        case 5: sweep_issue_n<5, UNI>(row0, lb, sidx, pos, deg); break;
+        case 4: sweep_issue_n<4, UNI>(row0, lb, sidx, pos, deg); break;
+        case 3: sweep_issue_n<3, UNI>(row0, lb, sidx, pos, deg); break;
+        case 2: sweep_issue_n<2, UNI>(row0, lb, sidx, pos, deg); break;
+        case 1: sweep_issue_n<1, UNI>(row0, lb, sidx, pos, deg); break;
+        default: break;
+    }
+}
+
+// batches of <= 4 LDS.64 then their arithmetic (8 at once would cost 16 registers at the kernel's pressure peak)
+template <int D, bool UNI, typename ACC>
+__device__ __forceinline__ void sweep_consume_n(ACC &acc, const float2 *row0, int deg) {
+#pragma unroll
+    for (int b = 0; b < D; b += 4) {
+        float2 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (b + u < D) v[u] = row0[(b + u) * 32];
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (b + u < D && (UNI || b + u < deg)) acc.add(v[u]);
+    }
+}
+
+// row0 = pointer to this lane's float2 in row 0 of the ring slot: the first min(deg, kDB) neighbours
+template <bool UNI, typename ACC>
+__device__ __forceinline__ void sweep_consume(ACC &acc, const float2 *row0, int deg, int dmax) {
+    switch (dmax < kDB ? dmax : kDB) {
+        case 8: sweep_consume_n<8, UNI>(acc, row0, deg); break;
+        case 7: sweep_consume_n<7, UNI>(acc, row0, deg); break;
+        case 6: sweep_consume_n<6, UNI>(acc, row0, deg); break;
+        case 5: sweep_consume_n<5, UNI>(acc, row0, deg); break;
+        case 4: sweep_consume_n<4, UNI>(acc, row0, deg); break;
+        case 3: sweep_consume_n<3, UNI>(acc, row0, deg); break;
+        case 2: sweep_consume_n<2, UNI>(acc, row0, deg); break;
+        case 1: sweep_consume_n<1, UNI>(acc, row0, deg); break;
+        default: break;
+    }
+}
+
+// ---- arguments ---------------------------------------------------------------------------------------------
+// One launch runs, for every sample of the group (blockIdx.y):
+//   repeat n_rep times:
+//     for k = 1..sps:  sweep = sweep0 + rep*sps + k
+//        if do_met:  Metropolis on colours c_lo..c_hi-1
+//        orps x [ over-relaxation on colours c_lo..c_hi-1 ]
+//        if me > 0 and sweep % me == 0:  measure + accumulate
+//     end_measure: 1 = E per slot unless just measured (no accumulation), 2 = measure + accumulate
+//     if do_swap:  one swap round (round0 + rep)
+struct SweepArgs {
+    TileArgs t;
+    int n_rep, sps, do_met, orps, me, end_measure, do_swap, c_lo, c_hi;
+    uint32_t sweep0, round0;
+    unsigned int *bar;             // [S] per-sample barrier counters, zero at launch
+    const int32_t *part;           // [S][q_stride][nw + 1] cost-balanced first site of every warp's share (colour q_max =
+                                   // the measure pass over all sites), nw = gridDim.x * kWarps; nullptr = equal shares
+    // swap round
+    const double *betaT;           // [R] 1/T fp64
+    const float *beta_f, *w_f;     // [R]
+    int32_t *slot_of_temp, *temp_of_slot;   // [S][R]
+    float *beta_slot, *w_slot;     // [S][R]
+    const uint8_t *decisions;      // [S][R] or nullptr
+    long long *attempts, *accepts; // [S][R]
+};
+
+// barrier of the CTAs that work on one sample (gridDim.x * gridDim.z of them), split in two halves so that work
+// that does not depend on the other CTAs (staging the next phase's graph data) overlaps the barrier latency.
+// `target` counts arrivals so far.  Thread 0 releases the CTA's stores (fence) and arrives; later it polls with
+// relaxed loads, and its trailing fence + bar.sync order every thread's later (weak, L1-cached) loads after the
+// other CTAs' stores, as cooperative groups' grid sync does (MEMBAR.SC.GPU + CCTL.IVALL in SASS).
+__device__ __forceinline__ void sample_barrier_arrive(unsigned int *bar, unsigned int &target, unsigned int n_cta) {
+    __syncthreads();
+    target += n_cta;
+    if (n_cta > 1u && threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(bar, 1u);
+    }
+}
+__device__ __forceinline__ void sample_barrier_wait(const unsigned int *bar, unsigned int target, unsigned int n_cta) {
+    if (n_cta > 1u) {
+        if (threadIdx.x == 0) {
+            while (ld_relaxed_gpu(bar) < target) { }     // relaxed polls: no L1 invalidation per iteration
+            __threadfence();                              // acquire side: MEMBAR + CCTL.IVALL once
+        }
+    }
+    __syncthreads();
+}
+
+// ---- phase sequencing (uniform over the grid) ---------------------------------------------------------------
+enum : int { kPhaseSwap = 3 };
+struct PhaseDesc { int mode, colour; uint32_t sweep; int flag; };   // flag: measure -> accumulate; swap: sweep = round
+struct PhaseIter { int rep = 0, k = 1, stage = 0, c = 0, o = 0; bool fresh = false; };
+
+// the order of DESIGN.md section 2 as a state machine; returns false when the launch is complete
+__device__ __forceinline__ bool next_phase(const SweepArgs &a, PhaseIter &it, PhaseDesc &d) {
+    for (;;) {
+        if (it.rep >= a.n_rep) return false;
+        const uint32_t sweep = a.sweep0 + static_cast<uint32_t>(it.rep) * static_cast<uint32_t>(a.sps) + static_cast<uint32_t>(it.k);
+        switch (it.stage) {
+            case 0:     // Metropolis colours of sweep k
+                if (it.k > a.sps) { it.stage = 3; break; }
+                if (a.do_met && it.c < a.c_hi) { d = PhaseDesc{kModeMetropolis, it.c++, sweep, 0}; return true; }
+                it.stage = 1; it.c = a.c_lo; it.o = 0;
+                break;
+            case 1:     // orps over-relaxation sweeps
+                if (it.o < a.orps) {
+                    if (it.c < a.c_hi) { d = PhaseDesc{kModeOverrelax, it.c++, 0u, 0}; return true; }
+                    it.o++; it.c = a.c_lo;
+                    break;
+                }
+                it.stage = 2;
+                break;
+            case 2:     // measurement of sweep k
+                it.stage = 0; it.c = a.c_lo; it.k++; it.fresh = false;
+                if (a.me > 0 && sweep % static_cast<uint32_t>(a.me) == 0u) {
+                    it.fresh = true;
+                    d = PhaseDesc{kModeMeasure, 0, 0u, 1};
+                    return true;
+                }
+                break;
+            case 3:     // energies for the swap / an explicit xy_measure
+                it.stage = 4;
+                if (a.end_measure == 2 || (a.end_measure == 1 && !it.fresh)) {
+                    d = PhaseDesc{kModeMeasure, 0, 0u, a.end_measure == 2 ? 1 : 0};
+                    return true;
+                }
+                break;
+            case 4:     // swap round
+                it.stage = 5;
+                if (a.do_swap) { d = PhaseDesc{kPhaseSwap, 0, a.round0 + static_cast<uint32_t>(it.rep), 0}; return true; }
+                break;
+            default:
+                it.rep++; it.k = 1; it.stage = 0; it.c = a.c_lo; it.fresh = false;
+                break;
+        }
+    }
+}
+
+// per-thread constants of a launch
+struct SweepCtx {
+    float2 *lb;                 // this lane's column of the sample: theta2 + s*N*R2 + q
+    const int2 *rec;            // rec of the sample
+    uint32_t *sidx;             // the warp's staged ids
+    const float2 *ring_l;       // this lane's column of the warp's ring (generic pointer)
+    uint32_t ring_s;            // same, shared-space address
+    int s, lane, warp, sub, q;
+};
+
+// what a warp stages for a phase BEFORE the barrier that opens it (graph data only, never theta): its share
+// [i0, w1) of the colour class, the rec[] of the share's first chunk, and that chunk's neighbour ids in shared memory
+struct PhasePrep { int i0, w1; int2 rc; };
+
+// leading sites of a chunk whose neighbour ids fit the staging slice; start0 = first col_idx entry of the chunk,
+// endl = end of this lane's list relative to start0
+__device__ __forceinline__ int chunk_fit(const int2 rc, int lane, int nsite, int &start0, int &endl) {
+    start0 = __shfl_sync(kFull, rc.x, 0);
+    endl = rc.x + (rc.y & 0xffff) - start0;
+    const unsigned fits = __ballot_sync(kFull, lane < nsite && endl <= kStageCap);
+    return fits == kFull ? 32 : __ffs(~fits) - 1;
+}
+
+// stage the chunk's ids (pre-scaled by the site stride): 4 loads in flight per lane
+__device__ __forceinline__ void chunk_stage(const int32_t *gidx, uint32_t *sidx, int lane, int n_run, uint32_t R2) {
+    for (int p0 = 0; p0 < n_run; p0 += 128) {
+        int32_t g[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (p0 + u * 32 + lane < n_run) g[u] = gidx[p0 + u * 32 + lane];
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (p0 + u * 32 + lane < n_run) sidx[p0 + u * 32 + lane] = static_cast<uint32_t>(g[u]) * R2;
+    }
+}
+
+template <int G, int CB>
+__device__ __forceinline__ PhasePrep sweep_prep(const SweepArgs &sa, const SweepCtx &x, int mode, int colour) {
+    constexpr int SPW = 32 / G;
+    const TileArgs &a = sa.t;
+    const uint32_t R2 = CB ? static_cast<uint32_t>(G) : static_cast<uint32_t>(a.R >> 1);
+    PhasePrep P;
+    P.rc = make_int2(0, 0);
+    const int nw = gridDim.x * kWarps, gw = blockIdx.x * kWarps + x.warp;
+    const int cidx = mode == kModeMeasure ? a.q_stride - 1 : colour;
+    if (sa.part) {      // cost-balanced shares (host-computed: cost = const + degree)
+        const int32_t *pp = sa.part + (static_cast<size_t>(x.s) * a.q_stride + cidx) * (nw + 1) + gw;
+        P.i0 = pp[0]; P.w1 = pp[1];
+    } else {            // contiguous equal shares (whole rows)
+        int cbeg = 0, cend = a.N;
+        if (mode != kModeMeasure) {
+            cbeg = a.class_ptr[x.s * a.q_stride + colour];
+            cend = a.class_ptr[x.s * a.q_stride + colour + 1];
+        }
+        const int per = ((cend - cbeg + nw - 1) / nw + SPW - 1) / SPW * SPW;
+        P.i0 = min(cend, cbeg + gw * per); P.w1 = min(cend, P.i0 + per);
+    }
+    if (P.i0 < P.w1) {
+        const int nsite = min(32, P.w1 - P.i0);
+        if (x.lane < nsite) P.rc = x.rec[P.i0 + x.lane];
+        int start0, endl;
+        const int msite = chunk_fit(P.rc, x.lane, nsite, start0, endl);
+        if (msite > 0) chunk_stage(a.col_idx + start0, x.sidx, x.lane, __shfl_sync(kFull, endl, msite - 1), R2);
+    }
+    return P;
+}
+
+// ---- one phase: MODE 0 Metropolis / 1 over-relaxation on a colour class, 2 measure on all sites ----
+// G lanes per site; CB = 1: the site stride R/2 equals G (known at compile time), CB = 0: G = 32, R a multiple of 64
+// larger than 64 (blockIdx.z = block of 64 slots).  P: the share and its first chunk as staged by sweep_prep (the
+// staged ids are visible: a bar.sync separates the two).  iacc: measure only, fixed-point sums (E, Mx, My) of the
+// .x slot, then of the .y slot.
+template <int G, int CB, int MODE>
+__device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x, const PhasePrep &P, uint32_t sweep,
+                                            long long (&iacc)[6]) {
+    constexpr int SPW = 32 / G;
+    constexpr bool UNI = SPW == 1;
+    const uint32_t R2 = CB ? static_cast<uint32_t>(G) : static_cast<uint32_t>(a.R >> 1);
+    constexpr uint32_t kSlotBytes = (kDB + 1) * 32 * sizeof(float2);
+    constexpr int kSlotElems = (kDB + 1) * 32;
+    const int s = x.s, lane = x.lane, sub = x.sub;
+    float2 *lb = x.lb;
+    const int2 *__restrict__ rec = x.rec;
+    uint32_t *sidx = x.sidx;
+    const int w1 = P.w1;
+    if (P.i0 >= w1) return;
+
+    float2 nbeta = make_float2(0.f, 0.f), w = make_float2(0.f, 0.f);
+    uint32_t c2 = 0;
+    if constexpr (MODE == kModeMetropolis) {
+        const float2 b = __ldcg(reinterpret_cast<const float2 *>(a.beta_slot) + static_cast<size_t>(s) * R2 + x.q);
+        nbeta = make_float2(-b.x, -b.y);
+        w = __ldcg(reinterpret_cast<const float2 *>(a.w_slot) + static_cast<size_t>(s) * R2 + x.q);
+        c2 = ((a.sample_base + static_cast<uint32_t>(s)) << 16) | static_cast<uint32_t>(x.q);
+    }
+
+    // Metropolis proposal of site i (both slots of the lane): th' = th + w (u1 - 1/2), half = (th' - th)/2
+    auto begin = [&](int i, const float2 own, PairAcc<MODE> &acc, float2 &thp, float2 &u2) {
+        if constexpr (MODE == kModeMetropolis) {
+            uint32_t r[4];
+            philox4x32_10(static_cast<uint32_t>(i), sweep, c2, kDomMetropolis, a.keys, r);
+            // u = (k + 1/2) 2^-23 with k = x >> 9 (R11), every step exact:
+            //   u1 - 1/2 = ((1 + k 2^-23) - 3/2) + 2^-24,   u2 = (1 + k 2^-23) - (1 - 2^-24)
+            const float2 u1mh = add2(add2(make_float2(mant12(r[0]), mant12(r[2])), make_float2(-1.5f, -1.5f)),
+                                     make_float2(5.9604644775390625e-08f, 5.9604644775390625e-08f));
+            u2 = add2(make_float2(mant12(r[1]), mant12(r[3])), make_float2(-0.99999994f, -0.99999994f));
+            // R5: delta = fp32(w * (u1 - 1/2)), th' = fp32(th + delta): two roundings.  Scalar mul.rn / add.rn on purpose:
+            // ptxas contracts mul.rn.f32x2 + add.rn.f32x2 into one FFMA2 (single rounding, 1 ulp off in 11 % of the moves)
+            thp = make_float2(__fadd_rn(own.x, __fmul_rn(w.x, u1mh.x)), __fadd_rn(own.y, __fmul_rn(w.y, u1mh.y)));
+            acc.mid = add2(own, mul2(sub2(thp, own), make_float2(0.5f, 0.5f)));
+        } else if constexpr (MODE == kModeMeasure) {
+            acc.own = own;
+        }
+    };
+    auto finish = [&](int i, bool valid, const float2 own, PairAcc<MODE> &acc, const float2 thp, const float2 u2) {
+        if constexpr (MODE == kModeMetropolis) {
+            // dE = 2 sin((th'-th)/2) sum_j sin((th'+th)/2 - th_j)
+            const float2 half = mul2(sub2(thp, own), make_float2(0.5f, 0.5f));      // recomputed: two registers fewer across the gather
+            const float2 sh = make_float2(__sinf(half.x), __sinf(half.y));
+            const float2 arg = mul2(nbeta, mul2(add2(sh, sh), acc.s));
+            float2 out;
+            out.x = metropolis_select(own.x, thp.x, u2.x, __expf(arg.x));
+            out.y = metropolis_select(own.y, thp.y, u2.y, __expf(arg.y));
+            if (UNI || valid) lb[static_cast<unsigned long long>(static_cast<uint32_t>(i) * R2)] = out;
+        } else if constexpr (MODE == kModeOverrelax) {
+            float2 out;
+            out.x = overrelax_finish(own.x, acc.hx.x, acc.hy.x);
+            out.y = overrelax_finish(own.y, acc.hx.y, acc.hy.y);
+            if (UNI || valid) lb[static_cast<unsigned long long>(static_cast<uint32_t>(i) * R2)] = out;
+        } else {
+            if (UNI || valid) {
+                float sx, cx, sy, cy;
+                __sincosf(own.x, &sx, &cx);
+                __sincosf(own.y, &sy, &cy);
+                iacc[1] += quant1(cx); iacc[2] += quant1(sx);
+                iacc[4] += quant1(cy); iacc[5] += quant1(sy);
+            }
+        }
+    };
+    // neighbours beyond the pipelined kDB: direct loads in groups of 4 (rare: P(deg > 8) ~ 15 % at z = 6)
+    auto tail = [&](PairAcc<MODE> &acc, int pos, int deg, int dmax) {
+        for (int k = kDB; k < dmax; k += 4) {
+            float2 t[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (k + u < deg) t[u] = sweep_ld(lb, sidx[pos + k + u]);
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (k + u < deg) acc.add(t[u]);
+            if constexpr (MODE == kModeMeasure) acc.flush(iacc[0], iacc[3]);
+        }
+    };
+
+    bool staged = true;      // the first chunk comes from sweep_prep
+    int2 rc = P.rc;
+    for (int i0 = P.i0; i0 < w1;) {
+        // ---- chunk: the longest prefix of <= 32 sites whose neighbour ids fit the staging slice ----
+        const int nsite = min(32, w1 - i0);
+        if (!staged) {
+            rc = make_int2(0, 0);
+            if (lane < nsite) rc = rec[i0 + lane];
+        }
+        int start0, endl;
+        const int msite = chunk_fit(rc, lane, nsite, start0, endl);
+
+        if (msite == 0) {
+            // a single site with more neighbours than the staging slice: lane group 0 walks its ids in blocks
+            const int ry = __shfl_sync(kFull, rc.y, 0);
+            int deg = ry & 0xffff, pos = 0;
+            if constexpr (MODE == kModeMeasure) { pos = ry >> 16; deg -= pos; }
+            const int32_t *gidx = a.col_idx + start0 + pos;
+            const bool valid = UNI || sub == 0;
+            float2 own = make_float2(0.f, 0.f);
+            if (valid) own = __ldcg(lb + static_cast<unsigned long long>(static_cast<uint32_t>(i0) * R2));
+            float2 thp = make_float2(0.f, 0.f), u2 = thp;
+            PairAcc<MODE> acc;
+            begin(i0, own, acc, thp, u2);
+            for (int k0 = 0; k0 < deg; k0 += kStageCap) {
+                const int nb = min(kStageCap, deg - k0);
+                __syncwarp();
+                for (int p = lane; p < nb; p += 32) sidx[p] = static_cast<uint32_t>(gidx[k0 + p]) * R2;
+                __syncwarp();
+                for (int k = 0; k < nb; k += 4) {
+                    float2 t[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u)
+                        if (k + u < nb && valid) t[u] = sweep_ld(lb, sidx[k + u]);
+#pragma unroll
+                    for (int u = 0; u < 4; ++u)
+                        if (k + u < nb && valid) acc.add(t[u]);
+                    if constexpr (MODE == kModeMeasure) acc.flush(iacc[0], iacc[3]);
+                }
+            }
+            finish(i0, valid, own, acc, thp, u2);
+            __syncwarp();
+            i0 += 1;
+            staged = false;
+            continue;
+        }
+
+        if (!staged) {
+            chunk_stage(a.col_idx + start0, sidx, lane, __shfl_sync(kFull, endl, msite - 1), R2);
+            __syncwarp();
+        }
+        staged = false;
+
+        rc.x -= start0;      // list starts relative to the staged run from here on (one register fewer in the row loop)
+        auto site_of = [&](int t) {
+            const int m = t * SPW + sub;
+            const int ry = __shfl_sync(kFull, rc.y, m & 31), rx = __shfl_sync(kFull, rc.x, m & 31);
+            RowSite st;
+            st.valid = UNI || m < msite;
+            st.i = i0 + m;
+            st.deg = st.valid ? (ry & 0xffff) : 0;
+            st.pos = rx;
+            if constexpr (MODE == kModeMeasure) {     // bonds counted once: neighbours j > i are the tail of the list
+                const int nlow = st.valid ? (ry >> 16) : 0;
+                st.pos += nlow;
+                st.deg -= nlow;
+            }
+            return st;
+        };
+        auto row_max = [&](int deg) { return UNI ? deg : static_cast<int>(__reduce_max_sync(kFull, static_cast<unsigned>(deg))); };
+        // async copies of the row (own angle -> ring row kDB, first kDB neighbours -> rows 0..) into ring slot `slot`
+        auto issue = [&](const RowSite st, int dmax, int slot) {
+            const uint32_t row0 = x.ring_s + static_cast<uint32_t>(slot) * kSlotBytes;
+            if (st.valid) cp_async8(row0 + kDB * 256u, lb + static_cast<unsigned long long>(static_cast<uint32_t>(st.i) * R2));
+            sweep_issue<UNI>(row0, lb, sidx, st.pos, st.deg, dmax);
+            cp_async_commit();
+        };
+
+        // software pipeline over the chunk: the copies of row t+1 fly while row t is computed.  The row's site is
+        // re-derived from rc (two shuffles) rather than carried across the iteration: registers matter more here.
+        {
+            const RowSite first = site_of(0);
+            issue(first, row_max(first.deg), 0);
+        }
+        for (int t = 0; t * SPW < msite; ++t) {
+            if ((t + 1) * SPW < msite) {
+                const RowSite nxt = site_of(t + 1);
+                issue(nxt, row_max(nxt.deg), (t + 1) & 1);
+                cp_async_wait<1>();
+            } else {
+                cp_async_wait<0>();
+            }
+            const RowSite cur = site_of(t);
+            const int cmax = row_max(cur.deg);
+            const float2 *row0 = x.ring_l + (t & 1) * kSlotElems;
+            float2 own = make_float2(0.f, 0.f);
+            if (cur.valid) own = row0[kDB * 32];
+            float2 thp = make_float2(0.f, 0.f), u2 = thp;
+            PairAcc<MODE> acc;
+            begin(cur.i, own, acc, thp, u2);
+            sweep_consume<UNI>(acc, row0, cur.deg, cmax);
+            if constexpr (MODE == kModeMeasure) acc.flush(iacc[0], iacc[3]);
+            if (cmax > kDB) tail(acc, cur.pos, cur.deg, cmax);
+            finish(cur.i, cur.valid, own, acc, thp, u2);
+        }
+        __syncwarp();
+        i0 += msite;
+    }
+}
+
+// CTA (x = 0, z = 0) of a sample, after the barrier that follows a measure phase: fixed-point sums -> E, M per slot,
+// optional accumulation under the slot's temperature (Eq. 13-16); leaves fx zeroed for the next measure phase
+__device__ __forceinline__ void sweep_finalize(const TileArgs &a, int s, bool accumulate) {
+    for (int r = threadIdx.x; r < a.R; r += blockDim.x) {
+        long long *f = a.fx + (static_cast<size_t>(s) * a.R + r) * 3;
+        const double e = -static_cast<double>(__ldcg(f)) * kInvScaleE;
+        const double mx = static_cast<double>(__ldcg(f + 1)) * kInvScaleM;
+        const double my = static_cast<double>(__ldcg(f + 2)) * kInvScaleM;
+        f[0] = 0; f[1] = 0; f[2] = 0;
+        const size_t sr = static_cast<size_t>(s) * a.R + r;
+        a.E_slot[sr] = e;
+        a.M_slot[2 * sr] = mx;
+        a.M_slot[2 * sr + 1] = my;
+        if (accumulate) {
+            double *o = a.acc + (static_cast<size_t>(s) * a.R + __ldcg(a.temp_of_slot + sr)) * 8;
+            const double ux = mx / a.N, uy = my / a.N, m2 = ux * ux + uy * uy;
+            o[0] += 1.0; o[1] += e; o[2] += e * e; o[3] += sqrt(m2); o[4] += m2; o[5] += m2 * m2;
+            o[6] += ux; o[7] += uy;
+        }
+    }
+}
+
+// one swap round of sample s by one CTA (R9): pairs (t, t+1), t = round (mod 2)
+__device__ __forceinline__ void sweep_swap(const SweepArgs &a, int s, uint32_t round) {
+    const int R = a.t.R;
+    const int parity = static_cast<int>(round & 1u);
+    int32_t *sot = a.slot_of_temp + static_cast<size_t>(s) * R;
+    int32_t *tos = a.temp_of_slot + static_cast<size_t>(s) * R;
+    __syncthreads();     // E_slot of sweep_finalize
+    for (int t = parity + 2 * static_cast<int>(threadIdx.x); t + 1 < R; t += 2 * blockDim.x) {
+        const int sa = sot[t], sb = sot[t + 1];
+        bool acc;
+        if (a.decisions) {
+            acc = a.decisions[static_cast<size_t>(s) * R + t] != 0;
+        } else {
+            uint32_t x[4];
+            philox4x32_10(static_cast<uint32_t>(t), round, (a.t.sample_base + static_cast<uint32_t>(s)) << 16, kDomSwap,
+                          a.t.keys, x);
+            const double u = static_cast<double>(u01(x[0]));
+            const double arg = (a.betaT[t] - a.betaT[t + 1]) *
+                               (a.t.E_slot[static_cast<size_t>(s) * R + sa] - a.t.E_slot[static_cast<size_t>(s) * R + sb]);
+            acc = u < exp(arg);
+        }
+        a.attempts[static_cast<size_t>(s) * R + t] += 1;
+        if (acc) {
+            a.accepts[static_cast<size_t>(s) * R + t] += 1;
+            sot[t] = sb; sot[t + 1] = sa;
+            tos[sa] = t + 1; tos[sb] = t;
+        }
+    }
+    __syncthreads();
+    for (int r = threadIdx.x; r < R; r += blockDim.x) {
+        const int t = tos[r];
+        a.beta_slot[static_cast<size_t>(s) * R + r] = a.beta_f[t];
+        a.w_slot[static_cast<size_t>(s) * R + r] = a.w_f[t];
+    }
+}
+
+// ---- one phase per launch (the path for large samples): same share / chunk / row code as k_sweep, but every colour
+// class is its own kernel, so each mode gets its own register allocation (64 registers, no spills) and the hardware
+// does the grid-wide ordering.  The launches are captured in a CUDA graph with PROGRAMMATIC DEPENDENT LAUNCH edges:
+// a kernel lets its successor start early (griddepcontrol.launch_dependents); the successor's CTAs become resident
+// as soon as CTAs of this kernel retire, stage their graph data (sweep_prep: never theta), and only then wait for
+// this kernel to complete and flush (griddepcontrol.wait).  Ramp-up thus overlaps the predecessor's tail.
+// MODE 0 / 1: Metropolis / over-relaxation on colour a.t.colour; MODE 2: measure (a.t.accumulate), the last CTA of
+// the sample converts the fixed-point sums.  grid as k_sweep (need not be co-resident).
+template <int G, int CB, int MODE>
+__global__ void __launch_bounds__(kBlock, kSweepMinBlocks) k_phase(const SweepArgs a) {
+    __shared__ SweepWarp s_w[kWarps];
+    __shared__ int s_last;
+    constexpr int SPW = 32 / G;
+
+    SweepCtx x;
+    x.s = a.t.s0 + blockIdx.y;
+    x.lane = threadIdx.x & 31;
+    x.warp = threadIdx.x >> 5;
+    x.sub = x.lane / G;
+    x.q = blockIdx.z * G + x.lane % G;
+    const uint32_t R2 = CB ? static_cast<uint32_t>(G) : static_cast<uint32_t>(a.t.R >> 1);
+    x.lb = reinterpret_cast<float2 *>(a.t.theta) + static_cast<size_t>(x.s) * a.t.N * R2 + x.q;
+    asm volatile("" : "+l"(x.lb));
+    x.rec = a.t.rec + static_cast<size_t>(x.s) * a.t.N;
+    x.sidx = s_w[x.warp].idx;
+    x.ring_l = &s_w[x.warp].ring[0][0][x.lane];
+    x.ring_s = static_cast<uint32_t>(__cvta_generic_to_shared(x.ring_l));
+
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    const PhasePrep P = sweep_prep<G, CB>(a, x, MODE, a.t.colour);
+    __syncwarp();
+    asm volatile("griddepcontrol.wait;" ::: "memory");      // the predecessor's theta / beta_slot / fx are final
+
+    long long iacc[6] = {0, 0, 0, 0, 0, 0};
+    const uint32_t sweep = a.t.use_counter ? a.t.counters[0] + static_cast<uint32_t>(a.t.sweep_offset) : a.t.sweep_fixed;
+    sweep_phase<G, CB, MODE>(a.t, x, P, sweep, iacc);
+
+    if constexpr (MODE == kModeMeasure) {
+        __syncthreads();
+        long long *s_red = reinterpret_cast<long long *>(&s_w[0]);
+#pragma unroll
+        for (int c = 0; c < 6; ++c) s_red[(x.warp * 32 + x.lane) * 6 + c] = iacc[c];
+        __syncthreads();
+        if (threadIdx.x < G * 6) {
+            const int ll = threadIdx.x / 6, c = threadIdx.x % 6;
+            long long v = 0;
+            for (int wi = 0; wi < kWarps; ++wi)
+                for (int sb = 0; sb < SPW; ++sb) v += s_red[(wi * 32 + sb * G + ll) * 6 + c];
+            const int slot = 2 * (blockIdx.z * G + ll) + c / 3;
+            atomicAdd(reinterpret_cast<unsigned long long *>(a.t.fx) + (static_cast<size_t>(x.s) * a.t.R + slot) * 3 + c % 3,
+                      static_cast<unsigned long long>(v));
+        }
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const unsigned int total = gridDim.x * gridDim.z;
+            s_last = (atomicAdd(a.t.ticket + x.s, 1u) == total - 1u) ? 1 : 0;
+        }
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            sweep_finalize(a.t, x.s, a.t.accumulate != 0);
+            if (threadIdx.x == 0) a.t.ticket[x.s] = 0u;
+        }
+    }
+}
+
+// ---- the kernel: grid (x = CTAs per sample and column block, y = samples of the group, z = blocks of 64 slots),
+// launched cooperatively (all CTAs resident) ---------------------------------------------------------------------
+template <int G, int CB>
+__global__ void __launch_bounds__(kBlock, kSweepMinBlocks) k_sweep(const SweepArgs a) {
+    __shared__ SweepWarp s_w[kWarps];
+    constexpr int SPW = 32 / G;
+
+    SweepCtx x;
+    x.s = a.t.s0 + blockIdx.y;
+    x.lane = threadIdx.x & 31;
+    x.warp = threadIdx.x >> 5;
+    x.sub = x.lane / G;
+    x.q = blockIdx.z * G + x.lane % G;          // slot pair handled by this lane
+    const uint32_t R2 = CB ? static_cast<uint32_t>(G) : static_cast<uint32_t>(a.t.R >> 1);
+    x.lb = reinterpret_cast<float2 *>(a.t.theta) + static_cast<size_t>(x.s) * a.t.N * R2 + x.q;
+    asm volatile("" : "+l"(x.lb));   // keep the lane's base as one materialised pointer: gather address = one IMAD.WIDE.U32
+    x.rec = a.t.rec + static_cast<size_t>(x.s) * a.t.N;
+    x.sidx = s_w[x.warp].idx;
+    x.ring_l = &s_w[x.warp].ring[0][0][x.lane];
+    x.ring_s = static_cast<uint32_t>(__cvta_generic_to_shared(x.ring_l));
+
+    unsigned int *bar = a.bar + x.s;
+    unsigned int target = 0;
+    const unsigned int n_cta = gridDim.x * gridDim.z;
+    const bool cta0 = blockIdx.x == 0 && blockIdx.z == 0;
+
+    PhaseIter it;
+    it.c = a.c_lo;
+    PhaseDesc cur, nxt;
+    bool more = next_phase(a, it, cur);
+    PhasePrep P;
+    P.i0 = P.w1 = 0; P.rc = make_int2(0, 0);
+    if (more && cur.mode != kPhaseSwap) P = sweep_prep<G, CB>(a, x, cur.mode, cur.colour);
+    __syncthreads();
+
+    while (more) {
+        long long iacc[6] = {0, 0, 0, 0, 0, 0};
+        switch (cur.mode) {
+            case kModeMetropolis: sweep_phase<G, CB, kModeMetropolis>(a.t, x, P, cur.sweep, iacc); break;
+            case kModeOverrelax: sweep_phase<G, CB, kModeOverrelax>(a.t, x, P, 0u, iacc); break;
+            case kModeMeasure: {
+                // every CTA reduces its sites: one fixed-point atomic per (slot, quantity) and CTA
+                sweep_phase<G, CB, kModeMeasure>(a.t, x, P, 0u, iacc);
+                __syncthreads();
+                long long *s_red = reinterpret_cast<long long *>(&s_w[0]);      // the ring is free now
+#pragma unroll
+                for (int c = 0; c < 6; ++c) s_red[(x.warp * 32 + x.lane) * 6 + c] = iacc[c];
+                __syncthreads();
+                if (threadIdx.x < G * 6) {
+                    const int ll = threadIdx.x / 6, c = threadIdx.x % 6;
+                    long long v = 0;
+                    for (int wi = 0; wi < kWarps; ++wi)
+                        for (int sb = 0; sb < SPW; ++sb) v += s_red[(wi * 32 + sb * G + ll) * 6 + c];
+                    const int slot = 2 * (blockIdx.z * G + ll) + c / 3;
+                    atomicAdd(reinterpret_cast<unsigned long long *>(a.t.fx) + (static_cast<size_t>(x.s) * a.t.R + slot) * 3 + c % 3,
+                              static_cast<unsigned long long>(v));
+                }
+                break;
+            }
+            default:    // swap round: one CTA per sample
+                if (cta0) sweep_swap(a, x.s, cur.sweep);
+                break;
+        }
+        more = next_phase(a, it, nxt);
+        // barrier, with the next phase's graph data staged between arrival and wait
+        sample_barrier_arrive(bar, target, n_cta);
+        P.i0 = P.w1 = 0;
+        if (more && nxt.mode != kPhaseSwap) P = sweep_prep<G, CB>(a, x, nxt.mode, nxt.colour);
+        sample_barrier_wait(bar, target, n_cta);
+        // after a measure phase CTA 0 of the sample converts and (optionally) accumulates; the others go on:
+        // nothing they touch before the next barrier is written by sweep_finalize
+        if (cur.mode == kModeMeasure && cta0) sweep_finalize(a.t, x.s, cur.flag != 0);
+        cur = nxt;
+    }
+}
+
+}  // namespace xy

@@ -67,14 +67,16 @@ def test_lockstep_one_sweep_metropolis_and_overrelax(L, rho, R, S):
     ens.close()
 
 
-def test_metropolis_sweep_trajectory_config0():
-    """one full Metropolis sweep (all colours) from an identical state: angles are bit-identical except inside
-    the influence cone of a near-threshold site (none expected at this size)."""
+@pytest.mark.parametrize("R", [8, 2, 16, 32, 64, 128, 6])
+def test_metropolis_sweep_trajectory_config0(R):
+    """full Metropolis sweeps (all colours in one persistent launch) from an identical state: angles are
+    BIT-identical to the oracle's until the first near-threshold decision (R5: the accepted angle is the same
+    fp32 number on both sides).  config 0's graph; R = 8 is config 0 itself, the other R cover every kernel flavour."""
     w = workloads.CONFIGS[0]
     g = levy.build(w.L, w.rho, w.z, w.seed, S=1)
-    T = w.temperatures()
+    T = w.temperatures() if R == w.R else O.geometric_temperatures(R, w.T_min, w.T_max)
     ens = U.ensemble_from_levy(g, T, SEED)
-    ref = O.init_theta(w.N, w.R, SEED, 0)
+    ref = O.init_theta(w.N, R, SEED, 0)
     cp = g.class_ptr(0)
     bs, ws = O.temperature_params(T)
     min_margin = np.inf
