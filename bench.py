@@ -210,7 +210,7 @@ def main():
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
     value = upd_per_step * world * args.steps / (ms * 1e6)
 
-    # ---- dominant kernel (k_update_class: the Metropolis / OR colour-class kernel): same launches, same
+    # ---- dominant kernel (k_phase: the Metropolis / OR colour-class kernel): same launches, same
     #      schedule, without measure/swap, timed with CUDA events on the same stream ----
     ens.run_sweeps(2, sps, orps)
     lk0 = ens.launch_count()
@@ -227,7 +227,7 @@ def main():
         except Exception:
             traffic = None
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic, "kernel": "k_update_class (Metropolis and OR colour-class launches)",
+                "traffic": traffic, "kernel": "k_phase<G,CB,0|1> (Metropolis and over-relaxation colour-class launches)",
                 "peak_source": peak_src, "bytes_per_update": w.bytes_per_update(),
                 "updates_per_launch_avg": upd_per_step * args.steps / max(n_class_launches, 1),
                 "avg_launch_us": ms_k * 1e3 / max(n_class_launches, 1), "launches_timed": n_class_launches,

@@ -106,14 +106,12 @@ int xy_run_sweeps(xy_pt *pt, int n_blocks, int sweeps_per_block, int or_per_swee
  * are bit-identical for every value.  0 = automatic (default), S = all samples per launch. */
 int xy_set_schedule(xy_pt *pt, int samples_per_group);
 
-/* Execution path of the float2 kernel flavours (R = 2 * 2^k <= 64, R % 64 == 0); results are bit-identical for every
- * choice.  path 0 = automatic (by sample size), 1 = persistent cooperative kernel (one launch per sample group and
- * call; colour classes are phases separated by a per-sample barrier), 2 = one launch per colour class, captured in a
- * CUDA graph.  balance != 0: cost-balanced shares of a colour class per warp (default), 0: equal shares.
- * pdl != 0: programmatic-dependent-launch edges between the per-class launches (default).  l2_persist != 0: theta
- * of the running sample group is marked persisting in L2 through an access-policy window (default).
- * Synchronises the stream. */
-int xy_set_path(xy_pt *pt, int path, int balance, int pdl, int l2_persist);
+/* Tuning switches of the float2 kernel flavours (R = 2 * 2^k <= 64, R % 64 == 0); results are bit-identical for
+ * every setting (tests/test_gpu_parity.py).  balance != 0: cost-balanced shares of a colour class per warp (default),
+ * 0: equal shares.  pdl != 0: programmatic-dependent-launch edges between the colour-class launches (default).
+ * l2_persist != 0: theta of the running sample group is marked persisting in L2 through an access-policy window
+ * (default).  Synchronises the stream and drops the captured graphs. */
+int xy_set_tuning(xy_pt *pt, int balance, int pdl, int l2_persist);
 
 /* ---- single-colour steps (lockstep parity tests) ----
  * Metropolis on colour class `colour` of every sample with Philox sweep index `sweep` (the handle's

@@ -43,19 +43,7 @@ int dev_alloc(T **p, size_t n) {
 
 int ceil_div(long long a, long long b) { return static_cast<int>((a + b - 1) / b); }
 
-// the k_sweep<G, CB> instantiation for G lanes per site (CB = 0: R a multiple of 64 larger than 64)
-const void *sweep_function(int G, bool single_block) {
-    switch (G) {
-        case 32: return single_block ? reinterpret_cast<const void *>(xy::k_sweep<32, 1>)
-                                     : reinterpret_cast<const void *>(xy::k_sweep<32, 0>);
-        case 16: return reinterpret_cast<const void *>(xy::k_sweep<16, 1>);
-        case 8: return reinterpret_cast<const void *>(xy::k_sweep<8, 1>);
-        case 4: return reinterpret_cast<const void *>(xy::k_sweep<4, 1>);
-        case 2: return reinterpret_cast<const void *>(xy::k_sweep<2, 1>);
-        default: return reinterpret_cast<const void *>(xy::k_sweep<1, 1>);
-    }
-}
-
+// the k_phase<G, CB, MODE> instantiation for G lanes per site (CB = 0: R a multiple of 64 larger than 64)
 template <int MODE>
 const void *phase_function_mode(int G, bool single_block) {
     switch (G) {
@@ -117,18 +105,15 @@ struct xy_pt {
     long long *attempts = nullptr, *accepts = nullptr;
     uint8_t *decisions = nullptr;
     xy::PhiloxKeys keys;
-    int fast_G = 0;  // lanes per site of the persistent float2 kernel (k_sweep), 0 = legacy generic kernels
+    int fast_G = 0;  // lanes per site of the float2 kernel (k_phase), 0 = any-R kernels
     int col_blocks = 1;
     int l2_persist = 1;              // mark the running sample group's theta as persisting in L2 (access policy window)
     size_t l2_persist_bytes = 0, l2_window_max = 0;   // device limits (0 = not supported)
     int balance = 1;                 // cost-balanced share tables (1) or equal shares (0)
     int pdl = 1;                     // programmatic dependent launch edges between the k_phase launches
-    int path = 0;                    // 0 = automatic, 1 = persistent kernel (k_sweep), 2 = one launch per phase (k_phase, CUDA graph)
     const void *phase_fn[3] = {nullptr, nullptr, nullptr};   // k_phase<G, CB, MODE>
     std::map<int, int32_t *> parts;  // warps per sample -> device [S][q_stride][nw + 1] cost-balanced share tables
-    const void *sweep_fn = nullptr;  // the k_sweep<G, CB> instantiation of this ensemble
-    int sweep_capacity = 0;          // co-resident CTAs of sweep_fn on this device (cooperative launch limit)
-    unsigned int *bar = nullptr;     // [S] per-sample barrier counters of k_sweep
+    int sweep_capacity = 0;          // co-resident CTAs of k_phase on this device: the grid is one such wave
     int measure_chunk = 256;  // sites per CTA of the generic measure kernel
     int samples_per_group = 0;  // 0 = automatic
     // host mirrors
@@ -218,13 +203,7 @@ int sweep_grid_x(const xy_pt *pt, int ns, int nmax) {
 xy::SweepArgs sweep_args(xy_pt *pt, int s0) {
     xy::SweepArgs a;
     a.t = tile_args(pt, 0, s0);
-    a.n_rep = 1; a.sps = 0; a.do_met = 0; a.orps = 0; a.me = 0; a.end_measure = 0; a.do_swap = 0; a.c_lo = 0; a.c_hi = 0;
-    a.sweep0 = 0; a.round0 = 0;
-    a.bar = pt->bar; a.part = nullptr;
-    a.betaT = pt->betaT; a.beta_f = pt->beta_f; a.w_f = pt->w_f;
-    a.slot_of_temp = pt->slot_of_temp; a.temp_of_slot = pt->temp_of_slot;
-    a.beta_slot = pt->beta_slot; a.w_slot = pt->w_slot;
-    a.decisions = nullptr; a.attempts = pt->attempts; a.accepts = pt->accepts;
+    a.part = nullptr;
     return a;
 }
 
@@ -344,80 +323,8 @@ int auto_group(const xy_pt *pt) {
     if (pt->samples_per_group > 0) group = std::min(pt->samples_per_group, g->S);
     else if (per_sample * g->S <= l2_budget) group = g->S;
     else group = std::max(1, std::min(g->S, static_cast<int>(l2_budget / per_sample)));
-    // k_sweep is launched cooperatively: at least one CTA per (sample, column block) must be resident
-    if (pt->fast_G) group = std::max(1, std::min(group, pt->sweep_capacity / pt->col_blocks));
+    if (pt->fast_G) group = std::max(1, std::min(group, pt->sweep_capacity / pt->col_blocks));   // >= 1 CTA per (sample, block)
     return group;
-}
-
-// ---- the persistent path: what one k_sweep launch does for every sample of a group (xy_sweep.cuh, SweepArgs) ----
-struct SweepCtl {
-    int n_rep = 1, sps = 0, do_met = 0, orps = 0, me = 0, end_measure = 0, do_swap = 0, c_lo = 0, c_hi = -1;
-    uint32_t sweep0 = 0, round0 = 0;
-    const uint8_t *decisions = nullptr;
-};
-
-int launch_sweep_group(xy_pt *pt, int s0, int s1, const SweepCtl &c) {
-    const xy_graph *g = pt->g;
-    xy::SweepArgs a = sweep_args(pt, s0);
-    a.n_rep = c.n_rep; a.sps = c.sps; a.do_met = c.do_met; a.orps = c.orps; a.me = c.me;
-    a.end_measure = c.end_measure; a.do_swap = c.do_swap;
-    a.c_lo = c.c_lo; a.c_hi = c.c_hi < 0 ? g->q_max : c.c_hi;
-    a.sweep0 = c.sweep0; a.round0 = c.round0;
-    a.decisions = c.decisions;
-    // grid: per sample enough warps to give every warp at least one row of the largest colour class (the measure
-    // phase walks all N sites); all CTAs co-resident (cooperative launch)
-    const int ns = s1 - s0;
-    int nmax = 1;
-    const bool updates = c.sps > 0 && (c.do_met || c.orps > 0);
-    if (updates) for (int col = a.c_lo; col < a.c_hi; ++col) nmax = std::max(nmax, max_class_size(g, col, s0, s1));
-    else nmax = g->N;
-    // a barrier between two CTAs costs microseconds, a bar.sync inside one CTA nanoseconds: few, fat CTAs per sample
-    const int gx = sweep_grid_x(pt, ns, ceil_div(nmax, 4));
-    if (pt->balance) {
-        const int rc = get_partition(pt, gx * xy::kWarps, &a.part);
-        if (rc != XY_OK) return rc;
-    }
-    XY_CUDA(cudaMemsetAsync(pt->bar + s0, 0, static_cast<size_t>(ns) * sizeof(unsigned int), pt->stream));
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(gx, ns, pt->col_blocks);
-    cfg.blockDim = dim3(xy::kBlock);
-    cfg.dynamicSmemBytes = 0;
-    cfg.stream = pt->stream;
-    cudaLaunchAttribute attr[2];
-    int na = l2_window_attr(pt, s0, s1, &attr[0]);
-    attr[na].id = cudaLaunchAttributeCooperative;
-    attr[na].val.cooperative = 1;
-    ++na;
-    cfg.attrs = attr; cfg.numAttrs = na;
-    void *params[] = {&a};
-    XY_CUDA(cudaLaunchKernelExC(&cfg, pt->sweep_fn, params));
-    pt->launches += 1;
-    return XY_OK;
-}
-
-// which path runs the float2 flavours: the persistent kernel when a sample is small (launch- and latency-bound
-// phases: a per-sample barrier is cheaper than a kernel boundary), one launch per phase otherwise
-bool use_persistent(const xy_pt *pt) {
-    if (!pt->fast_G) return false;
-    if (pt->path == 1) return true;
-    if (pt->path == 2) return false;
-    return false;   // measured: the per-phase launches win at every BASELINE config
-}
-
-// run `c` for every sample group (all repetitions of a group before the next group starts: sample-major time
-// blocking, legal because samples never interact), then advance the device counters
-int run_sweep(xy_pt *pt, const SweepCtl &c, uint32_t d_sweep, uint32_t d_round) {
-    const int S = pt->g->S, group = auto_group(pt);
-    for (int s0 = 0; s0 < S; s0 += group) {
-        const int rc = launch_sweep_group(pt, s0, std::min(S, s0 + group), c);
-        if (rc != XY_OK) return rc;
-    }
-    if (d_sweep || d_round) {
-        xy::k_tick<<<1, 1, 0, pt->stream>>>(pt->counters, d_sweep, d_round);
-        XY_CUDA(cudaGetLastError());
-        pt->launches += 1;
-    }
-    return XY_OK;
 }
 
 // enqueue one PT cycle on the stream; `phase` = sweep counter mod measure_every at entry
@@ -688,7 +595,6 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
     pt->keys = xy::philox_key_schedule(pt->key0, pt->key1);
     pt->measure_chunk = std::max(256, ((N + 127) / 128 + 7) / 8 * 8);   // legacy measure partition: a function of N only
     if (pt->fast_G) {
-        pt->sweep_fn = sweep_function(pt->fast_G, pt->col_blocks == 1);
         for (int m = 0; m < 3; ++m) {
             pt->phase_fn[m] = phase_function(pt->fast_G, pt->col_blocks == 1, m);
             cudaFuncSetAttribute(pt->phase_fn[m], cudaFuncAttributePreferredSharedMemoryCarveout,
@@ -697,14 +603,12 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
         int per_sm = 0, n_sm = 0, dev = 0;
         cudaError_t eo = cudaGetDevice(&dev);
         if (eo == cudaSuccess) eo = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        if (eo == cudaSuccess)   // k_sweep keeps kSweepMinBlocks CTAs x 45 KB of shared memory resident per SM
-            eo = cudaFuncSetAttribute(pt->sweep_fn, cudaFuncAttributePreferredSharedMemoryCarveout,
-                                      static_cast<int>(cudaSharedmemCarveoutMaxShared));
-        if (eo == cudaSuccess) eo = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pt->sweep_fn, xy::kBlock, 0);
+        // k_phase keeps kSweepMinBlocks CTAs x 45 KB of shared memory resident per SM (carve-out set above)
+        if (eo == cudaSuccess) eo = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pt->phase_fn[0], xy::kBlock, 0);
         if (eo != cudaSuccess || per_sm < 1 || n_sm < 1) {
             if (pt->owns_stream) cudaStreamDestroy(pt->stream);
             delete pt;
-            return fail(XY_ECUDA, std::string("k_sweep occupancy query: ") + cudaGetErrorString(eo));
+            return fail(XY_ECUDA, std::string("k_phase occupancy query: ") + cudaGetErrorString(eo));
         }
         pt->sweep_capacity = per_sm * n_sm;
         int max_persist = 0, max_window = 0;
@@ -729,7 +633,7 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
     A(dev_alloc(&pt->E_slot, SR)); A(dev_alloc(&pt->M_slot, SR * 2));
     A(dev_alloc(&pt->fx, SR * 3)); A(dev_alloc(&pt->ticket, S)); A(dev_alloc(&pt->acc, SR * XY_NACC));
     A(dev_alloc(&pt->attempts, SR)); A(dev_alloc(&pt->accepts, SR)); A(dev_alloc(&pt->decisions, SR));
-    A(dev_alloc(&pt->bar, S));
+
     if (rc != XY_OK) { xy_pt_destroy(pt); return rc; }
     std::vector<float> hb(R), hw(R);
     std::vector<double> hbT(R);
@@ -776,7 +680,7 @@ int xy_pt_destroy(xy_pt *pt) {
     cudaFree(pt->beta_slot); cudaFree(pt->w_slot); cudaFree(pt->beta_f); cudaFree(pt->w_f); cudaFree(pt->betaT);
     cudaFree(pt->temp_of_slot); cudaFree(pt->slot_of_temp); cudaFree(pt->counters);
     cudaFree(pt->E_slot); cudaFree(pt->M_slot); cudaFree(pt->fx); cudaFree(pt->ticket); cudaFree(pt->acc);
-    cudaFree(pt->attempts); cudaFree(pt->accepts); cudaFree(pt->decisions); cudaFree(pt->bar);
+    cudaFree(pt->attempts); cudaFree(pt->accepts); cudaFree(pt->decisions);
     for (auto &kv : pt->parts) cudaFree(kv.second);
     if (pt->owns_stream) cudaStreamDestroy(pt->stream);
     delete pt;
@@ -785,16 +689,6 @@ int xy_pt_destroy(xy_pt *pt) {
 
 int xy_sweep(xy_pt *pt, int n_sweeps) {
     if (!check_pt(pt) || n_sweeps < 0) return fail(XY_EINVAL, "bad handle or n_sweeps < 0");
-    if (use_persistent(pt)) {
-        if (n_sweeps == 0) return XY_OK;
-        SweepCtl c;
-        c.n_rep = n_sweeps; c.sps = 1; c.do_met = 1; c.sweep0 = pt->sweep;
-        const int rc = run_sweep(pt, c, static_cast<uint32_t>(n_sweeps), 0u);
-        if (rc != XY_OK) return rc;
-        pt->sweep += static_cast<uint32_t>(n_sweeps);
-        pt->e_fresh = false;
-        return XY_OK;
-    }
     for (int n = 0; n < n_sweeps; ++n) {
         const int rc = sweep_group(pt, 0, 0, pt->g->S, true, 1, 0u);
         if (rc != XY_OK) return rc;
@@ -809,13 +703,6 @@ int xy_sweep(xy_pt *pt, int n_sweeps) {
 
 int xy_overrelax(xy_pt *pt, int n_sweeps) {
     if (!check_pt(pt) || n_sweeps < 0) return fail(XY_EINVAL, "bad handle or n_sweeps < 0");
-    if (use_persistent(pt)) {
-        if (n_sweeps == 0) return XY_OK;
-        SweepCtl c;
-        c.n_rep = n_sweeps; c.sps = 1; c.orps = 1;
-        pt->e_fresh = false;
-        return run_sweep(pt, c, 0u, 0u);
-    }
     for (int n = 0; n < n_sweeps; ++n) {
         const int rc = sweep_group(pt, 1, 0, pt->g->S, false, 0, 0u);
         if (rc != XY_OK) return rc;
@@ -827,11 +714,6 @@ int xy_overrelax(xy_pt *pt, int n_sweeps) {
 int xy_metropolis_colour(xy_pt *pt, int colour, uint32_t sweep) {
     if (!check_pt(pt) || colour < 0 || colour >= pt->g->q_max) return fail(XY_EINVAL, "bad handle or colour");
     pt->e_fresh = false;
-    if (use_persistent(pt)) {   // same kernel, same sample groups as xy_run / xy_run_sweeps
-        SweepCtl c;
-        c.sps = 1; c.do_met = 1; c.c_lo = colour; c.c_hi = colour + 1; c.sweep0 = sweep - 1u;
-        return run_sweep(pt, c, 0u, 0u);
-    }
     const int group = auto_group(pt);
     for (int s0 = 0; s0 < pt->g->S; s0 += group) {
         const int rc = launch_class<0>(pt, colour, s0, std::min(pt->g->S, s0 + group), false, 0, sweep);
@@ -843,11 +725,6 @@ int xy_metropolis_colour(xy_pt *pt, int colour, uint32_t sweep) {
 int xy_overrelax_colour(xy_pt *pt, int colour) {
     if (!check_pt(pt) || colour < 0 || colour >= pt->g->q_max) return fail(XY_EINVAL, "bad handle or colour");
     pt->e_fresh = false;
-    if (use_persistent(pt)) {
-        SweepCtl c;
-        c.sps = 1; c.orps = 1; c.c_lo = colour; c.c_hi = colour + 1;
-        return run_sweep(pt, c, 0u, 0u);
-    }
     const int group = auto_group(pt);
     for (int s0 = 0; s0 < pt->g->S; s0 += group) {
         const int rc = launch_class<1>(pt, colour, s0, std::min(pt->g->S, s0 + group), false, 0, 0u);
@@ -858,13 +735,6 @@ int xy_overrelax_colour(xy_pt *pt, int colour) {
 
 int xy_pt_swap(xy_pt *pt) {
     if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
-    if (use_persistent(pt)) {
-        SweepCtl c;
-        c.end_measure = pt->e_fresh ? 0 : 1; c.do_swap = 1; c.round0 = pt->round;
-        const int rc = run_sweep(pt, c, 0u, 1u);
-        if (rc == XY_OK) { pt->round += 1; pt->e_fresh = true; }
-        return rc;
-    }
     if (!pt->e_fresh) {
         const int rc = launch_measure(pt, 0, pt->g->S, false);
         if (rc != XY_OK) return rc;
@@ -880,13 +750,6 @@ int xy_swap_with_decisions(xy_pt *pt, const uint8_t *accept_host) {
     const size_t SR = static_cast<size_t>(pt->g->S) * pt->R;
     XY_CUDA(cudaMemcpyAsync(pt->decisions, accept_host, SR, cudaMemcpyHostToDevice, pt->stream));
     XY_CUDA(cudaStreamSynchronize(pt->stream));  // accept_host is borrowed for the call only
-    if (use_persistent(pt)) {
-        SweepCtl c;
-        c.do_swap = 1; c.round0 = pt->round; c.decisions = pt->decisions;
-        const int rc = run_sweep(pt, c, 0u, 1u);
-        if (rc == XY_OK) pt->round += 1;
-        return rc;
-    }
     const int rc = launch_swap(pt, pt->decisions, 0u);
     if (rc == XY_OK) pt->round += 1;
     return rc;
@@ -895,14 +758,7 @@ int xy_swap_with_decisions(xy_pt *pt, const uint8_t *accept_host) {
 int xy_measure(xy_pt *pt, double *out_host) {
     if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
     const int S = pt->g->S, R = pt->R;
-    int rc;
-    if (use_persistent(pt)) {
-        SweepCtl c;
-        c.end_measure = 2;
-        rc = run_sweep(pt, c, 0u, 0u);
-    } else {
-        rc = launch_measure(pt, 0, S, true);
-    }
+    const int rc = launch_measure(pt, 0, S, true);
     if (rc != XY_OK) return rc;
     pt->e_fresh = true;
     if (out_host) {
@@ -933,10 +789,10 @@ int xy_set_schedule(xy_pt *pt, int samples_per_group) {
     return XY_OK;
 }
 
-int xy_set_path(xy_pt *pt, int path, int balance, int pdl, int l2_persist) {
-    if (!check_pt(pt) || path < 0 || path > 2) return fail(XY_EINVAL, "bad handle or path not in {0, 1, 2}");
+int xy_set_tuning(xy_pt *pt, int balance, int pdl, int l2_persist) {
+    if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
     XY_CUDA(cudaStreamSynchronize(pt->stream));
-    pt->path = path; pt->balance = balance ? 1 : 0; pt->pdl = pdl ? 1 : 0; pt->l2_persist = l2_persist ? 1 : 0;
+    pt->balance = balance ? 1 : 0; pt->pdl = pdl ? 1 : 0; pt->l2_persist = l2_persist ? 1 : 0;
     drop_graphs(pt);
     return XY_OK;
 }
@@ -944,18 +800,6 @@ int xy_set_path(xy_pt *pt, int path, int balance, int pdl, int l2_persist) {
 int xy_run(xy_pt *pt, int n_cycles, int sps, int orps, int me) {
     if (!check_pt(pt) || n_cycles < 0 || sps < 1 || orps < 0 || me < 0)
         return fail(XY_EINVAL, "need n_cycles >= 0, sweeps_per_swap >= 1, or_per_sweep >= 0, measure_every >= 0");
-    if (use_persistent(pt)) {   // one persistent launch per sample group runs all n_cycles cycles of the group
-        if (n_cycles == 0) return XY_OK;
-        SweepCtl c;
-        c.n_rep = n_cycles; c.sps = sps; c.do_met = 1; c.orps = orps; c.me = me; c.end_measure = 1; c.do_swap = 1;
-        c.sweep0 = pt->sweep; c.round0 = pt->round;
-        const int rc = run_sweep(pt, c, static_cast<uint32_t>(n_cycles) * static_cast<uint32_t>(sps), static_cast<uint32_t>(n_cycles));
-        if (rc != XY_OK) return rc;
-        pt->sweep += static_cast<uint32_t>(n_cycles) * static_cast<uint32_t>(sps);
-        pt->round += static_cast<uint32_t>(n_cycles);
-        pt->e_fresh = false;
-        return XY_OK;
-    }
     const int group = auto_group(pt);
     {
         const int rc = prepare_partitions(pt, group);
@@ -979,16 +823,6 @@ int xy_run(xy_pt *pt, int n_cycles, int sps, int orps, int me) {
 int xy_run_sweeps(xy_pt *pt, int n_blocks, int sps, int orps) {
     if (!check_pt(pt) || n_blocks < 0 || sps < 1 || orps < 0)
         return fail(XY_EINVAL, "need n_blocks >= 0, sweeps_per_block >= 1, or_per_sweep >= 0");
-    if (use_persistent(pt)) {
-        if (n_blocks == 0) return XY_OK;
-        SweepCtl c;
-        c.n_rep = n_blocks; c.sps = sps; c.do_met = 1; c.orps = orps; c.sweep0 = pt->sweep;
-        const int rc = run_sweep(pt, c, static_cast<uint32_t>(n_blocks) * static_cast<uint32_t>(sps), 0u);
-        if (rc != XY_OK) return rc;
-        pt->sweep += static_cast<uint32_t>(n_blocks) * static_cast<uint32_t>(sps);
-        pt->e_fresh = false;
-        return XY_OK;
-    }
     const int group = auto_group(pt);
     {
         const int rc = prepare_partitions(pt, group);
@@ -1060,13 +894,6 @@ int xy_set_labels(xy_pt *pt, const int32_t *temp_of_slot_host) {
 
 int xy_get_energy(xy_pt *pt, double *E_slot_host) {
     if (!check_pt(pt) || !E_slot_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
-    if (!pt->e_fresh && use_persistent(pt)) {
-        SweepCtl c;
-        c.end_measure = 1;
-        const int rc = run_sweep(pt, c, 0u, 0u);
-        if (rc != XY_OK) return rc;
-        pt->e_fresh = true;
-    }
     if (!pt->e_fresh) {
         const int rc = launch_measure(pt, 0, pt->g->S, false);
         if (rc != XY_OK) return rc;
@@ -1127,6 +954,13 @@ int xy_launch_count(xy_pt *pt, int64_t *n) {
     *n = pt->launches;
     return XY_OK;
 }
+
+#ifdef XY_TRACE
+int xy_debug_trace(unsigned long long *out_host /*[8192][4]*/) {
+    XY_CUDA(cudaMemcpyFromSymbol(out_host, xy::g_trace, sizeof(unsigned long long) * 8192 * 4));
+    return XY_OK;
+}
+#endif
 
 int xy_synchronize(xy_pt *pt) {
     if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");

@@ -1,24 +1,22 @@
-// xy_sweep.cuh -- the persistent sweep kernel: every step of the hot path (Metropolis and over-relaxation colour
-// classes, E / M reductions with accumulation, parallel-tempering swap) for one group of samples in ONE launch.
+// xy_sweep.cuh -- the colour-class kernel k_phase<G, CB, MODE>: Metropolis / over-relaxation update of one colour
+// class, or the E / M reduction over all sites, for one group of samples.
 //
-// Why one kernel (profiles/r1c_full.md): with one launch per colour class the ramp-up (four
-// dependent global latencies before the first update) and the tail of the slowest warp were paid 100 times per
-// PT cycle and sample: 21 % of the cycles had no resident warp.  Here a cooperative grid stays resident and the
-// colour classes are PHASES separated by a per-sample barrier (samples never interact, so CTAs of
-// different samples never wait for one another).  The whole of xy_run(n_cycles) for a sample group is one launch.
+// Work layout: theta[S][N][R] fp32, replica fastest.  A lane owns TWO adjacent slots (one float2, one Philox4x32-10
+// call per site: words (x0,x1) feed the even slot, (x2,x3) the odd one), G = R/2 lanes cover a site (G = 32 and
+// column blocks of 64 slots when R % 64 == 0) and a warp works on SPW = 32/G sites at once ("row").  At R = 64 one
+// neighbour gather is one fully used 256-byte request.  A warp owns a contiguous, cost-balanced share of the colour
+// class and walks it in chunks of <= 32 sites: one coalesced load of the chunk's rec[], the chunk's neighbour ids
+// (one contiguous CSR run) staged in the warp's slice of shared memory, pre-scaled by the site stride.  Same-colour
+// sites share no bond, so the gathers of row t+1 never read what row t stores: they are issued BEFORE
+// row t is computed, as cp.async (LDGSTS) copies of the lane's own 8 bytes into a per-warp ring in shared memory --
+// in-flight data costs no registers (64 per thread, 32 warps per SM, no spills), each lane reads back only what it
+// copied itself (cp.async.wait_group, no cross-lane synchronisation), and the Philox / sin / exp work of row t
+// covers the latency of row t+1.  When SPW > 1 the sites of a row have different degrees: the loops run to the row
+// maximum and lanes whose site has fewer neighbours are predicated off (no memory request is made for them).
 //
-// Work layout inside a phase: theta[S][N][R] fp32, replica fastest.  A lane owns TWO adjacent slots (one float2,
-// one Philox4x32-10 call per site: words (x0,x1) feed the even slot, (x2,x3) the odd one), G = R/2 lanes cover a
-// site (G = 32 and column blocks of 64 slots when R % 64 == 0) and a warp works on SPW = 32/G sites at once
-// ("row").  At R = 64 one neighbour gather is one fully used 256-byte request.  A warp owns a contiguous share of
-// the colour class and walks it in chunks of <= 32 sites: one coalesced load of the chunk's rec[], the chunk's
-// neighbour ids (one contiguous CSR run) staged in the warp's slice of shared memory, pre-scaled by the site
-// stride.  Same-colour sites share no bond, so the gathers of row t+1 never read what row t stores:
-// they are issued BEFORE row t is computed, as cp.async (LDGSTS) copies of the lane's own 8 bytes into a per-warp
-// ring in shared memory -- in-flight data costs no registers, each lane reads back only what it copied itself
-// (cp.async.wait_group, no cross-lane synchronisation), and the Philox / sin / exp work of row t covers the
-// latency of row t+1.  When SPW > 1 the sites of a row have different degrees: the loops run to the row maximum
-// and lanes whose site has fewer neighbours are predicated off (no memory request is made for them).
+// The launches of a PT cycle are captured in a CUDA graph with PROGRAMMATIC DEPENDENT LAUNCH edges (see k_phase).
+// A persistent cooperative variant (all phases of a cycle in one launch, per-sample barriers) was built and measured
+// in round 1 and removed: it lost to the per-phase launches at every BASELINE config.
 //
 // PAPER.md:444,:454 (coloured single-spin Metropolis), :460 (over-relaxation, ref 66), :167-181 (E, m),
 // :460-472 (parallel tempering); readings R5-R11 in DESIGN.md.
@@ -78,12 +76,6 @@ __device__ __forceinline__ void cp_async8(uint32_t smem_addr, const void *gptr) 
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-__device__ __forceinline__ unsigned ld_relaxed_gpu(const unsigned *p) {
-    unsigned v;
-    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
 
 // ---- per-lane state of one site (two slots) ----------------------------------------------------------
 template <int MODE> struct PairAcc;
@@ -186,103 +178,12 @@ __device__ __forceinline__ void sweep_consume(ACC &acc, const float2 *row0, int 
     }
 }
 
-// ---- arguments ---------------------------------------------------------------------------------------------
-// One launch runs, for every sample of the group (blockIdx.y):
-//   repeat n_rep times:
-//     for k = 1..sps:  sweep = sweep0 + rep*sps + k
-//        if do_met:  Metropolis on colours c_lo..c_hi-1
-//        orps x [ over-relaxation on colours c_lo..c_hi-1 ]
-//        if me > 0 and sweep % me == 0:  measure + accumulate
-//     end_measure: 1 = E per slot unless just measured (no accumulation), 2 = measure + accumulate
-//     if do_swap:  one swap round (round0 + rep)
+// ---- arguments: the shared TileArgs plus the share table ---------------------------------------------------------
 struct SweepArgs {
     TileArgs t;
-    int n_rep, sps, do_met, orps, me, end_measure, do_swap, c_lo, c_hi;
-    uint32_t sweep0, round0;
-    unsigned int *bar;             // [S] per-sample barrier counters, zero at launch
     const int32_t *part;           // [S][q_stride][nw + 1] cost-balanced first site of every warp's share (colour q_max =
                                    // the measure pass over all sites), nw = gridDim.x * kWarps; nullptr = equal shares
-    // swap round
-    const double *betaT;           // [R] 1/T fp64
-    const float *beta_f, *w_f;     // [R]
-    int32_t *slot_of_temp, *temp_of_slot;   // [S][R]
-    float *beta_slot, *w_slot;     // [S][R]
-    const uint8_t *decisions;      // [S][R] or nullptr
-    long long *attempts, *accepts; // [S][R]
 };
-
-// barrier of the CTAs that work on one sample (gridDim.x * gridDim.z of them), split in two halves so that work
-// that does not depend on the other CTAs (staging the next phase's graph data) overlaps the barrier latency.
-// `target` counts arrivals so far.  Thread 0 releases the CTA's stores (fence) and arrives; later it polls with
-// relaxed loads, and its trailing fence + bar.sync order every thread's later (weak, L1-cached) loads after the
-// other CTAs' stores, as cooperative groups' grid sync does (MEMBAR.SC.GPU + CCTL.IVALL in SASS).
-__device__ __forceinline__ void sample_barrier_arrive(unsigned int *bar, unsigned int &target, unsigned int n_cta) {
-    __syncthreads();
-    target += n_cta;
-    if (n_cta > 1u && threadIdx.x == 0) {
-        __threadfence();
-        atomicAdd(bar, 1u);
-    }
-}
-__device__ __forceinline__ void sample_barrier_wait(const unsigned int *bar, unsigned int target, unsigned int n_cta) {
-    if (n_cta > 1u) {
-        if (threadIdx.x == 0) {
-            while (ld_relaxed_gpu(bar) < target) { }     // relaxed polls: no L1 invalidation per iteration
-            __threadfence();                              // acquire side: MEMBAR + CCTL.IVALL once
-        }
-    }
-    __syncthreads();
-}
-
-// ---- phase sequencing (uniform over the grid) ---------------------------------------------------------------
-enum : int { kPhaseSwap = 3 };
-struct PhaseDesc { int mode, colour; uint32_t sweep; int flag; };   // flag: measure -> accumulate; swap: sweep = round
-struct PhaseIter { int rep = 0, k = 1, stage = 0, c = 0, o = 0; bool fresh = false; };
-
-// the order of DESIGN.md section 2 as a state machine; returns false when the launch is complete
-__device__ __forceinline__ bool next_phase(const SweepArgs &a, PhaseIter &it, PhaseDesc &d) {
-    for (;;) {
-        if (it.rep >= a.n_rep) return false;
-        const uint32_t sweep = a.sweep0 + static_cast<uint32_t>(it.rep) * static_cast<uint32_t>(a.sps) + static_cast<uint32_t>(it.k);
-        switch (it.stage) {
-            case 0:     // Metropolis colours of sweep k
-                if (it.k > a.sps) { it.stage = 3; break; }
-                if (a.do_met && it.c < a.c_hi) { d = PhaseDesc{kModeMetropolis, it.c++, sweep, 0}; return true; }
-                it.stage = 1; it.c = a.c_lo; it.o = 0;
-                break;
-            case 1:     // orps over-relaxation sweeps
-                if (it.o < a.orps) {
-                    if (it.c < a.c_hi) { d = PhaseDesc{kModeOverrelax, it.c++, 0u, 0}; return true; }
-                    it.o++; it.c = a.c_lo;
-                    break;
-                }
-                it.stage = 2;
-                break;
-            case 2:     // measurement of sweep k
-                it.stage = 0; it.c = a.c_lo; it.k++; it.fresh = false;
-                if (a.me > 0 && sweep % static_cast<uint32_t>(a.me) == 0u) {
-                    it.fresh = true;
-                    d = PhaseDesc{kModeMeasure, 0, 0u, 1};
-                    return true;
-                }
-                break;
-            case 3:     // energies for the swap / an explicit xy_measure
-                it.stage = 4;
-                if (a.end_measure == 2 || (a.end_measure == 1 && !it.fresh)) {
-                    d = PhaseDesc{kModeMeasure, 0, 0u, a.end_measure == 2 ? 1 : 0};
-                    return true;
-                }
-                break;
-            case 4:     // swap round
-                it.stage = 5;
-                if (a.do_swap) { d = PhaseDesc{kPhaseSwap, 0, a.round0 + static_cast<uint32_t>(it.rep), 0}; return true; }
-                break;
-            default:
-                it.rep++; it.k = 1; it.stage = 0; it.c = a.c_lo; it.fresh = false;
-                break;
-        }
-    }
-}
 
 // per-thread constants of a launch
 struct SweepCtx {
@@ -294,7 +195,7 @@ struct SweepCtx {
     int s, lane, warp, sub, q;
 };
 
-// what a warp stages for a phase BEFORE the barrier that opens it (graph data only, never theta): its share
+// what a warp stages BEFORE it waits for the preceding launch (graph data only, never theta): its share
 // [i0, w1) of the colour class, the rec[] of the share's first chunk, and that chunk's neighbour ids in shared memory
 struct PhasePrep { int i0, w1; int2 rc; };
 
@@ -354,7 +255,7 @@ __device__ __forceinline__ PhasePrep sweep_prep(const SweepArgs &sa, const Sweep
 // ---- one phase: MODE 0 Metropolis / 1 over-relaxation on a colour class, 2 measure on all sites ----
 // G lanes per site; CB = 1: the site stride R/2 equals G (known at compile time), CB = 0: G = 32, R a multiple of 64
 // larger than 64 (blockIdx.z = block of 64 slots).  P: the share and its first chunk as staged by sweep_prep (the
-// staged ids are visible: a bar.sync separates the two).  iacc: measure only, fixed-point sums (E, Mx, My) of the
+// staged ids are visible: a __syncwarp separates the two).  iacc: measure only, fixed-point sums (E, Mx, My) of the
 // .x slot, then of the .y slot.
 template <int G, int CB, int MODE>
 __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x, const PhasePrep &P, uint32_t sweep,
@@ -547,8 +448,8 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
     }
 }
 
-// CTA (x = 0, z = 0) of a sample, after the barrier that follows a measure phase: fixed-point sums -> E, M per slot,
-// optional accumulation under the slot's temperature (Eq. 13-16); leaves fx zeroed for the next measure phase
+// last CTA of a sample in a measure launch: fixed-point sums -> E, M per slot, optional accumulation under the
+// slot's temperature (Eq. 13-16); leaves fx zeroed for the next measure launch
 __device__ __forceinline__ void sweep_finalize(const TileArgs &a, int s, bool accumulate) {
     for (int r = threadIdx.x; r < a.R; r += blockDim.x) {
         long long *f = a.fx + (static_cast<size_t>(s) * a.R + r) * 3;
@@ -569,55 +470,32 @@ __device__ __forceinline__ void sweep_finalize(const TileArgs &a, int s, bool ac
     }
 }
 
-// one swap round of sample s by one CTA (R9): pairs (t, t+1), t = round (mod 2)
-__device__ __forceinline__ void sweep_swap(const SweepArgs &a, int s, uint32_t round) {
-    const int R = a.t.R;
-    const int parity = static_cast<int>(round & 1u);
-    int32_t *sot = a.slot_of_temp + static_cast<size_t>(s) * R;
-    int32_t *tos = a.temp_of_slot + static_cast<size_t>(s) * R;
-    __syncthreads();     // E_slot of sweep_finalize
-    for (int t = parity + 2 * static_cast<int>(threadIdx.x); t + 1 < R; t += 2 * blockDim.x) {
-        const int sa = sot[t], sb = sot[t + 1];
-        bool acc;
-        if (a.decisions) {
-            acc = a.decisions[static_cast<size_t>(s) * R + t] != 0;
-        } else {
-            uint32_t x[4];
-            philox4x32_10(static_cast<uint32_t>(t), round, (a.t.sample_base + static_cast<uint32_t>(s)) << 16, kDomSwap,
-                          a.t.keys, x);
-            const double u = static_cast<double>(u01(x[0]));
-            const double arg = (a.betaT[t] - a.betaT[t + 1]) *
-                               (a.t.E_slot[static_cast<size_t>(s) * R + sa] - a.t.E_slot[static_cast<size_t>(s) * R + sb]);
-            acc = u < exp(arg);
-        }
-        a.attempts[static_cast<size_t>(s) * R + t] += 1;
-        if (acc) {
-            a.accepts[static_cast<size_t>(s) * R + t] += 1;
-            sot[t] = sb; sot[t + 1] = sa;
-            tos[sa] = t + 1; tos[sb] = t;
-        }
-    }
-    __syncthreads();
-    for (int r = threadIdx.x; r < R; r += blockDim.x) {
-        const int t = tos[r];
-        a.beta_slot[static_cast<size_t>(s) * R + r] = a.beta_f[t];
-        a.w_slot[static_cast<size_t>(s) * R + r] = a.w_f[t];
-    }
-}
-
-// ---- one phase per launch (the path for large samples): same share / chunk / row code as k_sweep, but every colour
-// class is its own kernel, so each mode gets its own register allocation (64 registers, no spills) and the hardware
-// does the grid-wide ordering.  The launches are captured in a CUDA graph with PROGRAMMATIC DEPENDENT LAUNCH edges:
+// ---- the kernel: one colour class (or the measure pass) per launch, so each mode gets its own register allocation
+// (64 registers, no spills) and the hardware does the grid-wide ordering between colour classes.  grid (x = CTAs per
+// sample and column block, y = samples of the group, z = blocks of 64 slots).
+// The launches are captured in a CUDA graph with PROGRAMMATIC DEPENDENT LAUNCH edges:
 // a kernel lets its successor start early (griddepcontrol.launch_dependents); the successor's CTAs become resident
 // as soon as CTAs of this kernel retire, stage their graph data (sweep_prep: never theta), and only then wait for
 // this kernel to complete and flush (griddepcontrol.wait).  Ramp-up thus overlaps the predecessor's tail.
 // MODE 0 / 1: Metropolis / over-relaxation on colour a.t.colour; MODE 2: measure (a.t.accumulate), the last CTA of
-// the sample converts the fixed-point sums.  grid as k_sweep (need not be co-resident).
+// the sample converts the fixed-point sums.
+#ifdef XY_TRACE   // tuning builds only (_work): per-warp time stamps of the last k_phase launch
+__device__ unsigned long long g_trace[8192][4];
+__device__ __forceinline__ unsigned long long trace_now() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#endif
+
 template <int G, int CB, int MODE>
 __global__ void __launch_bounds__(kBlock, kSweepMinBlocks) k_phase(const SweepArgs a) {
     __shared__ SweepWarp s_w[kWarps];
     __shared__ int s_last;
     constexpr int SPW = 32 / G;
+#ifdef XY_TRACE
+    const unsigned long long tr0 = trace_now();
+#endif
 
     SweepCtx x;
     x.s = a.t.s0 + blockIdx.y;
@@ -640,7 +518,18 @@ __global__ void __launch_bounds__(kBlock, kSweepMinBlocks) k_phase(const SweepAr
 
     long long iacc[6] = {0, 0, 0, 0, 0, 0};
     const uint32_t sweep = a.t.use_counter ? a.t.counters[0] + static_cast<uint32_t>(a.t.sweep_offset) : a.t.sweep_fixed;
+#ifdef XY_TRACE
+    const unsigned long long tr1 = trace_now();
+#endif
     sweep_phase<G, CB, MODE>(a.t, x, P, sweep, iacc);
+#ifdef XY_TRACE
+    if (x.lane == 0 && blockIdx.y == 0 && blockIdx.z == 0 && blockIdx.x * kWarps + x.warp < 8192) {
+        unsigned long long *o = g_trace[blockIdx.x * kWarps + x.warp];
+        unsigned smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        o[0] = tr0; o[1] = tr1; o[2] = trace_now(); o[3] = (static_cast<unsigned long long>(smid) << 32) | static_cast<unsigned>(P.w1 - P.i0);
+    }
+#endif
 
     if constexpr (MODE == kModeMeasure) {
         __syncthreads();
@@ -669,82 +558,6 @@ __global__ void __launch_bounds__(kBlock, kSweepMinBlocks) k_phase(const SweepAr
             sweep_finalize(a.t, x.s, a.t.accumulate != 0);
             if (threadIdx.x == 0) a.t.ticket[x.s] = 0u;
         }
-    }
-}
-
-// ---- the kernel: grid (x = CTAs per sample and column block, y = samples of the group, z = blocks of 64 slots),
-// launched cooperatively (all CTAs resident) ---------------------------------------------------------------------
-template <int G, int CB>
-__global__ void __launch_bounds__(kBlock, kSweepMinBlocks) k_sweep(const SweepArgs a) {
-    __shared__ SweepWarp s_w[kWarps];
-    constexpr int SPW = 32 / G;
-
-    SweepCtx x;
-    x.s = a.t.s0 + blockIdx.y;
-    x.lane = threadIdx.x & 31;
-    x.warp = threadIdx.x >> 5;
-    x.sub = x.lane / G;
-    x.q = blockIdx.z * G + x.lane % G;          // slot pair handled by this lane
-    const uint32_t R2 = CB ? static_cast<uint32_t>(G) : static_cast<uint32_t>(a.t.R >> 1);
-    x.lb = reinterpret_cast<float2 *>(a.t.theta) + static_cast<size_t>(x.s) * a.t.N * R2 + x.q;
-    asm volatile("" : "+l"(x.lb));   // keep the lane's base as one materialised pointer: gather address = one IMAD.WIDE.U32
-    x.rec = a.t.rec + static_cast<size_t>(x.s) * a.t.N;
-    x.sidx = s_w[x.warp].idx;
-    x.ring_l = &s_w[x.warp].ring[0][0][x.lane];
-    x.ring_s = static_cast<uint32_t>(__cvta_generic_to_shared(x.ring_l));
-
-    unsigned int *bar = a.bar + x.s;
-    unsigned int target = 0;
-    const unsigned int n_cta = gridDim.x * gridDim.z;
-    const bool cta0 = blockIdx.x == 0 && blockIdx.z == 0;
-
-    PhaseIter it;
-    it.c = a.c_lo;
-    PhaseDesc cur, nxt;
-    bool more = next_phase(a, it, cur);
-    PhasePrep P;
-    P.i0 = P.w1 = 0; P.rc = make_int2(0, 0);
-    if (more && cur.mode != kPhaseSwap) P = sweep_prep<G, CB>(a, x, cur.mode, cur.colour);
-    __syncthreads();
-
-    while (more) {
-        long long iacc[6] = {0, 0, 0, 0, 0, 0};
-        switch (cur.mode) {
-            case kModeMetropolis: sweep_phase<G, CB, kModeMetropolis>(a.t, x, P, cur.sweep, iacc); break;
-            case kModeOverrelax: sweep_phase<G, CB, kModeOverrelax>(a.t, x, P, 0u, iacc); break;
-            case kModeMeasure: {
-                // every CTA reduces its sites: one fixed-point atomic per (slot, quantity) and CTA
-                sweep_phase<G, CB, kModeMeasure>(a.t, x, P, 0u, iacc);
-                __syncthreads();
-                long long *s_red = reinterpret_cast<long long *>(&s_w[0]);      // the ring is free now
-#pragma unroll
-                for (int c = 0; c < 6; ++c) s_red[(x.warp * 32 + x.lane) * 6 + c] = iacc[c];
-                __syncthreads();
-                if (threadIdx.x < G * 6) {
-                    const int ll = threadIdx.x / 6, c = threadIdx.x % 6;
-                    long long v = 0;
-                    for (int wi = 0; wi < kWarps; ++wi)
-                        for (int sb = 0; sb < SPW; ++sb) v += s_red[(wi * 32 + sb * G + ll) * 6 + c];
-                    const int slot = 2 * (blockIdx.z * G + ll) + c / 3;
-                    atomicAdd(reinterpret_cast<unsigned long long *>(a.t.fx) + (static_cast<size_t>(x.s) * a.t.R + slot) * 3 + c % 3,
-                              static_cast<unsigned long long>(v));
-                }
-                break;
-            }
-            default:    // swap round: one CTA per sample
-                if (cta0) sweep_swap(a, x.s, cur.sweep);
-                break;
-        }
-        more = next_phase(a, it, nxt);
-        // barrier, with the next phase's graph data staged between arrival and wait
-        sample_barrier_arrive(bar, target, n_cta);
-        P.i0 = P.w1 = 0;
-        if (more && nxt.mode != kPhaseSwap) P = sweep_prep<G, CB>(a, x, nxt.mode, nxt.colour);
-        sample_barrier_wait(bar, target, n_cta);
-        // after a measure phase CTA 0 of the sample converts and (optionally) accumulates; the others go on:
-        // nothing they touch before the next barrier is written by sweep_finalize
-        if (cur.mode == kModeMeasure && cta0) sweep_finalize(a.t, x.s, cur.flag != 0);
-        cur = nxt;
     }
 }
 
