@@ -219,11 +219,14 @@ def main():
     bytes_alg = w.bytes_per_update() * upd_per_step * args.steps      # per rank
     achieved = bytes_alg / (ms_k * 1e-3) * 1e-9                       # GB/s
     peak, peak_src = measured_peak()
-    traffic = None
-    tj = os.path.join(ROOT, "profiles", "roofline_traffic.json")
-    if os.path.exists(tj):
+    traffic = None          # ncu dram__bytes per launch of this kernel on this workload (profiles/roofline_traffic.md)
+    tc = os.path.join(ROOT, "profiles", "roofline_traffic.csv")
+    if os.path.exists(tc):
         try:
-            traffic = json.load(open(tj)).get(w.name, {}).get("dram_bytes_per_launch")
+            import csv
+            for row in csv.DictReader(open(tc)):
+                if row["workload"] == w.name:
+                    traffic = float(row["dram_bytes_per_launch"])
         except Exception:
             traffic = None
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
