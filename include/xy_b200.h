@@ -110,8 +110,10 @@ int xy_set_schedule(xy_pt *pt, int samples_per_group);
  * every setting (tests/test_gpu_parity.py).  balance != 0: cost-balanced shares of a colour class per warp (default),
  * 0: equal shares.  pdl != 0: programmatic-dependent-launch edges between the colour-class launches (default).
  * l2_persist != 0: theta of the running sample group is marked persisting in L2 through an access-policy window
- * (default).  Synchronises the stream and drops the captured graphs. */
-int xy_set_tuning(xy_pt *pt, int balance, int pdl, int l2_persist);
+ * (default).  fuse_measure != 0: in xy_run the last over-relaxation sweep of a measured sweep also produces E, Mx, My
+ * (the local field already holds cos/sin of every neighbour), 0: a separate measure launch (default on).
+ * Synchronises the stream and drops the captured graphs. */
+int xy_set_tuning(xy_pt *pt, int balance, int pdl, int l2_persist, int fuse_measure);
 
 /* ---- single-colour steps (lockstep parity tests) ----
  * Metropolis on colour class `colour` of every sample with Philox sweep index `sweep` (the handle's

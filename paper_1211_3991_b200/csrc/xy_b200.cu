@@ -58,7 +58,8 @@ const void *phase_function_mode(int G, bool single_block) {
 }
 const void *phase_function(int G, bool single_block, int mode) {
     return mode == 0 ? phase_function_mode<0>(G, single_block)
-         : mode == 1 ? phase_function_mode<1>(G, single_block) : phase_function_mode<2>(G, single_block);
+         : mode == 1 ? phase_function_mode<1>(G, single_block)
+         : mode == 2 ? phase_function_mode<2>(G, single_block) : phase_function_mode<3>(G, single_block);
 }
 
 }  // namespace
@@ -111,7 +112,8 @@ struct xy_pt {
     size_t l2_persist_bytes = 0, l2_window_max = 0;   // device limits (0 = not supported)
     int balance = 1;                 // cost-balanced share tables (1) or equal shares (0)
     int pdl = 1;                     // programmatic dependent launch edges between the k_phase launches
-    const void *phase_fn[3] = {nullptr, nullptr, nullptr};   // k_phase<G, CB, MODE>
+    const void *phase_fn[4] = {nullptr, nullptr, nullptr, nullptr};   // k_phase<G, CB, MODE>
+    int fuse_measure = 1;            // measured sweeps: the last over-relaxation sweep also produces E, Mx, My (MODE 3)
     std::map<int, int32_t *> parts;  // warps per sample -> device [S][q_stride][nw + 1] cost-balanced share tables
     int sweep_capacity = 0;          // co-resident CTAs of k_phase on this device: the grid is one such wave
     int measure_chunk = 256;  // sites per CTA of the generic measure kernel
@@ -170,7 +172,7 @@ int get_partition(xy_pt *pt, int nw, const int32_t **out) {
             pre[0] = 0;
             for (int i = cbeg; i < cend; ++i) {
                 const int deg = static_cast<int>(dg[i] & 0xffffu), nlow = static_cast<int>(dg[i] >> 16);
-                pre[i - cbeg + 1] = pre[i - cbeg] + (meas ? 10 + deg - nlow : 12 + deg);
+                pre[i - cbeg + 1] = pre[i - cbeg] + (meas ? 10 + nlow : 12 + deg);
             }
             const long long total = pre[cend - cbeg];
             int32_t *row = h.data() + (static_cast<size_t>(s) * QS + c) * (nw + 1);
@@ -226,14 +228,14 @@ int l2_window_attr(const xy_pt *pt, int s0, int s1, cudaLaunchAttribute *attr) {
 // one phase (mode 0 Metropolis / 1 over-relaxation on `colour`, 2 measure) of samples s0..s1-1 as one k_phase launch
 // with a programmatic-dependent-launch edge to its predecessor in the stream
 int launch_phase(xy_pt *pt, int mode, int colour, int s0, int s1, bool use_counter, int sweep_offset, uint32_t sweep_fixed,
-                 bool accumulate) {
+                 int accumulate /* bit 0: add to the accumulators; bit 1 (mode 3): this launch converts the sums */) {
     const xy_graph *g = pt->g;
     const int nmax = mode == 2 ? g->N : max_class_size(g, colour, s0, s1);
     if (nmax == 0 || s1 <= s0) return XY_OK;
     xy::SweepArgs a = sweep_args(pt, s0);
     a.t.colour = colour;
     a.t.sweep_fixed = sweep_fixed; a.t.sweep_offset = sweep_offset; a.t.use_counter = use_counter ? 1 : 0;
-    a.t.accumulate = accumulate ? 1 : 0;
+    a.t.accumulate = accumulate;
     const int gx = sweep_grid_x(pt, s1 - s0, nmax);
     if (pt->balance) {
         const int rc = get_partition(pt, gx * xy::kWarps, &a.part);
@@ -262,7 +264,7 @@ int launch_phase(xy_pt *pt, int mode, int colour, int s0, int s1, bool use_count
 // the any-R kernels when R has none (odd R, R = 6, 10, ...) ----
 template <int MODE>
 int launch_class(xy_pt *pt, int colour, int s0, int s1, bool use_counter, int sweep_offset, uint32_t sweep_fixed) {
-    if (pt->fast_G) return launch_phase(pt, MODE, colour, s0, s1, use_counter, sweep_offset, sweep_fixed, false);
+    if (pt->fast_G) return launch_phase(pt, MODE, colour, s0, s1, use_counter, sweep_offset, sweep_fixed, 0);
     const xy_graph *g = pt->g;
     const int nmax = max_class_size(g, colour, s0, s1);
     if (nmax == 0 || s1 <= s0) return XY_OK;
@@ -279,7 +281,7 @@ int launch_class(xy_pt *pt, int colour, int s0, int s1, bool use_counter, int sw
 }
 
 int launch_measure(xy_pt *pt, int s0, int s1, bool accumulate) {
-    if (pt->fast_G) return launch_phase(pt, 2, 0, s0, s1, false, 0, 0u, accumulate);
+    if (pt->fast_G) return launch_phase(pt, 2, 0, s0, s1, false, 0, 0u, accumulate ? 1 : 0);
     const xy_graph *g = pt->g;
     if (s1 <= s0) return XY_OK;
     xy::TileArgs a = tile_args(pt, 0, s0);
@@ -328,6 +330,21 @@ int auto_group(const xy_pt *pt) {
 }
 
 // enqueue one PT cycle on the stream; `phase` = sweep counter mod measure_every at entry
+// one over-relaxation sweep of samples s0..s1-1 whose launches also produce the sweep's E, Mx, My (k_phase MODE 3);
+// the launch of the last non-empty colour class converts the sums (and accumulates them when `accumulate`)
+int sweep_group_fused(xy_pt *pt, int s0, int s1, bool accumulate) {
+    const xy_graph *g = pt->g;
+    int last = -1;
+    for (int c = 0; c < g->q_max; ++c)
+        if (max_class_size(g, c, s0, s1) > 0) last = c;
+    if (last < 0) return launch_measure(pt, s0, s1, accumulate);
+    for (int c = 0; c <= last; ++c) {
+        const int rc = launch_phase(pt, 3, c, s0, s1, false, 0, 0u, (accumulate ? 1 : 0) | (c == last ? 2 : 0));
+        if (rc != XY_OK) return rc;
+    }
+    return XY_OK;
+}
+
 int issue_cycle(xy_pt *pt, int sps, int orps, int me, int phase, int group) {
     const int S = pt->g->S;
     for (int s0 = 0; s0 < S; s0 += group) {
@@ -336,10 +353,17 @@ int issue_cycle(xy_pt *pt, int sps, int orps, int me, int phase, int group) {
         for (int k = 1; k <= sps; ++k) {
             int rc = sweep_group(pt, 0, s0, s1, true, k, 0u);
             if (rc != XY_OK) return rc;
-            for (int o = 0; o < orps; ++o)
-                if ((rc = sweep_group(pt, 1, s0, s1, false, 0, 0u)) != XY_OK) return rc;
-            fresh = false;
-            if (me > 0 && (phase + k) % me == 0) {
+            const bool measured = me > 0 && (phase + k) % me == 0;
+            // E is needed after this sweep: for the accumulators, or (last sweep of the cycle) for the swap round
+            const bool need_e = measured || k == sps;
+            const bool fuse = need_e && pt->fast_G && pt->fuse_measure && orps > 0;
+            for (int o = 0; o < orps; ++o) {
+                if (fuse && o == orps - 1) rc = sweep_group_fused(pt, s0, s1, measured);
+                else rc = sweep_group(pt, 1, s0, s1, false, 0, 0u);
+                if (rc != XY_OK) return rc;
+            }
+            fresh = fuse;
+            if (measured && !fuse) {
                 if ((rc = launch_measure(pt, s0, s1, true)) != XY_OK) return rc;
                 fresh = true;
             }
@@ -595,7 +619,7 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
     pt->keys = xy::philox_key_schedule(pt->key0, pt->key1);
     pt->measure_chunk = std::max(256, ((N + 127) / 128 + 7) / 8 * 8);   // legacy measure partition: a function of N only
     if (pt->fast_G) {
-        for (int m = 0; m < 3; ++m) {
+        for (int m = 0; m < 4; ++m) {
             pt->phase_fn[m] = phase_function(pt->fast_G, pt->col_blocks == 1, m);
             cudaFuncSetAttribute(pt->phase_fn[m], cudaFuncAttributePreferredSharedMemoryCarveout,
                                  static_cast<int>(cudaSharedmemCarveoutMaxShared));
@@ -789,10 +813,11 @@ int xy_set_schedule(xy_pt *pt, int samples_per_group) {
     return XY_OK;
 }
 
-int xy_set_tuning(xy_pt *pt, int balance, int pdl, int l2_persist) {
+int xy_set_tuning(xy_pt *pt, int balance, int pdl, int l2_persist, int fuse_measure) {
     if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
     XY_CUDA(cudaStreamSynchronize(pt->stream));
     pt->balance = balance ? 1 : 0; pt->pdl = pdl ? 1 : 0; pt->l2_persist = l2_persist ? 1 : 0;
+    pt->fuse_measure = fuse_measure ? 1 : 0;
     drop_graphs(pt);
     return XY_OK;
 }

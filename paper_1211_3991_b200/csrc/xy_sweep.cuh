@@ -68,6 +68,8 @@ __device__ __forceinline__ float mant12(uint32_t x) { return __uint_as_float((x 
 //   |x| <= 1:  x + 3  lies in [2, 4],   ulp 2^-22, so bits(x + 3)  - bits(3)  = rn(x 2^22)
 __device__ __forceinline__ int quant8(float x) { return __float_as_int(__fadd_rn(x, 24.0f)) - 0x41C00000; }
 __device__ __forceinline__ int quant1(float x) { return __float_as_int(__fadd_rn(x, 3.0f)) - 0x40400000; }
+//   |x| <= 32: x + 96 lies in [64, 128], ulp 2^-17, so bits(x + 96) - bits(96) = rn(x 2^17)
+__device__ __forceinline__ int quant32(float x) { return __float_as_int(__fadd_rn(x, 96.0f)) - 0x42C00000; }
 
 // ---- cp.async (LDGSTS): 8 bytes per lane, global -> shared, no register staging ---------------------------
 __device__ __forceinline__ void cp_async8(uint32_t smem_addr, const void *gptr) {
@@ -78,17 +80,18 @@ template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // ---- per-lane state of one site (two slots) ----------------------------------------------------------
+// add(t, k): t = the angles of the site's k-th neighbour (CSR order) in the lane's two slots
 template <int MODE> struct PairAcc;
 template <> struct PairAcc<kModeMetropolis> {
     float2 mid, s = make_float2(0.f, 0.f);
-    __device__ __forceinline__ void add(const float2 t) {
+    __device__ __forceinline__ void add(const float2 t, int) {
         const float2 d = sub2(mid, t);
         s = add2(s, make_float2(__sinf(d.x), __sinf(d.y)));
     }
 };
 template <> struct PairAcc<kModeOverrelax> {
     float2 hx = make_float2(0.f, 0.f), hy = make_float2(0.f, 0.f);   // hx = (h_x of slot .x, h_x of slot .y)
-    __device__ __forceinline__ void add(const float2 t) {
+    __device__ __forceinline__ void add(const float2 t, int) {
         float sx, cx, sy, cy;
         __sincosf(t.x, &sx, &cx);
         __sincosf(t.y, &sy, &cy);
@@ -96,21 +99,47 @@ template <> struct PairAcc<kModeOverrelax> {
         hy = add2(hy, make_float2(sx, sy));
     }
 };
+// measure: l = sum over the LOWER neighbours j < i (the head of the ascending list: every bond is counted once, at
+// its upper end) of (cos th_j, sin th_j); the bond energy of the site is then cos th_i l_x + sin th_i l_y
+// (site_energy_fixed).  Only lower neighbours are gathered, so every add() is a lower one.
 template <> struct PairAcc<kModeMeasure> {
-    float2 own, e = make_float2(0.f, 0.f);
-    __device__ __forceinline__ void add(const float2 t) {
-        const float2 d = sub2(own, t);
-        e = add2(e, make_float2(__cosf(d.x), __cosf(d.y)));
+    float2 lx = make_float2(0.f, 0.f), ly = make_float2(0.f, 0.f);
+    __device__ __forceinline__ void add(const float2 t, int) {
+        float sx, cx, sy, cy;
+        __sincosf(t.x, &sx, &cx);
+        __sincosf(t.y, &sy, &cy);
+        lx = add2(lx, make_float2(cx, cy));
+        ly = add2(ly, make_float2(sx, sy));
     }
-    // fixed-point flush after every batch of <= 8 bonds (|e| <= 8): the integer sums do not depend on who adds them
-    __device__ __forceinline__ void flush(long long &ex, long long &ey) {
-        ex += quant8(e.x); ey += quant8(e.y);
-        e = make_float2(0.f, 0.f);
+};
+// over-relaxation with the measurement as a by-product: the local field h needs (cos th_j, sin th_j) of every
+// neighbour anyway; the partial field l of the lower neighbours is the same sum, in the same order, that the measure
+// kernel forms, so both give bit-identical energies.  After the class's update th_i and all its lower neighbours are
+// final for this sweep (colour-major numbering: j < i has a lower or equal colour, and same-colour sites share no bond).
+template <> struct PairAcc<kModeOrMeasure> {
+    float2 hx = make_float2(0.f, 0.f), hy = make_float2(0.f, 0.f), lx = make_float2(0.f, 0.f), ly = make_float2(0.f, 0.f);
+    int nlow = 0;
+    __device__ __forceinline__ void add(const float2 t, int k) {
+        float sx, cx, sy, cy;
+        __sincosf(t.x, &sx, &cx);
+        __sincosf(t.y, &sy, &cy);
+        hx = add2(hx, make_float2(cx, cy));
+        hy = add2(hy, make_float2(sx, sy));
+        if (k < nlow) {
+            lx = add2(lx, make_float2(cx, cy));
+            ly = add2(ly, make_float2(sx, sy));
+        }
     }
 };
 
+// fixed-point (scale 2^19) bond energy of one slot of a site: -E_i = cos th_i l_x + sin th_i l_y, |.| <= nlow.
+// Explicit fma/mul so that the measure kernel and the fused over-relaxation kernel round identically.
+__device__ __forceinline__ float site_energy(float c, float s, float lx, float ly) {
+    return __fmaf_rn(c, lx, __fmul_rn(s, ly));
+}
+
 // per-lane description of the site a lane works on in the current row (warp-uniform when SPW == 1)
-struct RowSite { int i, deg, pos; bool valid; };
+struct RowSite { int i, deg, pos, nlow; bool valid; };
 
 // direct gather of the neighbour with pre-scaled id `sid` (float2 units), L2 only: one IMAD.WIDE.U32 + one LDG.64
 __device__ __forceinline__ float2 sweep_ld(const float2 *lb, uint32_t sid) {
@@ -158,7 +187,7 @@ __device__ __forceinline__ void sweep_consume_n(ACC &acc, const float2 *row0, in
             if (b + u < D) v[u] = row0[(b + u) * 32];
 #pragma unroll
         for (int u = 0; u < 4; ++u)
-            if (b + u < D && (UNI || b + u < deg)) acc.add(v[u]);
+            if (b + u < D && (UNI || b + u < deg)) acc.add(v[u], b + u);
     }
 }
 
@@ -252,14 +281,15 @@ __device__ __forceinline__ PhasePrep sweep_prep(const SweepArgs &sa, const Sweep
     return P;
 }
 
-// ---- one phase: MODE 0 Metropolis / 1 over-relaxation on a colour class, 2 measure on all sites ----
+// ---- one phase: MODE 0 Metropolis / 1 over-relaxation / 3 over-relaxation + measure by-product on a colour class,
+// 2 measure on all sites ----
 // G lanes per site; CB = 1: the site stride R/2 equals G (known at compile time), CB = 0: G = 32, R a multiple of 64
 // larger than 64 (blockIdx.z = block of 64 slots).  P: the share and its first chunk as staged by sweep_prep (the
-// staged ids are visible: a __syncwarp separates the two).  iacc: measure only, fixed-point sums (E, Mx, My) of the
-// .x slot, then of the .y slot.
+// staged ids are visible: a __syncwarp separates the two).  iacc: measure modes only, 32-bit fixed-point partial sums
+// (E, Mx, My) of the .x slot, then of the .y slot.
 template <int G, int CB, int MODE>
 __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x, const PhasePrep &P, uint32_t sweep,
-                                            long long (&iacc)[6]) {
+                                            int (&iacc)[6]) {
     constexpr int SPW = 32 / G;
     constexpr bool UNI = SPW == 1;
     const uint32_t R2 = CB ? static_cast<uint32_t>(G) : static_cast<uint32_t>(a.R >> 1);
@@ -282,7 +312,7 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
     }
 
     // Metropolis proposal of site i (both slots of the lane): th' = th + w (u1 - 1/2), half = (th' - th)/2
-    auto begin = [&](int i, const float2 own, PairAcc<MODE> &acc, float2 &thp, float2 &u2) {
+    auto begin = [&](int i, int nlow, const float2 own, PairAcc<MODE> &acc, float2 &thp, float2 &u2) {
         if constexpr (MODE == kModeMetropolis) {
             uint32_t r[4];
             philox4x32_10(static_cast<uint32_t>(i), sweep, c2, kDomMetropolis, a.keys, r);
@@ -295,11 +325,49 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
             // ptxas contracts mul.rn.f32x2 + add.rn.f32x2 into one FFMA2 (single rounding, 1 ulp off in 11 % of the moves)
             thp = make_float2(__fadd_rn(own.x, __fmul_rn(w.x, u1mh.x)), __fadd_rn(own.y, __fmul_rn(w.y, u1mh.y)));
             acc.mid = add2(own, mul2(sub2(thp, own), make_float2(0.5f, 0.5f)));
-        } else if constexpr (MODE == kModeMeasure) {
-            acc.own = own;
+        } else if constexpr (MODE == kModeOrMeasure) {
+            acc.nlow = nlow;
         }
     };
-    auto finish = [&](int i, bool valid, const float2 own, PairAcc<MODE> &acc, const float2 thp, const float2 u2) {
+    // measure by-product of one site: fixed-point bond energy (lower neighbours) and magnetisation of both slots
+    // The per-lane partial sums are 32-bit.  A site adds at most 2^22 per quantity (one "unit"), or 2^24 to the energy
+    // when it has 9..32 lower neighbours (coarser quantiser, 4 units); the partial sums are flushed to the 64-bit sums
+    // in global memory before 2^31 can be reached (rarely: same-address atomics are slow).  A site with more than 32
+    // lower neighbours goes to the 64-bit sum directly.
+    auto fx_lane = [&]() {      // this lane's six 64-bit sums (recomputed where needed: cold code, no live registers)
+        return reinterpret_cast<unsigned long long *>(a.fx) + (static_cast<size_t>(x.s) * a.R + 2 * x.q) * 3;
+    };
+    int units = 0;
+    auto tally = [&](const float2 th, const float2 lx, const float2 ly, int nlow) {
+        float sx, cx, sy, cy;
+        __sincosf(th.x, &sx, &cx);
+        __sincosf(th.y, &sy, &cy);
+        const float ex = site_energy(cx, sx, lx.x, ly.x), ey = site_energy(cy, sy, lx.y, ly.y);
+        units += 1;
+        if (nlow <= 8) {
+            iacc[0] += quant8(ex);
+            iacc[3] += quant8(ey);
+        } else if (nlow <= 32) {
+            iacc[0] += quant32(ex) << 2;
+            iacc[3] += quant32(ey) << 2;
+            units += 3;
+        } else {
+            atomicAdd(fx_lane(), static_cast<unsigned long long>(__double2ll_rn(static_cast<double>(ex) * 524288.0)));
+            atomicAdd(fx_lane() + 3, static_cast<unsigned long long>(__double2ll_rn(static_cast<double>(ey) * 524288.0)));
+        }
+        iacc[1] += quant1(cx); iacc[2] += quant1(sx);
+        iacc[4] += quant1(cy); iacc[5] += quant1(sy);
+    };
+    auto flush_partial = [&]() {
+        unsigned long long *fxl = fx_lane();
+#pragma unroll
+        for (int c = 0; c < 6; ++c) {
+            atomicAdd(fxl + c, static_cast<unsigned long long>(static_cast<long long>(iacc[c])));
+            iacc[c] = 0;
+        }
+    };
+
+    auto finish = [&](int i, int nlow, bool valid, const float2 own, PairAcc<MODE> &acc, const float2 thp, const float2 u2) {
         if constexpr (MODE == kModeMetropolis) {
             // dE = 2 sin((th'-th)/2) sum_j sin((th'+th)/2 - th_j)
             const float2 half = mul2(sub2(thp, own), make_float2(0.5f, 0.5f));      // recomputed: two registers fewer across the gather
@@ -314,14 +382,16 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
             out.x = overrelax_finish(own.x, acc.hx.x, acc.hy.x);
             out.y = overrelax_finish(own.y, acc.hx.y, acc.hy.y);
             if (UNI || valid) lb[static_cast<unsigned long long>(static_cast<uint32_t>(i) * R2)] = out;
-        } else {
+        } else if constexpr (MODE == kModeOrMeasure) {
+            float2 out;
+            out.x = overrelax_finish(own.x, acc.hx.x, acc.hy.x);
+            out.y = overrelax_finish(own.y, acc.hx.y, acc.hy.y);
             if (UNI || valid) {
-                float sx, cx, sy, cy;
-                __sincosf(own.x, &sx, &cx);
-                __sincosf(own.y, &sy, &cy);
-                iacc[1] += quant1(cx); iacc[2] += quant1(sx);
-                iacc[4] += quant1(cy); iacc[5] += quant1(sy);
+                lb[static_cast<unsigned long long>(static_cast<uint32_t>(i) * R2)] = out;
+                tally(out, acc.lx, acc.ly, nlow);
             }
+        } else {
+            if (UNI || valid) tally(own, acc.lx, acc.ly, nlow);
         }
     };
     // neighbours beyond the pipelined kDB: direct loads in groups of 4 (rare: P(deg > 8) ~ 15 % at z = 6)
@@ -333,8 +403,7 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
                 if (k + u < deg) t[u] = sweep_ld(lb, sidx[pos + k + u]);
 #pragma unroll
             for (int u = 0; u < 4; ++u)
-                if (k + u < deg) acc.add(t[u]);
-            if constexpr (MODE == kModeMeasure) acc.flush(iacc[0], iacc[3]);
+                if (k + u < deg) acc.add(t[u], k + u);
         }
     };
 
@@ -353,15 +422,16 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
         if (msite == 0) {
             // a single site with more neighbours than the staging slice: lane group 0 walks its ids in blocks
             const int ry = __shfl_sync(kFull, rc.y, 0);
-            int deg = ry & 0xffff, pos = 0;
-            if constexpr (MODE == kModeMeasure) { pos = ry >> 16; deg -= pos; }
-            const int32_t *gidx = a.col_idx + start0 + pos;
+            int deg = ry & 0xffff;
+            const int nlow = ry >> 16;
+            if constexpr (MODE == kModeMeasure) deg = nlow;      // lower neighbours only: the head of the list
+            const int32_t *gidx = a.col_idx + start0;
             const bool valid = UNI || sub == 0;
             float2 own = make_float2(0.f, 0.f);
             if (valid) own = __ldcg(lb + static_cast<unsigned long long>(static_cast<uint32_t>(i0) * R2));
             float2 thp = make_float2(0.f, 0.f), u2 = thp;
             PairAcc<MODE> acc;
-            begin(i0, own, acc, thp, u2);
+            begin(i0, nlow, own, acc, thp, u2);
             for (int k0 = 0; k0 < deg; k0 += kStageCap) {
                 const int nb = min(kStageCap, deg - k0);
                 __syncwarp();
@@ -374,11 +444,10 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
                         if (k + u < nb && valid) t[u] = sweep_ld(lb, sidx[k + u]);
 #pragma unroll
                     for (int u = 0; u < 4; ++u)
-                        if (k + u < nb && valid) acc.add(t[u]);
-                    if constexpr (MODE == kModeMeasure) acc.flush(iacc[0], iacc[3]);
+                        if (k + u < nb && valid) acc.add(t[u], k0 + k + u);
                 }
             }
-            finish(i0, valid, own, acc, thp, u2);
+            finish(i0, nlow, valid, own, acc, thp, u2);
             __syncwarp();
             i0 += 1;
             staged = false;
@@ -400,11 +469,8 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
             st.i = i0 + m;
             st.deg = st.valid ? (ry & 0xffff) : 0;
             st.pos = rx;
-            if constexpr (MODE == kModeMeasure) {     // bonds counted once: neighbours j > i are the tail of the list
-                const int nlow = st.valid ? (ry >> 16) : 0;
-                st.pos += nlow;
-                st.deg -= nlow;
-            }
+            st.nlow = st.valid ? (ry >> 16) : 0;
+            if constexpr (MODE == kModeMeasure) st.deg = st.nlow;   // bonds counted once: neighbours j < i are the head of the list
             return st;
         };
         auto row_max = [&](int deg) { return UNI ? deg : static_cast<int>(__reduce_max_sync(kFull, static_cast<unsigned>(deg))); };
@@ -437,14 +503,19 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
             if (cur.valid) own = row0[kDB * 32];
             float2 thp = make_float2(0.f, 0.f), u2 = thp;
             PairAcc<MODE> acc;
-            begin(cur.i, own, acc, thp, u2);
+            begin(cur.i, cur.nlow, own, acc, thp, u2);
             sweep_consume<UNI>(acc, row0, cur.deg, cmax);
-            if constexpr (MODE == kModeMeasure) acc.flush(iacc[0], iacc[3]);
             if (cmax > kDB) tail(acc, cur.pos, cur.deg, cmax);
-            finish(cur.i, cur.valid, own, acc, thp, u2);
+            finish(cur.i, cur.nlow, cur.valid, own, acc, thp, u2);
         }
         __syncwarp();
         i0 += msite;
+        if constexpr (MODE == kModeMeasure || MODE == kModeOrMeasure) {
+            if (units >= 320 && i0 < w1) {      // a chunk adds at most 128 units: the partial sums stay below 448 * 2^22 < 2^31
+                flush_partial();
+                units = 0;
+            }
+        }
     }
 }
 
@@ -477,8 +548,9 @@ __device__ __forceinline__ void sweep_finalize(const TileArgs &a, int s, bool ac
 // a kernel lets its successor start early (griddepcontrol.launch_dependents); the successor's CTAs become resident
 // as soon as CTAs of this kernel retire, stage their graph data (sweep_prep: never theta), and only then wait for
 // this kernel to complete and flush (griddepcontrol.wait).  Ramp-up thus overlaps the predecessor's tail.
-// MODE 0 / 1: Metropolis / over-relaxation on colour a.t.colour; MODE 2: measure (a.t.accumulate), the last CTA of
-// the sample converts the fixed-point sums.
+// MODE 0 / 1: Metropolis / over-relaxation on colour a.t.colour; MODE 2: measure (a.t.accumulate bit 0), the last CTA
+// of the sample converts the fixed-point sums; MODE 3: over-relaxation that also adds the class's share of E, Mx, My
+// to the fixed-point sums (the measurement costs no extra gather), converted by the launch of the sweep's last colour.
 #ifdef XY_TRACE   // tuning builds only (_work): per-warp time stamps of the last k_phase launch
 __device__ unsigned long long g_trace[8192][4];
 __device__ __forceinline__ unsigned long long trace_now() {
@@ -512,11 +584,11 @@ __global__ void __launch_bounds__(kBlock, kSweepMinBlocks) k_phase(const SweepAr
     x.ring_s = static_cast<uint32_t>(__cvta_generic_to_shared(x.ring_l));
 
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    const PhasePrep P = sweep_prep<G, CB>(a, x, MODE, a.t.colour);
+    const PhasePrep P = sweep_prep<G, CB>(a, x, MODE == kModeOrMeasure ? kModeOverrelax : MODE, a.t.colour);
     __syncwarp();
     asm volatile("griddepcontrol.wait;" ::: "memory");      // the predecessor's theta / beta_slot / fx are final
 
-    long long iacc[6] = {0, 0, 0, 0, 0, 0};
+    int iacc[6] = {0, 0, 0, 0, 0, 0};
     const uint32_t sweep = a.t.use_counter ? a.t.counters[0] + static_cast<uint32_t>(a.t.sweep_offset) : a.t.sweep_fixed;
 #ifdef XY_TRACE
     const unsigned long long tr1 = trace_now();
@@ -531,11 +603,11 @@ __global__ void __launch_bounds__(kBlock, kSweepMinBlocks) k_phase(const SweepAr
     }
 #endif
 
-    if constexpr (MODE == kModeMeasure) {
+    if constexpr (MODE == kModeMeasure || MODE == kModeOrMeasure) {
         __syncthreads();
         long long *s_red = reinterpret_cast<long long *>(&s_w[0]);
 #pragma unroll
-        for (int c = 0; c < 6; ++c) s_red[(x.warp * 32 + x.lane) * 6 + c] = iacc[c];
+        for (int c = 0; c < 6; ++c) s_red[(x.warp * 32 + x.lane) * 6 + c] = static_cast<long long>(iacc[c]);
         __syncthreads();
         if (threadIdx.x < G * 6) {
             const int ll = threadIdx.x / 6, c = threadIdx.x % 6;
@@ -546,17 +618,21 @@ __global__ void __launch_bounds__(kBlock, kSweepMinBlocks) k_phase(const SweepAr
             atomicAdd(reinterpret_cast<unsigned long long *>(a.t.fx) + (static_cast<size_t>(x.s) * a.t.R + slot) * 3 + c % 3,
                       static_cast<unsigned long long>(v));
         }
-        __threadfence();
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            const unsigned int total = gridDim.x * gridDim.z;
-            s_last = (atomicAdd(a.t.ticket + x.s, 1u) == total - 1u) ? 1 : 0;
-        }
-        __syncthreads();
-        if (s_last) {
+        // the sums are complete after the measure launch, or after the fused launch of the sweep's last colour
+        // (a.t.accumulate bit 1); its last CTA converts them
+        if (MODE == kModeMeasure || (a.t.accumulate & 2)) {
             __threadfence();
-            sweep_finalize(a.t, x.s, a.t.accumulate != 0);
-            if (threadIdx.x == 0) a.t.ticket[x.s] = 0u;
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                const unsigned int total = gridDim.x * gridDim.z;
+                s_last = (atomicAdd(a.t.ticket + x.s, 1u) == total - 1u) ? 1 : 0;
+            }
+            __syncthreads();
+            if (s_last) {
+                __threadfence();
+                sweep_finalize(a.t, x.s, (a.t.accumulate & 1) != 0);
+                if (threadIdx.x == 0) a.t.ticket[x.s] = 0u;
+            }
         }
     }
 }
