@@ -112,8 +112,9 @@ int xy_set_schedule(xy_pt *pt, int samples_per_group);
  * l2_persist != 0: theta of the running sample group is marked persisting in L2 through an access-policy window
  * (default).  fuse_measure != 0: in xy_run the last over-relaxation sweep of a measured sweep also produces E, Mx, My
  * (the local field already holds cos/sin of every neighbour), 0: a separate measure launch (default on).
- * Synchronises the stream and drops the captured graphs. */
-int xy_set_tuning(xy_pt *pt, int balance, int pdl, int l2_persist, int fuse_measure);
+ * cta_shape: 0 = 32-warp CTAs (one per SM) for large colour classes and 8-warp CTAs (four per SM) for small ones
+ * (default), 1 = always 8-warp, 2 = always 32-warp.  Synchronises the stream and drops the captured graphs. */
+int xy_set_tuning(xy_pt *pt, int balance, int pdl, int l2_persist, int fuse_measure, int cta_shape);
 
 /* ---- single-colour steps (lockstep parity tests) ----
  * Metropolis on colour class `colour` of every sample with Philox sweep index `sweep` (the handle's

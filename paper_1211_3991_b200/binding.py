@@ -34,7 +34,7 @@ SYMBOLS = {
     "xy_run": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]),
     "xy_run_sweeps": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int]),
     "xy_set_schedule": (C.c_int, [C.c_void_p, C.c_int]),
-    "xy_set_tuning": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]),
+    "xy_set_tuning": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]),
     "xy_metropolis_colour": (C.c_int, [C.c_void_p, C.c_int, C.c_uint32]),
     "xy_overrelax_colour": (C.c_int, [C.c_void_p, C.c_int]),
     "xy_get_theta": (C.c_int, [C.c_void_p, C.c_void_p]),
@@ -167,8 +167,8 @@ def xy_set_schedule(pt, samples_per_group):
     _check(lib().xy_set_schedule(pt, samples_per_group))
 
 
-def xy_set_tuning(pt, balance=1, pdl=1, l2_persist=1, fuse_measure=1):
-    _check(lib().xy_set_tuning(pt, balance, pdl, l2_persist, fuse_measure))
+def xy_set_tuning(pt, balance=1, pdl=1, l2_persist=1, fuse_measure=1, cta_shape=0):
+    _check(lib().xy_set_tuning(pt, balance, pdl, l2_persist, fuse_measure, cta_shape))
 
 
 def xy_metropolis_colour(pt, colour, sweep):
@@ -296,8 +296,8 @@ class Ensemble:
     def run_sweeps(self, n_blocks, sweeps_per_block=10, or_per_sweep=1):
         xy_run_sweeps(self.pt, n_blocks, sweeps_per_block, or_per_sweep)
     def set_schedule(self, g): xy_set_schedule(self.pt, g)
-    def set_tuning(self, balance=1, pdl=1, l2_persist=1, fuse_measure=1):
-        xy_set_tuning(self.pt, balance, pdl, l2_persist, fuse_measure)
+    def set_tuning(self, balance=1, pdl=1, l2_persist=1, fuse_measure=1, cta_shape=0):
+        xy_set_tuning(self.pt, balance, pdl, l2_persist, fuse_measure, cta_shape)
     def metropolis_colour(self, c, sweep): xy_metropolis_colour(self.pt, c, sweep)
     def overrelax_colour(self, c): xy_overrelax_colour(self.pt, c)
     def get_theta(self, out=None): return xy_get_theta(self.pt, (self.S, self.N, self.R), out)

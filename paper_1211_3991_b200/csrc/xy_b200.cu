@@ -44,22 +44,23 @@ int dev_alloc(T **p, size_t n) {
 int ceil_div(long long a, long long b) { return static_cast<int>((a + b - 1) / b); }
 
 // the k_phase<G, CB, MODE> instantiation for G lanes per site (CB = 0: R a multiple of 64 larger than 64)
-template <int MODE>
+template <int MODE, int W>
 const void *phase_function_mode(int G, bool single_block) {
     switch (G) {
-        case 32: return single_block ? reinterpret_cast<const void *>(xy::k_phase<32, 1, MODE>)
-                                     : reinterpret_cast<const void *>(xy::k_phase<32, 0, MODE>);
-        case 16: return reinterpret_cast<const void *>(xy::k_phase<16, 1, MODE>);
-        case 8: return reinterpret_cast<const void *>(xy::k_phase<8, 1, MODE>);
-        case 4: return reinterpret_cast<const void *>(xy::k_phase<4, 1, MODE>);
-        case 2: return reinterpret_cast<const void *>(xy::k_phase<2, 1, MODE>);
-        default: return reinterpret_cast<const void *>(xy::k_phase<1, 1, MODE>);
+        case 32: return single_block ? reinterpret_cast<const void *>(xy::k_phase<32, 1, MODE, W>)
+                                     : reinterpret_cast<const void *>(xy::k_phase<32, 0, MODE, W>);
+        case 16: return reinterpret_cast<const void *>(xy::k_phase<16, 1, MODE, W>);
+        case 8: return reinterpret_cast<const void *>(xy::k_phase<8, 1, MODE, W>);
+        case 4: return reinterpret_cast<const void *>(xy::k_phase<4, 1, MODE, W>);
+        case 2: return reinterpret_cast<const void *>(xy::k_phase<2, 1, MODE, W>);
+        default: return reinterpret_cast<const void *>(xy::k_phase<1, 1, MODE, W>);
     }
 }
+template <int W>
 const void *phase_function(int G, bool single_block, int mode) {
-    return mode == 0 ? phase_function_mode<0>(G, single_block)
-         : mode == 1 ? phase_function_mode<1>(G, single_block)
-         : mode == 2 ? phase_function_mode<2>(G, single_block) : phase_function_mode<3>(G, single_block);
+    return mode == 0 ? phase_function_mode<0, W>(G, single_block)
+         : mode == 1 ? phase_function_mode<1, W>(G, single_block)
+         : mode == 2 ? phase_function_mode<2, W>(G, single_block) : phase_function_mode<3, W>(G, single_block);
 }
 
 }  // namespace
@@ -112,7 +113,9 @@ struct xy_pt {
     size_t l2_persist_bytes = 0, l2_window_max = 0;   // device limits (0 = not supported)
     int balance = 1;                 // cost-balanced share tables (1) or equal shares (0)
     int pdl = 1;                     // programmatic dependent launch edges between the k_phase launches
-    const void *phase_fn[4] = {nullptr, nullptr, nullptr, nullptr};   // k_phase<G, CB, MODE>
+    const void *phase_fn[2][4] = {};   // k_phase<G, CB, MODE, W>: [0] W = 8 warps per CTA, [1] W = 32
+    int capacity_big = 0;            // co-resident 32-warp CTAs (one per SM)
+    int cta_shape = 0;               // 0 = by class size, 1 = always 8-warp CTAs, 2 = always 32-warp CTAs
     int fuse_measure = 1;            // measured sweeps: the last over-relaxation sweep also produces E, Mx, My (MODE 3)
     std::map<int, int32_t *> parts;  // warps per sample -> device [S][q_stride][nw + 1] cost-balanced share tables
     int sweep_capacity = 0;          // co-resident CTAs of k_phase on this device: the grid is one such wave
@@ -195,11 +198,20 @@ int get_partition(xy_pt *pt, int nw, const int32_t **out) {
     return XY_OK;
 }
 
-// CTAs per (sample, column block) for a group of ns samples: one wave of resident CTAs shared by the group, at most
-// one row of `nmax` sites per warp
-int sweep_grid_x(const xy_pt *pt, int ns, int nmax) {
+// CTA shape and CTAs per (sample, column block) for a launch over a group of ns samples whose largest class has nmax
+// sites: one wave of resident CTAs shared by the group, at most one row per warp.  The shape is chosen per group from
+// the whole sweep (all launches of a group alike): 32-warp CTAs when a warp gets at least 32 rows per sweep.
+struct SweepGrid { int big, gx, warps; };
+SweepGrid sweep_grid(const xy_pt *pt, int ns, int nmax) {
     const int spw = 32 / pt->fast_G;
-    return std::max(1, std::min(ceil_div(nmax, xy::kWarps * spw), pt->sweep_capacity / (ns * pt->col_blocks)));
+    const long long rows = static_cast<long long>(ceil_div(pt->g->N, spw)) * ns * pt->col_blocks;
+    SweepGrid g;
+    g.big = pt->cta_shape == 2 || (pt->cta_shape == 0 && rows >= 32ll * xy::kWarpsBig * pt->capacity_big);
+    if (g.big && pt->capacity_big < ns * pt->col_blocks) g.big = 0;
+    g.warps = g.big ? xy::kWarpsBig : xy::kWarpsSmall;
+    const int cap = g.big ? pt->capacity_big : pt->sweep_capacity;
+    g.gx = std::max(1, std::min(ceil_div(nmax, g.warps * spw), cap / (ns * pt->col_blocks)));
+    return g;
 }
 
 xy::SweepArgs sweep_args(xy_pt *pt, int s0) {
@@ -236,15 +248,15 @@ int launch_phase(xy_pt *pt, int mode, int colour, int s0, int s1, bool use_count
     a.t.colour = colour;
     a.t.sweep_fixed = sweep_fixed; a.t.sweep_offset = sweep_offset; a.t.use_counter = use_counter ? 1 : 0;
     a.t.accumulate = accumulate;
-    const int gx = sweep_grid_x(pt, s1 - s0, nmax);
+    const SweepGrid sg = sweep_grid(pt, s1 - s0, nmax);
     if (pt->balance) {
-        const int rc = get_partition(pt, gx * xy::kWarps, &a.part);
+        const int rc = get_partition(pt, sg.gx * sg.warps, &a.part);
         if (rc != XY_OK) return rc;
     }
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(gx, s1 - s0, pt->col_blocks);
-    cfg.blockDim = dim3(xy::kBlock);
-    cfg.dynamicSmemBytes = 0;
+    cfg.gridDim = dim3(sg.gx, s1 - s0, pt->col_blocks);
+    cfg.blockDim = dim3(sg.warps * 32);
+    cfg.dynamicSmemBytes = xy::sweep_smem(sg.warps);
     cfg.stream = pt->stream;
     cudaLaunchAttribute attr[2];
     int na = l2_window_attr(pt, s0, s1, &attr[0]);
@@ -255,7 +267,7 @@ int launch_phase(xy_pt *pt, int mode, int colour, int s0, int s1, bool use_count
     }
     cfg.attrs = attr; cfg.numAttrs = na;
     void *params[] = {&a};
-    XY_CUDA(cudaLaunchKernelExC(&cfg, pt->phase_fn[mode], params));
+    XY_CUDA(cudaLaunchKernelExC(&cfg, pt->phase_fn[sg.big][mode], params));
     pt->launches += 1;
     return XY_OK;
 }
@@ -404,7 +416,8 @@ int prepare_partitions(xy_pt *pt, int group) {
             const int nmax = c == g->q_max ? g->N : max_class_size(g, c, s0, s1);
             if (nmax == 0) continue;
             const int32_t *unused = nullptr;
-            const int rc = get_partition(pt, sweep_grid_x(pt, s1 - s0, nmax) * xy::kWarps, &unused);
+            const SweepGrid sg = sweep_grid(pt, s1 - s0, nmax);
+            const int rc = get_partition(pt, sg.gx * sg.warps, &unused);
             if (rc != XY_OK) return rc;
         }
     }
@@ -620,21 +633,33 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
     pt->measure_chunk = std::max(256, ((N + 127) / 128 + 7) / 8 * 8);   // legacy measure partition: a function of N only
     if (pt->fast_G) {
         for (int m = 0; m < 4; ++m) {
-            pt->phase_fn[m] = phase_function(pt->fast_G, pt->col_blocks == 1, m);
-            cudaFuncSetAttribute(pt->phase_fn[m], cudaFuncAttributePreferredSharedMemoryCarveout,
-                                 static_cast<int>(cudaSharedmemCarveoutMaxShared));
+            pt->phase_fn[0][m] = phase_function<xy::kWarpsSmall>(pt->fast_G, pt->col_blocks == 1, m);
+            pt->phase_fn[1][m] = phase_function<xy::kWarpsBig>(pt->fast_G, pt->col_blocks == 1, m);
+            for (int b = 0; b < 2; ++b) {
+                cudaFuncSetAttribute(pt->phase_fn[b][m], cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     static_cast<int>(xy::sweep_smem(b ? xy::kWarpsBig : xy::kWarpsSmall)));
+                cudaFuncSetAttribute(pt->phase_fn[b][m], cudaFuncAttributePreferredSharedMemoryCarveout,
+                                     static_cast<int>(cudaSharedmemCarveoutMaxShared));
+            }
         }
         int per_sm = 0, n_sm = 0, dev = 0;
         cudaError_t eo = cudaGetDevice(&dev);
         if (eo == cudaSuccess) eo = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        // k_phase keeps kSweepMinBlocks CTAs x 45 KB of shared memory resident per SM (carve-out set above)
-        if (eo == cudaSuccess) eo = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pt->phase_fn[0], xy::kBlock, 0);
+        // 32 resident warps x 5.5 KB of shared memory per SM in either CTA shape (carve-out set above)
+        int per_sm_big = 0;
+        if (eo == cudaSuccess)
+            eo = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pt->phase_fn[0][0], xy::kWarpsSmall * 32,
+                                                               xy::sweep_smem(xy::kWarpsSmall));
+        if (eo == cudaSuccess)
+            eo = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_big, pt->phase_fn[1][0], xy::kWarpsBig * 32,
+                                                               xy::sweep_smem(xy::kWarpsBig));
         if (eo != cudaSuccess || per_sm < 1 || n_sm < 1) {
             if (pt->owns_stream) cudaStreamDestroy(pt->stream);
             delete pt;
             return fail(XY_ECUDA, std::string("k_phase occupancy query: ") + cudaGetErrorString(eo));
         }
         pt->sweep_capacity = per_sm * n_sm;
+        pt->capacity_big = std::max(1, per_sm_big) * n_sm;
         int max_persist = 0, max_window = 0;
         if (cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev) == cudaSuccess &&
             cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, dev) == cudaSuccess && max_persist > 0 &&
@@ -813,9 +838,10 @@ int xy_set_schedule(xy_pt *pt, int samples_per_group) {
     return XY_OK;
 }
 
-int xy_set_tuning(xy_pt *pt, int balance, int pdl, int l2_persist, int fuse_measure) {
-    if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+int xy_set_tuning(xy_pt *pt, int balance, int pdl, int l2_persist, int fuse_measure, int cta_shape) {
+    if (!check_pt(pt) || cta_shape < 0 || cta_shape > 2) return fail(XY_EINVAL, "bad handle or cta_shape not in {0, 1, 2}");
     XY_CUDA(cudaStreamSynchronize(pt->stream));
+    pt->cta_shape = cta_shape;
     pt->balance = balance ? 1 : 0; pt->pdl = pdl ? 1 : 0; pt->l2_persist = l2_persist ? 1 : 0;
     pt->fuse_measure = fuse_measure ? 1 : 0;
     drop_graphs(pt);

@@ -28,10 +28,12 @@ namespace xy {
 constexpr int kDB = 8;            // pipelined gathers per site
 constexpr int kDepth = 2;         // ring slots per warp (rows in flight)
 constexpr int kStageCap = 256;    // staged neighbour ids per warp and chunk (ints)
-#ifndef XY_SWEEP_MIN_BLOCKS
-#define XY_SWEEP_MIN_BLOCKS 4
-#endif
-constexpr int kSweepMinBlocks = XY_SWEEP_MIN_BLOCKS;   // resident CTAs per SM the register / shared budget is sized for
+// k_phase comes in two CTA shapes with the same 32 resident warps per SM (64 registers): W = 32 warps (one CTA per SM)
+// for large colour classes, W = 8 (four CTAs per SM) for small ones.  Measured: the SM's warp scheduler
+// favours older CTAs, so four co-resident CTAs finish 2-3 us apart and the SM idles in the tail; the warps of ONE CTA
+// progress evenly (+8 % on config 4).  Small classes prefer the finer CTA granularity.
+constexpr int kWarpsBig = 32, kWarpsSmall = 8;
+constexpr int kSmPerWarpSlots = 32;                    // resident warps per SM the register / shared budget is sized for
 
 // fixed-point scales of the measure reduction (exact, order-independent integer sums; see quant8 / quant1)
 constexpr double kInvScaleE = 1.0 / 524288.0;      // 2^-19
@@ -42,8 +44,9 @@ struct __align__(16) SweepWarp {
     float2 ring[kDepth][kDB + 1][32];
     uint32_t idx[kStageCap];
 };
-static_assert(sizeof(SweepWarp) * kWarps <= 48 * 1024 - 64, "static shared memory limit");
-static_assert(sizeof(SweepWarp) * kWarps >= sizeof(long long) * kWarps * 32 * 6, "measure reduction reuses the ring");
+constexpr size_t sweep_smem(int warps) { return sizeof(SweepWarp) * warps; }     // dynamic shared memory of a k_phase CTA
+static_assert(sweep_smem(kSmPerWarpSlots) <= 227 * 1024 - 4 * 1024, "shared memory per SM");
+static_assert(sizeof(SweepWarp) >= sizeof(long long) * 32 * 6, "measure reduction reuses the ring");
 
 // ---- packed fp32x2 helpers (IEEE rn per component: bit-identical to the scalar operations) ----------
 __device__ __forceinline__ float2 add2(const float2 a, const float2 b) {
@@ -211,7 +214,7 @@ __device__ __forceinline__ void sweep_consume(ACC &acc, const float2 *row0, int 
 struct SweepArgs {
     TileArgs t;
     const int32_t *part;           // [S][q_stride][nw + 1] cost-balanced first site of every warp's share (colour q_max =
-                                   // the measure pass over all sites), nw = gridDim.x * kWarps; nullptr = equal shares
+                                   // the measure pass over all sites), nw = warps per sample and column block; nullptr = equal shares
 };
 
 // per-thread constants of a launch
@@ -250,14 +253,14 @@ __device__ __forceinline__ void chunk_stage(const int32_t *gidx, uint32_t *sidx,
     }
 }
 
-template <int G, int CB>
+template <int G, int CB, int W>
 __device__ __forceinline__ PhasePrep sweep_prep(const SweepArgs &sa, const SweepCtx &x, int mode, int colour) {
     constexpr int SPW = 32 / G;
     const TileArgs &a = sa.t;
     const uint32_t R2 = CB ? static_cast<uint32_t>(G) : static_cast<uint32_t>(a.R >> 1);
     PhasePrep P;
     P.rc = make_int2(0, 0);
-    const int nw = gridDim.x * kWarps, gw = blockIdx.x * kWarps + x.warp;
+    const int nw = gridDim.x * W, gw = blockIdx.x * W + x.warp;
     const int cidx = mode == kModeMeasure ? a.q_stride - 1 : colour;
     if (sa.part) {      // cost-balanced shares (host-computed: cost = const + degree)
         const int32_t *pp = sa.part + (static_cast<size_t>(x.s) * a.q_stride + cidx) * (nw + 1) + gw;
@@ -560,9 +563,10 @@ __device__ __forceinline__ unsigned long long trace_now() {
 }
 #endif
 
-template <int G, int CB, int MODE>
-__global__ void __launch_bounds__(kBlock, kSweepMinBlocks) k_phase(const SweepArgs a) {
-    __shared__ SweepWarp s_w[kWarps];
+template <int G, int CB, int MODE, int W>
+__global__ void __launch_bounds__(W * 32, kSmPerWarpSlots / W) k_phase(const SweepArgs a) {
+    extern __shared__ __align__(16) unsigned char s_raw[];
+    SweepWarp *s_w = reinterpret_cast<SweepWarp *>(s_raw);
     __shared__ int s_last;
     constexpr int SPW = 32 / G;
 #ifdef XY_TRACE
@@ -584,7 +588,7 @@ __global__ void __launch_bounds__(kBlock, kSweepMinBlocks) k_phase(const SweepAr
     x.ring_s = static_cast<uint32_t>(__cvta_generic_to_shared(x.ring_l));
 
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    const PhasePrep P = sweep_prep<G, CB>(a, x, MODE == kModeOrMeasure ? kModeOverrelax : MODE, a.t.colour);
+    const PhasePrep P = sweep_prep<G, CB, W>(a, x, MODE == kModeOrMeasure ? kModeOverrelax : MODE, a.t.colour);
     __syncwarp();
     asm volatile("griddepcontrol.wait;" ::: "memory");      // the predecessor's theta / beta_slot / fx are final
 
@@ -595,8 +599,8 @@ __global__ void __launch_bounds__(kBlock, kSweepMinBlocks) k_phase(const SweepAr
 #endif
     sweep_phase<G, CB, MODE>(a.t, x, P, sweep, iacc);
 #ifdef XY_TRACE
-    if (x.lane == 0 && blockIdx.y == 0 && blockIdx.z == 0 && blockIdx.x * kWarps + x.warp < 8192) {
-        unsigned long long *o = g_trace[blockIdx.x * kWarps + x.warp];
+    if (x.lane == 0 && blockIdx.y == 0 && blockIdx.z == 0 && blockIdx.x * W + x.warp < 8192) {
+        unsigned long long *o = g_trace[blockIdx.x * W + x.warp];
         unsigned smid;
         asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
         o[0] = tr0; o[1] = tr1; o[2] = trace_now(); o[3] = (static_cast<unsigned long long>(smid) << 32) | static_cast<unsigned>(P.w1 - P.i0);
@@ -612,7 +616,7 @@ __global__ void __launch_bounds__(kBlock, kSweepMinBlocks) k_phase(const SweepAr
         if (threadIdx.x < G * 6) {
             const int ll = threadIdx.x / 6, c = threadIdx.x % 6;
             long long v = 0;
-            for (int wi = 0; wi < kWarps; ++wi)
+            for (int wi = 0; wi < W; ++wi)
                 for (int sb = 0; sb < SPW; ++sb) v += s_red[(wi * 32 + sb * G + ll) * 6 + c];
             const int slot = 2 * (blockIdx.z * G + ll) + c / 3;
             atomicAdd(reinterpret_cast<unsigned long long *>(a.t.fx) + (static_cast<size_t>(x.s) * a.t.R + slot) * 3 + c % 3,

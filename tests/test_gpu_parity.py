@@ -183,12 +183,15 @@ def test_run_equals_stepwise_calls_and_schedule_invariance():
     assert a.read_accumulators()[..., 0].min() == 6 + (21 // 2 - 6)
     assert a.launch_count() > 0
     # tuning switches (equal shares, no programmatic dependent launch, no L2 window, separate measure launches): same bits
-    d = U.ensemble_from_levy(g, T, SEED)
-    d.set_tuning(balance=0, pdl=0, l2_persist=0, fuse_measure=0)
-    d.run(n_cycles, sps, orps, me); d.run(3, 3, 1, 2)
-    assert np.array_equal(a.get_theta(), d.get_theta()) and np.array_equal(a.read_accumulators(), d.read_accumulators())
-    assert np.array_equal(a.get_labels(), d.get_labels())
-    for e in (a, b, c, d): e.close()
+    # and both CTA shapes (8-warp / 32-warp CTAs)
+    for kw in (dict(balance=0, pdl=0, l2_persist=0, fuse_measure=0, cta_shape=1), dict(cta_shape=2), dict(cta_shape=1)):
+        d = U.ensemble_from_levy(g, T, SEED)
+        d.set_tuning(**kw)
+        d.run(n_cycles, sps, orps, me); d.run(3, 3, 1, 2)
+        assert np.array_equal(a.get_theta(), d.get_theta()) and np.array_equal(a.read_accumulators(), d.read_accumulators()), kw
+        assert np.array_equal(a.get_labels(), d.get_labels())
+        d.close()
+    for e in (a, b, c): e.close()
 
 
 def test_run_matches_oracle_protocol_short():
