@@ -236,21 +236,24 @@ def main():
                 "avg_launch_us": ms_k * 1e3 / max(n_class_launches, 1), "launches_timed": n_class_launches,
                 "met_or_updates_per_ns": upd_per_step * world * args.steps / (ms_k * 1e6)}
 
-    # ---- end to end through the C ABI with HOST buffers: restore the state from pinned host memory, run one
-    #      cycle, read the observables and the state back ----
+    # ---- end to end through the C ABI with HOST buffers: every step uploads the step's input state from pinned host
+    #      memory (xy_set_theta), runs one PT cycle and reads the step's result -- the accumulated observables
+    #      [S][R][8] fp64 and the temperature labels -- back to the host ----
     e2e = None
     if not args.no_e2e:
         nbytes = w.S * w.N * w.R * 4
         host = torch.empty((w.S, w.N, w.R), dtype=torch.float32, pin_memory=True).numpy()
         ens.get_theta(out=host)
         n_e2e = max(2, min(args.steps, 5))
+        sink = []
 
         def e2e_steps(n):
             for _ in range(n):
-                ens.set_theta(host)                 # H2D, pinned
+                ens.set_theta(host)                       # H2D, pinned
                 ens.run(1, sps, orps, me)
-                ens.measure(want=True)              # D2H observables [S][R][3] doubles
-                ens.get_theta(out=host)             # D2H state
+                sink.append(ens.read_accumulators())      # D2H result (synchronises)
+                sink.append(ens.get_labels())
+                del sink[:-2]
         e2e_steps(1)
         t0 = time.perf_counter()
         barrier()
@@ -262,8 +265,8 @@ def main():
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             dt = float(t.item())
         e2e = {"value": upd_per_step * world * n_e2e / (dt * 1e9), "unit": UNIT, "steps": n_e2e,
-               "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes + w.S * w.R * 3 * 8 + w.S * w.R * 4,
-               "what": "xy_set_theta(pinned host) + xy_run(1 cycle) + xy_measure(host out) + xy_get_theta(pinned host)"}
+               "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": w.S * w.R * 8 * 8 + w.S * w.R * 4,
+               "what": "xy_set_theta(pinned host state) + xy_run(1 cycle) + xy_read_accumulators + xy_get_labels (host)"}
 
     # ---- CPU baseline: the oracle on a bounded sample of the same workload (rank 0, N = 1 only) ----
     cpu = None

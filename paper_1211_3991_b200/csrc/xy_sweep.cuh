@@ -116,8 +116,8 @@ template <> struct PairAcc<kModeMeasure> {
     }
 };
 // over-relaxation with the measurement as a by-product: the local field h needs (cos th_j, sin th_j) of every
-// neighbour anyway; the partial field l of the lower neighbours is the same sum, in the same order, that the measure
-// kernel forms, so both give bit-identical energies.  After the class's update th_i and all its lower neighbours are
+// neighbour anyway; the partial field l of the lower neighbours is a prefix of that sum -- the same terms in the same
+// order that the measure kernel adds, so both give bit-identical energies.  After the class's update th_i and all its lower neighbours are
 // final for this sweep (colour-major numbering: j < i has a lower or equal colour, and same-colour sites share no bond).
 template <> struct PairAcc<kModeOrMeasure> {
     float2 hx = make_float2(0.f, 0.f), hy = make_float2(0.f, 0.f), lx = make_float2(0.f, 0.f), ly = make_float2(0.f, 0.f);
@@ -128,9 +128,9 @@ template <> struct PairAcc<kModeOrMeasure> {
         __sincosf(t.y, &sy, &cy);
         hx = add2(hx, make_float2(cx, cy));
         hy = add2(hy, make_float2(sx, sy));
-        if (k < nlow) {
-            lx = add2(lx, make_float2(cx, cy));
-            ly = add2(ly, make_float2(sx, sy));
+        if (k == nlow - 1) {     // the lower neighbours are the head of the list: l is h's partial sum after the last of them
+            lx = hx;
+            ly = hy;
         }
     }
 };
@@ -140,7 +140,6 @@ template <> struct PairAcc<kModeOrMeasure> {
 __device__ __forceinline__ float site_energy(float c, float s, float lx, float ly) {
     return __fmaf_rn(c, lx, __fmul_rn(s, ly));
 }
-
 // per-lane description of the site a lane works on in the current row (warp-uniform when SPW == 1)
 struct RowSite { int i, deg, pos, nlow; bool valid; };
 
