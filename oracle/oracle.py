@@ -66,6 +66,10 @@ def lib():
         L.orc_pt_swap.argtypes = [C.c_int, _f64p, _f64p, _i32p, _i32p, C.c_uint64, C.c_uint32,
                                   C.c_uint32, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_pt_swap.restype = None
+        L.orc_fourier.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, _i32p, _i32p, _f32p, _f64p, _f64p]
+        L.orc_fourier.restype = None
+        L.orc_xi2.argtypes = [C.c_double, C.c_double, C.c_int, C.c_double]
+        L.orc_xi2.restype = C.c_double
         L.orc_run.argtypes = [C.c_int, C.c_int, C.c_int, _i32p, _i32p, _i32p, _f32p, _f64p, _i32p,
                               _i32p, C.c_uint64, C.c_uint32, C.POINTER(C.c_uint32),
                               C.POINTER(C.c_uint32), C.c_int, C.c_int, C.c_int, C.c_int, _f64p,
@@ -196,6 +200,18 @@ def measure(row_ptr, col_idx, theta):
     E = np.zeros(R); Mx = np.zeros(R); My = np.zeros(R)
     lib().orc_measure(N, R, row_ptr, _ci(col_idx), theta, E, Mx, My)
     return E, Mx, My
+
+
+def fourier(Lx, Ly, x, y, theta):
+    """G1, G2 [R]: |sum_i S_i exp(i k r_i)|^2 / N at k = (2 pi/Lx, 0) and (0, 2 pi/Ly)."""
+    N, R = theta.shape
+    G1 = np.zeros(R); G2 = np.zeros(R)
+    lib().orc_fourier(N, R, Lx, Ly, np.ascontiguousarray(x, np.int32), np.ascontiguousarray(y, np.int32), theta, G1, G2)
+    return G1, G2
+
+
+def xi2(chi0, chik, L, psi=2.0):
+    return float(lib().orc_xi2(float(chi0), float(chik), int(L), float(psi)))
 
 
 def accumulate(N, E, Mx, My, temp_of_slot, acc):

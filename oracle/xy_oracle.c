@@ -372,6 +372,35 @@ void orc_accumulate(int N, int R, const double *E, const double *Mx, const doubl
 }
 
 /* ------------------------------------------------------------------------------------------
+ * a7. Structure factor at k_min and second-moment correlation length.
+ * Eq. 18: C(r) = (1/N) sum_i <S_i . S_{i+r}>; its Fourier transform at momentum k is
+ *   chi(k) = (1/N) < |sum_i S_i exp(i k . r_i)|^2 >,  the modulus taken per spin component and added.
+ * k_min = (2 pi / L, 0) and (0, 2 pi / L).  chi(0) = N <m^2>.
+ * ---------------------------------------------------------------------------------------- */
+void orc_fourier(int N, int R, int Lx, int Ly, const int32_t *x, const int32_t *y, const float *theta,
+                 double *G1, double *G2) {
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int r = 0; r < R; ++r) {
+        double cre1 = 0, cim1 = 0, sre1 = 0, sim1 = 0, cre2 = 0, cim2 = 0, sre2 = 0, sim2 = 0;
+        for (int i = 0; i < N; ++i) {
+            const double t = (double)theta[(size_t)i * R + r];
+            const double c = cos(t), s = sin(t);
+            const double p1 = two_pi * (double)x[i] / (double)Lx, p2 = two_pi * (double)y[i] / (double)Ly;
+            cre1 += c * cos(p1); cim1 += c * sin(p1); sre1 += s * cos(p1); sim1 += s * sin(p1);
+            cre2 += c * cos(p2); cim2 += c * sin(p2); sre2 += s * cos(p2); sim2 += s * sin(p2);
+        }
+        G1[r] = (cre1 * cre1 + cim1 * cim1 + sre1 * sre1 + sim1 * sim1) / (double)N;
+        G2[r] = (cre2 * cre2 + cim2 * cim2 + sre2 * sre2 + sim2 * sim2) / (double)N;
+    }
+}
+
+/* Eq. 17: psi = rho - d in the long-range regime, 2 in the short-range regime. */
+double orc_xi2(double chi0, double chik, int L, double psi) {
+    const double pi = 3.1415926535897932384626433832795;
+    return pow(chi0 / chik - 1.0, 1.0 / psi) / (2.0 * sin(pi / (double)L));
+}
+
+/* ------------------------------------------------------------------------------------------
  * a5. Parallel tempering (ref 65).  DESIGN R9: round k attempts the pairs
  * (t, t+1) with t = k mod 2, k mod 2 + 2, ...;  a = slot_of_temp[t], b = slot_of_temp[t+1];
  *   accept iff u < exp((beta_t - beta_{t+1}) (E_a - E_b)),   beta = 1/T in fp64;

@@ -88,6 +88,15 @@ void orc_measure(int N, int R, const int32_t *row_ptr, const int32_t *col_idx,
 void orc_accumulate(int N, int R, const double *E, const double *Mx, const double *My,
                     const int32_t *temp_of_slot, double *acc /*[R][ORC_NACC]*/);
 
+/* ---- a7: structure factor at the smallest momenta and the second-moment correlation
+ *      length (Eq. 17-18) ----
+ * G1[r] = |sum_i S_i exp(i 2 pi x_i / Lx)|^2 / N, G2[r] likewise with y_i / Ly, S_i = (cos th_i, sin th_i): the
+ * single-configuration estimators of chi(k_min) for k_min = (2 pi / L, 0) and (0, 2 pi / L); chi(0) = N m^2. */
+void orc_fourier(int N, int R, int Lx, int Ly, const int32_t *x /*[N]*/, const int32_t *y /*[N]*/,
+                 const float *theta /*[N][R]*/, double *G1 /*[R]*/, double *G2 /*[R]*/);
+/* Eq. 17: xi_2 = [chi(0)/chi(k_min) - 1]^(1/psi) / (2 sin(pi / L)) */
+double orc_xi2(double chi0, double chik, int L, double psi);
+
 /* ---- a5: one parallel-tempering swap round (App. B.b, ref 65; DESIGN R9) ----
  * decisions_in NULL: draw u from Philox(SWAP) and decide; else use decisions_in[t] for pair (t,t+1).
  * decisions_out[t], margin_out[t] (may be NULL) are written for every attempted pair. */

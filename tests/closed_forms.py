@@ -35,6 +35,17 @@ def ring(N, beta, nmax=60):
     return float(e), float(np.sum(C) / N)
 
 
+def ring_structure_factor(N, beta, k_index=1, nmax=60):
+    """chi(k) = sum_r C(r) cos(2 pi k_index r / N) of the periodic ring, C(r) = <cos(theta_0 - theta_r)>
+    = sum_n I_n^(N-r) I_(n+1)^r / sum_n I_n^N (transfer matrix in the angular-momentum basis)."""
+    n = np.arange(-nmax, nmax + 1)
+    In = iv(n, beta)
+    Inp1 = iv(n + 1, beta)
+    Z = np.sum(In ** N)
+    C = np.array([np.sum(In ** (N - r) * Inp1 ** r) / Z for r in range(N)])
+    return float(np.sum(C * np.cos(2.0 * np.pi * k_index * np.arange(N) / N)))
+
+
 def chain(N, beta):
     """energy per site and <m^2> of the open chain of N sites."""
     t = iv(1, beta) / iv(0, beta)
