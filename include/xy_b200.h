@@ -66,6 +66,10 @@ int xy_graph_free(xy_graph *g);
 /* any output pointer may be NULL */
 int xy_graph_info(const xy_graph *g, int *S, int *N, int64_t *nnz_total, int *q_max, int *max_degree);
 
+/* Lattice coordinates of the sites (needed only by xy_measure_fourier): x, y [S][N] host, 0 <= x < Lx, 0 <= y < Ly,
+ * Lx, Ly <= 65535.  For a Levy graph built by xy_levy_build: x = new_to_old % L, y = new_to_old / L.  Synchronous. */
+int xy_graph_set_coords(xy_graph *g, int Lx, int Ly, const int32_t *x /*host*/, const int32_t *y /*host*/);
+
 /* ---- PT ensemble ----
  * T [R] host, strictly positive, ascending (T = +inf allowed: beta = 0).  width [R] host or NULL;
  * NULL selects the BASELINE.json proposal width 2 pi min(1, T/2).  beta and width are rounded to fp32
@@ -90,6 +94,16 @@ int xy_pt_swap(xy_pt *pt);
  * current temperature (Eq. 13-15).  out_host: [S][R][3] doubles (E, Mx, My) indexed by TEMPERATURE,
  * or NULL; a non-NULL out_host synchronises the stream. */
 int xy_measure(xy_pt *pt, double *out_host);
+
+/* Structure factor at the smallest momenta (Eq. 17-18): for every replica
+ * G1 = |sum_i S_i exp(i 2 pi x_i / Lx)|^2 / N and G2 likewise with y_i / Ly -- the single-configuration estimators of
+ * chi(k_min), k_min = (2 pi / L, 0) and (0, 2 pi / L); added to the fp64 accumulators (n, sum G1, sum G2) of the
+ * replica's current temperature (xy_read_fourier_accumulators; cleared by xy_reset_accumulators).  chi(0) = N <m^2>
+ * comes from the ordinary accumulators, xi_2 = [chi(0)/chi(k_min) - 1]^(1/psi) / (2 sin(pi / L)).
+ * out_host: [S][R][2] doubles (G1, G2) indexed by TEMPERATURE, or NULL; non-NULL synchronises the stream.
+ * XY_ESTATE unless xy_graph_set_coords has been called. */
+int xy_measure_fourier(xy_pt *pt, double *out_host);
+int xy_read_fourier_accumulators(xy_pt *pt, double *acc_host /*[S][R][3]: n, sum G1, sum G2 by temperature*/);
 
 /* n_cycles PT cycles in the order stated at the top, replayed from a captured CUDA graph (SURVEY.md
  * 8(a) row a6).  measure_every = 0 disables measurements (energies are still computed for the swap).

@@ -22,6 +22,9 @@ SYMBOLS = {
     "xy_abi_version": (C.c_int, []),
     "xy_graph_load": (C.c_int, [C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p)]),
     "xy_graph_free": (C.c_int, [C.c_void_p]),
+    "xy_graph_set_coords": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]),
+    "xy_measure_fourier": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "xy_read_fourier_accumulators": (C.c_int, [C.c_void_p, C.c_void_p]),
     "xy_graph_info": (C.c_int, [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int64),
                                 C.POINTER(C.c_int), C.POINTER(C.c_int)]),
     "xy_pt_create": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_void_p,
@@ -116,6 +119,28 @@ def xy_graph_info(g):
     nnz = C.c_int64()
     _check(lib().xy_graph_info(g, C.byref(S), C.byref(N), C.byref(nnz), C.byref(q), C.byref(d)))
     return dict(S=S.value, N=N.value, nnz_total=nnz.value, q_max=q.value, max_degree=d.value)
+
+
+def xy_graph_set_coords(g, Lx, Ly, x, y):
+    x, xp = _host(x, np.int32)
+    y, yp = _host(y, np.int32)
+    _check(lib().xy_graph_set_coords(g, Lx, Ly, xp, yp))
+
+
+def xy_measure_fourier(pt, shape=None):
+    """shape = (S, R) to get (G1, G2) of this configuration back as a host array [S][R][2] by temperature."""
+    if shape is None:
+        _check(lib().xy_measure_fourier(pt, None))
+        return None
+    out = np.zeros((*shape, 2), np.float64)
+    _check(lib().xy_measure_fourier(pt, out.ctypes.data_as(C.c_void_p)))
+    return out
+
+
+def xy_read_fourier_accumulators(pt, shape):
+    out = np.empty((*shape, 3), np.float64)
+    _check(lib().xy_read_fourier_accumulators(pt, out.ctypes.data_as(C.c_void_p)))
+    return out
 
 
 def xy_pt_create(g, T, seed, width=None, sample_base=0, theta_dev=None, stream=None):
@@ -291,6 +316,9 @@ class Ensemble:
     def overrelax(self, n=1): xy_overrelax(self.pt, n)
     def pt_swap(self): xy_pt_swap(self.pt)
     def measure(self, want=False): return xy_measure(self.pt, (self.S, self.R) if want else None)
+    def set_coords(self, Lx, Ly, x, y): xy_graph_set_coords(self.graph, Lx, Ly, x, y)
+    def measure_fourier(self, want=False): return xy_measure_fourier(self.pt, (self.S, self.R) if want else None)
+    def read_fourier_accumulators(self): return xy_read_fourier_accumulators(self.pt, (self.S, self.R))
     def run(self, n_cycles, sweeps_per_swap=10, or_per_sweep=1, measure_every=1):
         xy_run(self.pt, n_cycles, sweeps_per_swap, or_per_sweep, measure_every)
     def run_sweeps(self, n_blocks, sweeps_per_block=10, or_per_sweep=1):

@@ -74,6 +74,9 @@ struct xy_graph {
     std::vector<int32_t> h_class_ptr;  // [S][q_stride]
     std::vector<uint32_t> h_deg;       // [S][N] degree | n_lower << 16 (host copy of rec.y, for the share tables)
     size_t bytes_per_sample = 0;       // rec + col_idx (average), for the schedule heuristic
+    int Lx = 0, Ly = 0;                // lattice extents of the site coordinates (0 = none set)
+    uint32_t *coords = nullptr;        // [S][N] x | y << 16
+    float2 *tab1 = nullptr, *tab2 = nullptr;   // [Lx], [Ly]: (cos, sin)(2 pi n / L)
     cudaStream_t stream = nullptr;
 };
 
@@ -102,6 +105,8 @@ struct xy_pt {
     int32_t *temp_of_slot = nullptr, *slot_of_temp = nullptr;
     uint32_t *counters = nullptr;
     double *E_slot = nullptr, *M_slot = nullptr, *acc = nullptr;
+    double *G_slot = nullptr, *acc_k = nullptr;   // structure factor at k_min: [S][R][2] per slot, [S][R][3] by temperature
+    long long *fk = nullptr;                      // [S][R][8] fixed-point sums of k_fourier
     long long *fx = nullptr;            // [S][R][3] fixed-point measure sums (zero between launches)
     unsigned int *ticket = nullptr;     // [S]
     long long *attempts = nullptr, *accepts = nullptr;
@@ -574,7 +579,38 @@ int xy_graph_load(int S, int N, const int32_t *row_ptr, const int32_t *col_idx, 
 int xy_graph_free(xy_graph *g) {
     if (!g) return XY_OK;
     cudaFree(g->rec); cudaFree(g->col_idx); cudaFree(g->class_ptr);
+    cudaFree(g->coords); cudaFree(g->tab1); cudaFree(g->tab2);
     delete g;
+    return XY_OK;
+}
+
+int xy_graph_set_coords(xy_graph *g, int Lx, int Ly, const int32_t *x, const int32_t *y) {
+    if (!g || !x || !y) return fail(XY_EINVAL, "graph or coordinate array is NULL");
+    if (Lx < 1 || Ly < 1 || Lx > 65535 || Ly > 65535) return fail(XY_EINVAL, "need 1 <= Lx, Ly <= 65535");
+    const size_t n = static_cast<size_t>(g->S) * g->N;
+    try {
+        std::vector<uint32_t> h(n);
+        for (size_t i = 0; i < n; ++i) {
+            if (x[i] < 0 || x[i] >= Lx || y[i] < 0 || y[i] >= Ly) return fail(XY_EINVAL, "site coordinate out of range");
+            h[i] = static_cast<uint32_t>(x[i]) | (static_cast<uint32_t>(y[i]) << 16);
+        }
+        std::vector<float2> t1(Lx), t2(Ly);
+        const double two_pi = 6.283185307179586476925286766559;
+        for (int k = 0; k < Lx; ++k) t1[k] = make_float2(static_cast<float>(std::cos(two_pi * k / Lx)), static_cast<float>(std::sin(two_pi * k / Lx)));
+        for (int k = 0; k < Ly; ++k) t2[k] = make_float2(static_cast<float>(std::cos(two_pi * k / Ly)), static_cast<float>(std::sin(two_pi * k / Ly)));
+        cudaFree(g->coords); cudaFree(g->tab1); cudaFree(g->tab2);
+        g->coords = nullptr; g->tab1 = g->tab2 = nullptr; g->Lx = g->Ly = 0;
+        int rc;
+        if ((rc = dev_alloc(&g->coords, n)) != XY_OK || (rc = dev_alloc(&g->tab1, Lx)) != XY_OK ||
+            (rc = dev_alloc(&g->tab2, Ly)) != XY_OK)
+            return rc;
+        XY_CUDA(cudaMemcpy(g->coords, h.data(), n * sizeof(uint32_t), cudaMemcpyHostToDevice));
+        XY_CUDA(cudaMemcpy(g->tab1, t1.data(), Lx * sizeof(float2), cudaMemcpyHostToDevice));
+        XY_CUDA(cudaMemcpy(g->tab2, t2.data(), Ly * sizeof(float2), cudaMemcpyHostToDevice));
+        g->Lx = Lx; g->Ly = Ly;
+    } catch (const std::bad_alloc &) {
+        return fail(XY_ENOMEM, "host allocation failed");
+    }
     return XY_OK;
 }
 
@@ -682,6 +718,7 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
     A(dev_alloc(&pt->E_slot, SR)); A(dev_alloc(&pt->M_slot, SR * 2));
     A(dev_alloc(&pt->fx, SR * 3)); A(dev_alloc(&pt->ticket, S)); A(dev_alloc(&pt->acc, SR * XY_NACC));
     A(dev_alloc(&pt->attempts, SR)); A(dev_alloc(&pt->accepts, SR)); A(dev_alloc(&pt->decisions, SR));
+    A(dev_alloc(&pt->G_slot, SR * 2)); A(dev_alloc(&pt->acc_k, SR * 3)); A(dev_alloc(&pt->fk, SR * 8));
 
     if (rc != XY_OK) { xy_pt_destroy(pt); return rc; }
     std::vector<float> hb(R), hw(R);
@@ -704,6 +741,9 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
     if (e == cudaSuccess) e = cudaMemsetAsync(pt->accepts, 0, SR * sizeof(long long), pt->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(pt->E_slot, 0, SR * sizeof(double), pt->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(pt->fx, 0, SR * 3 * sizeof(long long), pt->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(pt->fk, 0, SR * 8 * sizeof(long long), pt->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(pt->acc_k, 0, SR * 3 * sizeof(double), pt->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(pt->G_slot, 0, SR * 2 * sizeof(double), pt->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(pt->ticket, 0, S * sizeof(unsigned int), pt->stream);
     if (e == cudaSuccess) {
         xy::k_refresh_slot_params<<<ceil_div(SR, 128), 128, 0, pt->stream>>>(pt->temp_of_slot, pt->slot_of_temp, pt->beta_f,
@@ -730,6 +770,7 @@ int xy_pt_destroy(xy_pt *pt) {
     cudaFree(pt->temp_of_slot); cudaFree(pt->slot_of_temp); cudaFree(pt->counters);
     cudaFree(pt->E_slot); cudaFree(pt->M_slot); cudaFree(pt->fx); cudaFree(pt->ticket); cudaFree(pt->acc);
     cudaFree(pt->attempts); cudaFree(pt->accepts); cudaFree(pt->decisions);
+    cudaFree(pt->G_slot); cudaFree(pt->acc_k); cudaFree(pt->fk);
     for (auto &kv : pt->parts) cudaFree(kv.second);
     if (pt->owns_stream) cudaStreamDestroy(pt->stream);
     delete pt;
@@ -829,6 +870,60 @@ int xy_measure(xy_pt *pt, double *out_host) {
             return fail(XY_ENOMEM, "host allocation failed");
         }
     }
+    return XY_OK;
+}
+
+int xy_measure_fourier(xy_pt *pt, double *out_host) {
+    if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    const xy_graph *g = pt->g;
+    if (!g->coords) return fail(XY_ESTATE, "xy_graph_set_coords has not been called");
+    const int S = g->S, R = pt->R;
+    xy::FourierArgs a;
+    a.theta = pt->theta; a.coords = g->coords; a.tab1 = g->tab1; a.tab2 = g->tab2;
+    a.fk = pt->fk; a.ticket = pt->ticket; a.temp_of_slot = pt->temp_of_slot;
+    a.G_slot = pt->G_slot; a.acc_k = pt->acc_k; a.N = g->N; a.R = R; a.s0 = 0;
+    // one wave of CTAs over all samples and column blocks, at least 32 sites per warp
+    const int cb = pt->fast_G ? pt->col_blocks : 1;
+    const int warps_per_sample = std::max(1, std::min(ceil_div(g->N, 32), std::max(1, 148 * 8 * xy::kWarps / (S * cb))));   // two waves of 4 CTAs per SM (one wave measured slower)
+    a.sites_per_warp = ceil_div(g->N, warps_per_sample);
+    const dim3 grid(ceil_div(ceil_div(g->N, a.sites_per_warp), xy::kWarps), S, cb);
+    switch (pt->fast_G) {
+        case 32: xy::k_fourier2<32><<<grid, xy::kBlock, 0, pt->stream>>>(a); break;
+        case 16: xy::k_fourier2<16><<<grid, xy::kBlock, 0, pt->stream>>>(a); break;
+        case 8: xy::k_fourier2<8><<<grid, xy::kBlock, 0, pt->stream>>>(a); break;
+        case 4: xy::k_fourier2<4><<<grid, xy::kBlock, 0, pt->stream>>>(a); break;
+        case 2: xy::k_fourier2<2><<<grid, xy::kBlock, 0, pt->stream>>>(a); break;
+        case 1: xy::k_fourier2<1><<<grid, xy::kBlock, 0, pt->stream>>>(a); break;
+        default: xy::k_fourier<<<grid, xy::kBlock, 0, pt->stream>>>(a); break;      // any R
+    }
+    XY_CUDA(cudaGetLastError());
+    pt->launches += 1;
+    if (out_host) {
+        const size_t SR = static_cast<size_t>(S) * R;
+        try {
+            std::vector<double> G(SR * 2);
+            std::vector<int32_t> tos(SR);
+            XY_CUDA(cudaMemcpyAsync(G.data(), pt->G_slot, SR * 2 * sizeof(double), cudaMemcpyDeviceToHost, pt->stream));
+            XY_CUDA(cudaMemcpyAsync(tos.data(), pt->temp_of_slot, SR * sizeof(int32_t), cudaMemcpyDeviceToHost, pt->stream));
+            XY_CUDA(cudaStreamSynchronize(pt->stream));
+            for (int s = 0; s < S; ++s)
+                for (int r = 0; r < R; ++r) {
+                    const size_t i = static_cast<size_t>(s) * R + r;
+                    double *o = out_host + (static_cast<size_t>(s) * R + tos[i]) * 2;
+                    o[0] = G[2 * i]; o[1] = G[2 * i + 1];
+                }
+        } catch (const std::bad_alloc &) {
+            return fail(XY_ENOMEM, "host allocation failed");
+        }
+    }
+    return XY_OK;
+}
+
+int xy_read_fourier_accumulators(xy_pt *pt, double *acc_host) {
+    if (!check_pt(pt) || !acc_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
+    const size_t n = static_cast<size_t>(pt->g->S) * pt->R * 3;
+    XY_CUDA(cudaMemcpyAsync(acc_host, pt->acc_k, n * sizeof(double), cudaMemcpyDeviceToHost, pt->stream));
+    XY_CUDA(cudaStreamSynchronize(pt->stream));
     return XY_OK;
 }
 
@@ -968,6 +1063,7 @@ int xy_reset_accumulators(xy_pt *pt) {
     if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
     const size_t n = static_cast<size_t>(pt->g->S) * pt->R * XY_NACC;
     XY_CUDA(cudaMemsetAsync(pt->acc, 0, n * sizeof(double), pt->stream));
+    XY_CUDA(cudaMemsetAsync(pt->acc_k, 0, static_cast<size_t>(pt->g->S) * pt->R * 3 * sizeof(double), pt->stream));
     return XY_OK;
 }
 

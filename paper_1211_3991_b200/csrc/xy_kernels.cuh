@@ -247,6 +247,186 @@ __global__ void __launch_bounds__(kBlock) k_measure_generic(const TileArgs a, in
     }
 }
 
+// ---- structure factor at the smallest momenta (Eq. 17-18) ---------------
+// G1 = |sum_i S_i exp(i 2 pi x_i / Lx)|^2 / N, G2 likewise with y_i / Ly, per (sample, slot): the single-configuration
+// estimators of chi(k_min).  One streaming pass over theta (4 bytes per spin and slot, no gathers): a warp walks a
+// contiguous range of sites, lane = slot (blocks of 32 slots), eight sums per slot (Re/Im x two spin components x
+// two momenta) as exact fixed-point integers (scale 2^22, see quant of the measure kernel), so the result does not
+// depend on the grid.  The last CTA of a sample converts the sums and files G1, G2 under the slot's temperature.
+struct FourierArgs {
+    const float *theta;             // [S][N][R]
+    const uint32_t *coords;         // [S][N] x | y << 16
+    const float2 *tab1, *tab2;      // [Lx], [Ly]: (cos, sin)(2 pi n / L)
+    long long *fk;                  // [S][R][8] fixed-point sums, zero between launches
+    unsigned int *ticket;           // [S]
+    const int32_t *temp_of_slot;    // [S][R]
+    double *G_slot;                 // [S][R][2]
+    double *acc_k;                  // [S][R][3]: n, sum G1, sum G2 by temperature
+    int N, R, s0, sites_per_warp;
+};
+
+__device__ __forceinline__ int quant_unit(float x) { return __float_as_int(__fadd_rn(x, 3.0f)) - 0x40400000; }   // rn(x 2^22), |x| <= 1
+
+__global__ void __launch_bounds__(kBlock) k_fourier(const FourierArgs a) {
+    __shared__ int s_last;
+    const int s = a.s0 + blockIdx.y;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int i0 = (blockIdx.x * kWarps + warp) * a.sites_per_warp;
+    const int i1 = min(a.N, i0 + a.sites_per_warp);
+    const float *th = a.theta + static_cast<size_t>(s) * a.N * a.R;
+    const uint32_t *co = a.coords + static_cast<size_t>(s) * a.N;
+    for (int r = lane; r < a.R && i0 < i1; r += 32) {
+        long long acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        int part[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        int n_part = 0;
+        for (int i = i0; i < i1; ++i) {
+            const uint32_t xy = __ldg(co + i);
+            const float2 p1 = __ldg(a.tab1 + (xy & 0xffffu)), p2 = __ldg(a.tab2 + (xy >> 16));
+            float sn, cs;
+            __sincosf(th[static_cast<size_t>(i) * a.R + r], &sn, &cs);
+            part[0] += quant_unit(__fmul_rn(cs, p1.x)); part[1] += quant_unit(__fmul_rn(cs, p1.y));
+            part[2] += quant_unit(__fmul_rn(sn, p1.x)); part[3] += quant_unit(__fmul_rn(sn, p1.y));
+            part[4] += quant_unit(__fmul_rn(cs, p2.x)); part[5] += quant_unit(__fmul_rn(cs, p2.y));
+            part[6] += quant_unit(__fmul_rn(sn, p2.x)); part[7] += quant_unit(__fmul_rn(sn, p2.y));
+            if (++n_part == 256) {      // 256 * 2^22 < 2^31
+#pragma unroll
+                for (int c = 0; c < 8; ++c) { acc[c] += part[c]; part[c] = 0; }
+                n_part = 0;
+            }
+        }
+        unsigned long long *f = reinterpret_cast<unsigned long long *>(a.fk) + (static_cast<size_t>(s) * a.R + r) * 8;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) atomicAdd(f + c, static_cast<unsigned long long>(acc[c] + part[c]));
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(a.ticket + s, 1u) == gridDim.x - 1u) ? 1 : 0;
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+        const double inv = 1.0 / 4194304.0;
+        for (int r = threadIdx.x; r < a.R; r += blockDim.x) {
+            long long *f = a.fk + (static_cast<size_t>(s) * a.R + r) * 8;
+            double v[8];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) { v[c] = static_cast<double>(__ldcg(f + c)) * inv; f[c] = 0; }
+            const double g1 = (v[0] * v[0] + v[1] * v[1] + v[2] * v[2] + v[3] * v[3]) / a.N;
+            const double g2 = (v[4] * v[4] + v[5] * v[5] + v[6] * v[6] + v[7] * v[7]) / a.N;
+            const size_t sr = static_cast<size_t>(s) * a.R + r;
+            a.G_slot[2 * sr] = g1;
+            a.G_slot[2 * sr + 1] = g2;
+            double *o = a.acc_k + (static_cast<size_t>(s) * a.R + a.temp_of_slot[sr]) * 3;
+            o[0] += 1.0; o[1] += g1; o[2] += g2;
+        }
+        if (threadIdx.x == 0) a.ticket[s] = 0u;
+    }
+}
+
+// float2 flavour of k_fourier for R = 2G (G a power of two <= 32) or R a multiple of 64 (G = 32, blockIdx.z = block
+// of 64 slots): a lane owns two adjacent slots, G lanes cover a site, a warp reads 32/G sites per step (one fully used
+// 256-byte request at R >= 64), four steps of loads in flight.  Same fixed-point sums, same finalisation.
+template <int G>
+__global__ void __launch_bounds__(kBlock) k_fourier2(const FourierArgs a) {
+    constexpr int SPW = 32 / G;
+    __shared__ int s_last;
+    const int s = a.s0 + blockIdx.y;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int sub = lane / G, q = blockIdx.z * G + lane % G;           // slot pair of this lane
+    const int R2 = a.R >> 1;
+    const int i0 = (blockIdx.x * kWarps + warp) * a.sites_per_warp;
+    const int i1 = min(a.N, i0 + a.sites_per_warp);
+    const float2 *th = reinterpret_cast<const float2 *>(a.theta) + static_cast<size_t>(s) * a.N * R2 + q;
+    const uint32_t *co = a.coords + static_cast<size_t>(s) * a.N;
+    // fp32 partial sums over <= 256 sites of the lane's own range (fixed order: the partition is a function of N, S
+    // and R only, so a run is bit-reproducible), then exact fixed-point sums across flushes and warps
+    float part[16];
+#pragma unroll
+    for (int c = 0; c < 16; ++c) part[c] = 0.f;
+    int n_part = 0;
+    auto tally = [&](float t, const float2 p1, const float2 p2, int o) {
+        float sn, cs;
+        __sincosf(t, &sn, &cs);
+        part[o + 0] = fmaf(cs, p1.x, part[o + 0]); part[o + 1] = fmaf(cs, p1.y, part[o + 1]);
+        part[o + 2] = fmaf(sn, p1.x, part[o + 2]); part[o + 3] = fmaf(sn, p1.y, part[o + 3]);
+        part[o + 4] = fmaf(cs, p2.x, part[o + 4]); part[o + 5] = fmaf(cs, p2.y, part[o + 5]);
+        part[o + 6] = fmaf(sn, p2.x, part[o + 6]); part[o + 7] = fmaf(sn, p2.y, part[o + 7]);
+    };
+    auto flush = [&]() {      // rare (once per <= 256 sites and lane): no 64-bit accumulators live in the loop
+        unsigned long long *f = reinterpret_cast<unsigned long long *>(a.fk) + (static_cast<size_t>(s) * a.R + 2 * q) * 8;
+#pragma unroll
+        for (int c = 0; c < 16; ++c) {
+            atomicAdd(f + c, static_cast<unsigned long long>(__double2ll_rn(static_cast<double>(part[c]) * 4194304.0)));
+            part[c] = 0.f;
+        }
+    };
+    // software pipeline: the loads of batch k+1 (4 steps of theta + coordinates) fly while batch k is tallied
+    constexpr int UB = 4;
+    float2 t[UB], tn[UB];
+    uint32_t xy[UB], xyn[UB];
+    auto load = [&](int i, float2 (&tt)[UB], uint32_t (&cc)[UB]) {
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            const int iu = i + u * SPW;
+            tt[u] = make_float2(0.f, 0.f); cc[u] = 0u;
+            if (iu < i1) { tt[u] = __ldcs(th + static_cast<size_t>(iu) * R2); cc[u] = __ldg(co + iu); }
+        }
+    };
+    load(i0 + sub, t, xy);
+    for (int i = i0 + sub; i < i1; i += UB * SPW) {
+        load(i + UB * SPW, tn, xyn);
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            if (i + u * SPW < i1) {
+                const float2 p1 = __ldg(a.tab1 + (xy[u] & 0xffffu)), p2 = __ldg(a.tab2 + (xy[u] >> 16));
+                tally(t[u].x, p1, p2, 0);
+                tally(t[u].y, p1, p2, 8);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < UB; ++u) { t[u] = tn[u]; xy[u] = xyn[u]; }
+        n_part += UB;
+        if (n_part >= 256) {
+            flush();
+            n_part = 0;
+        }
+    }
+    // end of the range: quantise, add the CTA's warps in shared memory (exact integers), one atomic per CTA and sum
+    __shared__ long long s_red[kWarps][32][16];
+#pragma unroll
+    for (int c = 0; c < 16; ++c) s_red[warp][lane][c] = __double2ll_rn(static_cast<double>(part[c]) * 4194304.0);
+    __syncthreads();
+    for (int e = threadIdx.x; e < G * 16; e += blockDim.x) {
+        const int ll = e / 16, c = e % 16;
+        long long v = 0;
+        for (int wi = 0; wi < kWarps; ++wi)
+            for (int sb = 0; sb < SPW; ++sb) v += s_red[wi][sb * G + ll][c];
+        atomicAdd(reinterpret_cast<unsigned long long *>(a.fk) + (static_cast<size_t>(s) * a.R + 2 * (blockIdx.z * G + ll)) * 8 + c,
+                  static_cast<unsigned long long>(v));
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(a.ticket + s, 1u) == gridDim.x * gridDim.z - 1u) ? 1 : 0;
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+        const double inv = 1.0 / 4194304.0;
+        for (int r = threadIdx.x; r < a.R; r += blockDim.x) {
+            long long *f = a.fk + (static_cast<size_t>(s) * a.R + r) * 8;
+            double v[8];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) { v[c] = static_cast<double>(__ldcg(f + c)) * inv; f[c] = 0; }
+            const double g1 = (v[0] * v[0] + v[1] * v[1] + v[2] * v[2] + v[3] * v[3]) / a.N;
+            const double g2 = (v[4] * v[4] + v[5] * v[5] + v[6] * v[6] + v[7] * v[7]) / a.N;
+            const size_t sr = static_cast<size_t>(s) * a.R + r;
+            a.G_slot[2 * sr] = g1;
+            a.G_slot[2 * sr + 1] = g2;
+            double *o = a.acc_k + (static_cast<size_t>(s) * a.R + a.temp_of_slot[sr]) * 3;
+            o[0] += 1.0; o[1] += g1; o[2] += g2;
+        }
+        if (threadIdx.x == 0) a.ticket[s] = 0u;
+    }
+}
+
 // ---- init: theta = 2 pi_f * u, Philox domain 0, sweep 0 ------------------------------------------------
 __global__ void k_init_theta(float *theta, int S, int N, int R, PhiloxKeys keys, uint32_t sample_base) {
     const size_t total = static_cast<size_t>(S) * N * R;
