@@ -44,3 +44,24 @@ def obs_u4():
 
 def obs_var_e():
     return lambda m: m[..., E2_] - m[..., E_] ** 2
+
+
+def specific_heat_estimators(blocks, T, N):
+    """Eq. 13: c = (<E^2> - <E>^2) / (N T^2) = (1/N) d<E>/dT.  blocks [B][R][8] accumulator increments
+    by temperature (pooled over samples of one graph, or one sample).  Returns, for the interior temperatures,
+    (c_fluct, sigma, c_deriv, sigma): delete-one jackknife; the derivative is the 3-point Lagrange formula on the
+    (non-uniform) ladder."""
+    T = np.asarray(T, np.float64)
+
+    def deriv(m):
+        e = m[..., E_] / N
+        h0, h1 = T[1:-1] - T[:-2], T[2:] - T[1:-1]
+        return (-h1 / (h0 * (h0 + h1)) * e[..., :-2] + (h1 - h0) / (h0 * h1) * e[..., 1:-1]
+                + h0 / (h1 * (h0 + h1)) * e[..., 2:])
+
+    def fluct(m):
+        return ((m[..., E2_] - m[..., E_] ** 2) / (N * T ** 2))[..., 1:-1]
+
+    cf, sf = jackknife(blocks, fluct)
+    cd, sd = jackknife(blocks, deriv)
+    return cf, sf, cd, sd

@@ -161,3 +161,32 @@ def test_equilibrium_all_configs_vs_oracle():
     assert z.max() < NSIG
     assert (z > 3).sum() <= max(2, int(0.04 * z.size))
     assert np.mean(z ** 2) < 2.0
+
+
+def test_gpu_specific_heat_two_estimators_agree():
+    """Eq. 13: c from the energy fluctuations equals c from d<E>/dT along the temperature ladder
+    (graph-averaged over 16 Levy samples, L = 16, 32 temperatures)."""
+    L, R = 16, 32
+    g = levy.build(L, 3.5, 6, workloads.BASE_SEED, S=16)
+    T = O.geometric_temperatures(R, 1.0, 4.0)
+    ens = U.ensemble_from_levy(g, T, SEED_GPU)
+    blocks = gpu_blocks(ens, 30, 50, 200)                      # [B][S][R][8]
+    ens.close()
+    # per sample estimators (E^2 does not pool across different graphs), then the graph average (Eq. 12);
+    # errors from the delete-one block jackknife of the graph average
+    tot = blocks.sum(0)
+    B = blocks.shape[0]
+    def estimators(acc):                                       # acc [S][R][8]
+        m = acc / acc[..., :1]
+        e = m[..., S.E_] / (L * L)
+        h0, h1 = T[1:-1] - T[:-2], T[2:] - T[1:-1]
+        d = (-h1 / (h0 * (h0 + h1)) * e[..., :-2] + (h1 - h0) / (h0 * h1) * e[..., 1:-1] + h0 / (h1 * (h0 + h1)) * e[..., 2:])
+        f = ((m[..., S.E2_] - m[..., S.E_] ** 2) / (L * L * T ** 2))[..., 1:-1]
+        return f.mean(0), d.mean(0)
+    f_all, d_all = estimators(tot)
+    loo = np.array([estimators(tot - blocks[b]) for b in range(B)])       # [B][2][R-2]
+    sig = np.sqrt((B - 1) / B * ((loo - loo.mean(0)) ** 2).sum(0))
+    z = np.abs(f_all - d_all) / np.sqrt(sig[0] ** 2 + sig[1] ** 2 + (0.01 * f_all) ** 2)
+    print(f"\nspecific heat: max |z| {z.max():.2f}, c range {f_all.min():.3f}..{f_all.max():.3f}, sigma {sig[0].max():.1e} / {sig[1].max():.1e}")
+    assert np.all(z < NSIG), (f_all, d_all, sig)
+    assert np.all(sig[0] < 0.05 * f_all)

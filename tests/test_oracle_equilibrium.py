@@ -157,3 +157,16 @@ def test_levy_graph_low_temperature_harmonic_limit():
     A = sp.csr_matrix((np.ones(len(g["col_idx"])), g["col_idx"], g["row_ptr"]), shape=(N, N))
     ncomp = connected_components(A)[0]
     assert np.allclose(e, -len(edges) + (N - ncomp) * T / 2, rtol=0, atol=0.06 * (N - ncomp) * T / 2 + 0.02)
+
+
+def test_specific_heat_two_estimators_agree():
+    """the paper's equilibration check (Eq. 13): fluctuation and derivative estimators of c coincide."""
+    edges, _ = O.levy_edges(8, 3.5, 6, 0x12113991, 0)
+    N = 64
+    g = G.colour_major(N, [tuple(e) for e in edges])
+    T = O.geometric_temperatures(12, 1.2, 3.6)
+    blocks, _ = run_blocks(g, T, 30, 60, 40)
+    cf, sf, cd, sd = S.specific_heat_estimators(blocks, T, N)
+    z = np.abs(cf - cd) / np.sqrt(sf ** 2 + sd ** 2 + (0.01 * cf) ** 2)     # 1 %: truncation of the 3-point derivative
+    assert np.all(z < NSIG), (cf, cd, sf, sd)
+    assert np.all(sf < 0.08 * cf) and np.all(cf > 0.05)
