@@ -70,6 +70,9 @@ def lib():
         L.orc_fourier.restype = None
         L.orc_xi2.argtypes = [C.c_double, C.c_double, C.c_int, C.c_double]
         L.orc_xi2.restype = C.c_double
+        L.orc_random_walk.argtypes = [C.c_int, _i32p, _i32p, C.c_int, _i32p, C.c_int, C.c_uint64, C.c_uint32,
+                                      np.ctypeslib.ndpointer(np.int64, flags="C_CONTIGUOUS")]
+        L.orc_random_walk.restype = None
         L.orc_run.argtypes = [C.c_int, C.c_int, C.c_int, _i32p, _i32p, _i32p, _f32p, _f64p, _i32p,
                               _i32p, C.c_uint64, C.c_uint32, C.POINTER(C.c_uint32),
                               C.POINTER(C.c_uint32), C.c_int, C.c_int, C.c_int, C.c_int, _f64p,
@@ -212,6 +215,15 @@ def fourier(Lx, Ly, x, y, theta):
 
 def xi2(chi0, chik, L, psi=2.0):
     return float(lib().orc_xi2(float(chi0), float(chik), int(L), float(psi)))
+
+
+def random_walk(row_ptr, col_idx, start, n_steps, seed, sample=0):
+    """hist [n_steps+1] int64: visits of the origin at time t, summed over the walkers."""
+    start = np.ascontiguousarray(start, np.int32)
+    hist = np.zeros(n_steps + 1, np.int64)
+    lib().orc_random_walk(len(row_ptr) - 1, np.ascontiguousarray(row_ptr, np.int32), _ci(col_idx), len(start), start,
+                          n_steps, seed, sample, hist)
+    return hist
 
 
 def accumulate(N, E, Mx, My, temp_of_slot, acc):

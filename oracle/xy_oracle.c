@@ -401,6 +401,34 @@ double orc_xi2(double chi0, double chik, int L, double psi) {
 }
 
 /* ------------------------------------------------------------------------------------------
+ * a8. Random-walk self-return histogram (App. A): "the histogram of return
+ * times is proportional to the probability of self-return of a random walker in the graph after a
+ * time tau", P(tau) ~ tau^(-dbar/2).  DESIGN R19: every visit of the origin at time tau counts (not
+ * only the first return); the simple random walk jumps to a uniformly chosen neighbour.
+ * ---------------------------------------------------------------------------------------- */
+void orc_random_walk(int N, const int32_t *row_ptr, const int32_t *col_idx, int n_walkers,
+                     const int32_t *start, int n_steps, uint64_t seed, uint32_t sample, int64_t *hist) {
+    uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    (void)N;
+    for (int t = 0; t <= n_steps; ++t) hist[t] = 0;
+    hist[0] = n_walkers;
+    for (int w = 0; w < n_walkers; ++w) {
+        int pos = start[w];
+        uint32_t x[4] = {0, 0, 0, 0};
+        for (int t = 1; t <= n_steps; ++t) {
+            const int k = (t - 1) & 3;
+            if (k == 0) {
+                uint32_t ctr[4] = {(uint32_t)w, (uint32_t)((t - 1) >> 2), sample << 16, ORC_DOMAIN_WALK};
+                orc_philox4x32_10(ctr, key, x);
+            }
+            const int deg = row_ptr[pos + 1] - row_ptr[pos];
+            if (deg > 0) pos = col_idx[row_ptr[pos] + (int)(((uint64_t)x[k] * (uint64_t)deg) >> 32)];
+            if (pos == start[w]) hist[t] += 1;
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
  * a5. Parallel tempering (ref 65).  DESIGN R9: round k attempts the pairs
  * (t, t+1) with t = k mod 2, k mod 2 + 2, ...;  a = slot_of_temp[t], b = slot_of_temp[t+1];
  *   accept iff u < exp((beta_t - beta_{t+1}) (E_a - E_b)),   beta = 1/T in fp64;

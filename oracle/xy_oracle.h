@@ -27,6 +27,7 @@ extern "C" {
 #define ORC_DOMAIN_METROPOLIS 1u
 #define ORC_DOMAIN_SWAP 2u
 #define ORC_DOMAIN_GRAPH 3u
+#define ORC_DOMAIN_WALK 4u
 
 /* accumulator columns per (temperature) */
 #define ORC_NACC 8 /* n, E, E^2, |m|, m^2, m^4, Mx/N, My/N */
@@ -96,6 +97,15 @@ void orc_fourier(int N, int R, int Lx, int Ly, const int32_t *x /*[N]*/, const i
                  const float *theta /*[N][R]*/, double *G1 /*[R]*/, double *G2 /*[R]*/);
 /* Eq. 17: xi_2 = [chi(0)/chi(k_min) - 1]^(1/psi) / (2 sin(pi / L)) */
 double orc_xi2(double chi0, double chik, int L, double psi);
+
+/* ---- a8: random-walk self-return histogram for the spectral dimension
+ *      (Eq. 11 P(tau) ~ tau^(-dbar/2); :436-440 App. A; DESIGN R19) ----
+ * Walker w starts at start[w]; at step t = 1..n_steps it moves to a uniformly chosen neighbour of its site
+ * (stays if the site has none); hist[t] += 1 whenever it is back at start[w] after step t (hist[0] = n_walkers).
+ * Neighbour k = (x * deg) >> 32 with x = word (t-1) % 4 of Philox counter (w, (t-1)/4, sample << 16, WALK). */
+void orc_random_walk(int N, const int32_t *row_ptr, const int32_t *col_idx, int n_walkers,
+                     const int32_t *start, int n_steps, uint64_t seed, uint32_t sample,
+                     int64_t *hist /*[n_steps+1]*/);
 
 /* ---- a5: one parallel-tempering swap round (App. B.b, ref 65; DESIGN R9) ----
  * decisions_in NULL: draw u from Philox(SWAP) and decide; else use decisions_in[t] for pair (t,t+1).
