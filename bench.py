@@ -317,6 +317,20 @@ def main():
                                        "frac": bytes_f / (ms_f * 1e-3) * 1e-9 / peak, "bytes_per_spin": 4.0 + 4.0 / w.R}}),
               file=sys.stderr, flush=True)
 
+    # ---- auxiliary row: random-walk self-return histogram, the paper's 4e4 walkers per graph ----
+    if rank == 0 and not args.no_aux:
+        n_w, n_t = 40_000, 1024
+        rng = np.random.default_rng(1)
+        st = np.stack([rng.choice(np.where(np.diff(g.row_ptr[s]) > 2)[0], n_w) for s in range(w.S)]).astype(np.int32)
+        B.xy_random_walk(ens.graph, st, 16, seed)
+        t0 = time.perf_counter()
+        hist = B.xy_random_walk(ens.graph, st, n_t, seed)
+        dt = time.perf_counter() - t0
+        print(json.dumps({"aux": "xy_random_walk (k_random_walk)", "workload": w.name, "walkers_per_graph": n_w, "steps": n_t,
+                          "walker_steps_per_ns": w.S * n_w * n_t / (dt * 1e9), "seconds_incl_copies": dt,
+                          "bound": "latency (two dependent random 32-byte reads per step)",
+                          "returns_at_t2": int(hist[:, 2].sum())}), file=sys.stderr, flush=True)
+
     if args.lscan and rank == 0 and world == 1:
         ens.close()
         for L in (32, 64, 128, 256):

@@ -70,6 +70,16 @@ int xy_graph_info(const xy_graph *g, int *S, int *N, int64_t *nnz_total, int *q_
  * Lx, Ly <= 65535.  For a Levy graph built by xy_levy_build: x = new_to_old % L, y = new_to_old / L.  Synchronous. */
 int xy_graph_set_coords(xy_graph *g, int Lx, int Ly, const int32_t *x /*host*/, const int32_t *y /*host*/);
 
+/* Random-walk self-return histogram on the loaded graphs, for the spectral dimension (Eq. 11
+ * P(tau) ~ tau^(-dbar/2); :436-440 App. A).  For every sample, walker w starts at
+ * start[s][w] (host, [S][n_walkers]) and makes n_steps (<= 12000) jumps to a uniformly chosen neighbour (it stays on a
+ * site without neighbours); hist_host [S][n_steps+1] (host, int64) counts, per time t, the walkers that are back at
+ * their origin after step t (every visit counts; hist[s][0] = n_walkers).  Neighbour choice: (x * degree) >> 32 with
+ * x = word (t-1) % 4 of Philox4x32-10 counter (w, (t-1)/4, (sample_base + s) << 16, 4), key = seed.  Integer work,
+ * bit-exact against the oracle.  Runs on `stream` (cudaStream_t as void*, NULL = default) and synchronises it. */
+int xy_random_walk(const xy_graph *g, int n_walkers, const int32_t *start /*host*/, int n_steps, uint64_t seed,
+                   uint32_t sample_base, void *stream, int64_t *hist_host);
+
 /* ---- PT ensemble ----
  * T [R] host, strictly positive, ascending (T = +inf allowed: beta = 0).  width [R] host or NULL;
  * NULL selects the BASELINE.json proposal width 2 pi min(1, T/2).  beta and width are rounded to fp32

@@ -25,6 +25,7 @@ SYMBOLS = {
     "xy_graph_set_coords": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]),
     "xy_measure_fourier": (C.c_int, [C.c_void_p, C.c_void_p]),
     "xy_read_fourier_accumulators": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "xy_random_walk": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_uint64, C.c_uint32, C.c_void_p, C.c_void_p]),
     "xy_graph_info": (C.c_int, [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int64),
                                 C.POINTER(C.c_int), C.POINTER(C.c_int)]),
     "xy_pt_create": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_void_p,
@@ -141,6 +142,16 @@ def xy_read_fourier_accumulators(pt, shape):
     out = np.empty((*shape, 3), np.float64)
     _check(lib().xy_read_fourier_accumulators(pt, out.ctypes.data_as(C.c_void_p)))
     return out
+
+
+def xy_random_walk(g, start, n_steps, seed, sample_base=0, stream=None):
+    """start [S][n_walkers] host int32 -> hist [S][n_steps+1] int64 (visits of the origin at time t)."""
+    start, sp = _host(start, np.int32)
+    if start.ndim == 1:
+        start = start[None, :]
+    hist = np.zeros((start.shape[0], n_steps + 1), np.int64)
+    _check(lib().xy_random_walk(g, start.shape[1], sp, n_steps, seed, sample_base, stream, hist.ctypes.data_as(C.c_void_p)))
+    return hist
 
 
 def xy_pt_create(g, T, seed, width=None, sample_base=0, theta_dev=None, stream=None):

@@ -614,6 +614,38 @@ int xy_graph_set_coords(xy_graph *g, int Lx, int Ly, const int32_t *x, const int
     return XY_OK;
 }
 
+int xy_random_walk(const xy_graph *g, int n_walkers, const int32_t *start, int n_steps, uint64_t seed, uint32_t sample_base,
+                   void *stream, int64_t *hist_host) {
+    if (!g || !start || !hist_host) return fail(XY_EINVAL, "graph, start or hist is NULL");
+    if (n_walkers < 1 || n_steps < 0 || n_steps > 12000) return fail(XY_EINVAL, "need n_walkers >= 1, 0 <= n_steps <= 12000");
+    if (static_cast<uint64_t>(sample_base) + g->S > 65536u) return fail(XY_EINVAL, "sample_base + S must be <= 65536");
+    const size_t nw = static_cast<size_t>(g->S) * n_walkers, nh = static_cast<size_t>(g->S) * (n_steps + 1);
+    for (size_t i = 0; i < nw; ++i)
+        if (start[i] < 0 || start[i] >= g->N) return fail(XY_EINVAL, "start site out of range");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int32_t *d_start = nullptr;
+    unsigned long long *d_hist = nullptr;
+    int rc;
+    if ((rc = dev_alloc(&d_start, nw)) != XY_OK) return rc;
+    if ((rc = dev_alloc(&d_hist, nh)) != XY_OK) { cudaFree(d_start); return rc; }
+    xy::WalkArgs a;
+    a.rec = g->rec; a.col_idx = g->col_idx; a.start = d_start; a.hist = d_hist;
+    a.N = g->N; a.n_walkers = n_walkers; a.n_steps = n_steps; a.sample_base = sample_base;
+    a.keys = xy::philox_key_schedule(static_cast<uint32_t>(seed), static_cast<uint32_t>(seed >> 32));
+    cudaError_t e = cudaMemcpyAsync(d_start, start, nw * sizeof(int32_t), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(d_hist, 0, nh * sizeof(unsigned long long), st);
+    if (e == cudaSuccess) {
+        const dim3 grid(ceil_div(n_walkers, xy::kBlock), g->S);
+        xy::k_random_walk<<<grid, xy::kBlock, (n_steps + 1) * sizeof(unsigned int), st>>>(a);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(hist_host, d_hist, nh * sizeof(int64_t), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d_start); cudaFree(d_hist);
+    if (e != cudaSuccess) return fail(XY_ECUDA, std::string("xy_random_walk: ") + cudaGetErrorString(e));
+    return XY_OK;
+}
+
 int xy_graph_info(const xy_graph *g, int *S, int *N, int64_t *nnz_total, int *q_max, int *max_degree) {
     if (!g) return fail(XY_EINVAL, "graph is NULL");
     if (S) *S = g->S;

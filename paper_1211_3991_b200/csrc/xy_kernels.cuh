@@ -21,7 +21,7 @@ constexpr int kWarps = kBlock / 32;
 constexpr double kFix = 68719476736.0;          // 2^36: fixed-point scale of the measure reduction
 constexpr double kInvFix = 1.0 / 68719476736.0;
 
-enum : uint32_t { kDomInit = 0u, kDomMetropolis = 1u, kDomSwap = 2u };
+enum : uint32_t { kDomInit = 0u, kDomMetropolis = 1u, kDomSwap = 2u, kDomWalk = 4u };
 enum : int { kModeMetropolis = 0, kModeOverrelax = 1, kModeMeasure = 2, kModeOrMeasure = 3 };
 
 // ---- Philox4x32-10 (Salmon et al., SC'11), written from the round function -------------------------
@@ -425,6 +425,51 @@ __global__ void __launch_bounds__(kBlock) k_fourier2(const FourierArgs a) {
         }
         if (threadIdx.x == 0) a.ticket[s] = 0u;
     }
+}
+
+// ---- random-walk self-return histogram (PAPER.md:149-155 Eq. 11, :436-440 App. A) ------------
+// One thread per walker: at step t it jumps to neighbour (x * deg) >> 32 of its site (stays if the site has none), x =
+// word (t-1) % 4 of Philox counter (walker, (t-1)/4, sample << 16, domain 4); every visit of its origin at time t adds
+// one to hist[sample][t].  Integer work: bit-exact against the oracle.  A step is two dependent random reads (rec,
+// col_idx): latency-bound pointer chasing; the walkers of a warp are independent, so the loads of a warp overlap.
+// The per-CTA histogram lives in shared memory (32-bit counts), flushed with one 64-bit atomic per time and CTA.
+struct WalkArgs {
+    const int2 *rec;            // [S][N]
+    const int32_t *col_idx;
+    const int32_t *start;       // [S][n_walkers]
+    unsigned long long *hist;   // [S][n_steps + 1], zero at launch
+    int N, n_walkers, n_steps;
+    uint32_t sample_base;
+    PhiloxKeys keys;
+};
+
+__global__ void __launch_bounds__(kBlock) k_random_walk(const WalkArgs a) {
+    extern __shared__ unsigned int s_hist[];      // [n_steps + 1]
+    const int s = blockIdx.y;
+    for (int t = threadIdx.x; t <= a.n_steps; t += blockDim.x) s_hist[t] = 0u;
+    __syncthreads();
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w < a.n_walkers) {
+        const int2 *rec = a.rec + static_cast<size_t>(s) * a.N;
+        const int origin = a.start[static_cast<size_t>(s) * a.n_walkers + w];
+        int pos = origin;
+        atomicAdd(&s_hist[0], 1u);
+        uint32_t x[4] = {0u, 0u, 0u, 0u};
+        for (int t = 1; t <= a.n_steps; ++t) {
+            const int k = (t - 1) & 3;
+            if (k == 0)
+                philox4x32_10(static_cast<uint32_t>(w), static_cast<uint32_t>((t - 1) >> 2),
+                              (a.sample_base + static_cast<uint32_t>(s)) << 16, kDomWalk, a.keys, x);
+            const int2 rc = __ldg(rec + pos);
+            const uint32_t deg = static_cast<uint32_t>(rc.y & 0xffff);
+            const uint32_t xk = k == 0 ? x[0] : k == 1 ? x[1] : k == 2 ? x[2] : x[3];
+            if (deg > 0u) pos = __ldg(a.col_idx + rc.x + static_cast<int>(__umulhi(xk, deg)));
+            if (pos == origin) atomicAdd(&s_hist[t], 1u);
+        }
+    }
+    __syncthreads();
+    for (int t = threadIdx.x; t <= a.n_steps; t += blockDim.x)
+        if (s_hist[t]) atomicAdd(a.hist + static_cast<size_t>(s) * (a.n_steps + 1) + t, static_cast<unsigned long long>(s_hist[t]));
 }
 
 // ---- init: theta = 2 pi_f * u, Philox domain 0, sweep 0 ------------------------------------------------
