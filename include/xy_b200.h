@@ -140,12 +140,23 @@ int xy_set_schedule(xy_pt *pt, int samples_per_group);
  * (default), 1 = always 8-warp, 2 = always 32-warp.  Synchronises the stream and drops the captured graphs. */
 int xy_set_tuning(xy_pt *pt, int balance, int pdl, int l2_persist, int fuse_measure, int cta_shape);
 
+/* Order of a sweep.  0 (default): the order stated at the top -- a Metropolis sweep over all
+ * colours, then the over-relaxation sweep(s).  1 = INTERLEAVED: for every colour class in turn, Metropolis and then
+ * over-relaxation of each of its sites (a different, equally valid Markov chain: each update leaves the Gibbs measure
+ * invariant in any order).  Same-colour sites share no bond, so both updates of a site see the same neighbours and the
+ * kernel serves them from ONE gather of the local field.  Needs or_per_sweep == 1 and a float2 kernel flavour
+ * (R = 2 * 2^k <= 64 or R % 64 == 0), else XY_ESTATE / XY_EINVAL.  Applies to xy_run and xy_run_sweeps; xy_sweep and
+ * xy_overrelax keep their meaning.  Synchronises the stream. */
+int xy_set_order(xy_pt *pt, int order);
+
 /* ---- single-colour steps (lockstep parity tests) ----
  * Metropolis on colour class `colour` of every sample with Philox sweep index `sweep` (the handle's
  * sweep counter is not touched); OR on one colour class.  Launched sample group by sample group with the
  * same grids as xy_run (xy_set_schedule), so a lockstep check exercises the timed launch configuration. */
 int xy_metropolis_colour(xy_pt *pt, int colour, uint32_t sweep);
 int xy_overrelax_colour(xy_pt *pt, int colour);
+/* interleaved order: Metropolis (Philox sweep index `sweep`) and then over-relaxation of every site of the class */
+int xy_metor_colour(xy_pt *pt, int colour, uint32_t sweep);
 
 /* ---- state access (all synchronise the stream) ---- */
 int xy_get_theta(xy_pt *pt, float *theta_host /*[S][N][R]*/);

@@ -78,6 +78,11 @@ def lib():
                               C.POINTER(C.c_uint32), C.c_int, C.c_int, C.c_int, C.c_int, _f64p,
                               C.c_void_p, C.c_void_p]
         L.orc_run.restype = None
+        L.orc_run_order.argtypes = [C.c_int, C.c_int, C.c_int, _i32p, _i32p, _i32p, _f32p, _f64p, _i32p,
+                                    _i32p, C.c_uint64, C.c_uint32, C.POINTER(C.c_uint32),
+                                    C.POINTER(C.c_uint32), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _f64p,
+                                    C.c_void_p, C.c_void_p]
+        L.orc_run_order.restype = None
         _lib = L
     return _lib
 
@@ -262,12 +267,12 @@ class Chain:
         self.swap_attempts = np.zeros(max(self.R - 1, 1), np.int64)
         self.swap_accepts = np.zeros(max(self.R - 1, 1), np.int64)
 
-    def run(self, n_cycles, sweeps_per_swap=10, or_per_sweep=1, measure_every=1):
-        lib().orc_run(self.N, self.R, self.Q, self.row_ptr, self.col_idx, self.class_ptr,
-                      self.theta, self.T, self.temp_of_slot, self.slot_of_temp, self.seed,
-                      self.sample, C.byref(self.sweep), C.byref(self.round), n_cycles,
-                      sweeps_per_swap, or_per_sweep, measure_every, self.acc,
-                      _ptr(self.swap_attempts), _ptr(self.swap_accepts))
+    def run(self, n_cycles, sweeps_per_swap=10, or_per_sweep=1, measure_every=1, order=0):
+        lib().orc_run_order(self.N, self.R, self.Q, self.row_ptr, self.col_idx, self.class_ptr,
+                            self.theta, self.T, self.temp_of_slot, self.slot_of_temp, self.seed,
+                            self.sample, C.byref(self.sweep), C.byref(self.round), n_cycles,
+                            sweeps_per_swap, or_per_sweep, measure_every, order, self.acc,
+                            _ptr(self.swap_attempts), _ptr(self.swap_accepts))
 
     def reset_acc(self):
         self.acc[:] = 0.0

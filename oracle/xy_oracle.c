@@ -464,11 +464,12 @@ void orc_pt_swap(int R, const double *T, const double *E_slot, int32_t *slot_of_
  * swaps every `sweeps_per_swap` sweeps).  Colours are processed sequentially, same-colour sites
  * are mutually independent.
  * ---------------------------------------------------------------------------------------- */
-void orc_run(int N, int R, int Q, const int32_t *row_ptr, const int32_t *col_idx,
-             const int32_t *class_ptr, float *theta, const double *T, int32_t *temp_of_slot,
-             int32_t *slot_of_temp, uint64_t seed, uint32_t sample, uint32_t *sweep,
-             uint32_t *round, int n_cycles, int sweeps_per_swap, int or_per_sweep,
-             int measure_every, double *acc, int64_t *swap_attempts, int64_t *swap_accepts) {
+void orc_run_order(int N, int R, int Q, const int32_t *row_ptr, const int32_t *col_idx,
+                   const int32_t *class_ptr, float *theta, const double *T, int32_t *temp_of_slot,
+                   int32_t *slot_of_temp, uint64_t seed, uint32_t sample, uint32_t *sweep,
+                   uint32_t *round, int n_cycles, int sweeps_per_swap, int or_per_sweep,
+                   int measure_every, int order, double *acc, int64_t *swap_attempts,
+                   int64_t *swap_accepts) {
     float *beta_f = (float *)malloc((size_t)R * sizeof(float));
     float *w_f = (float *)malloc((size_t)R * sizeof(float));
     float *beta_slot = (float *)malloc((size_t)R * sizeof(float));
@@ -488,14 +489,27 @@ void orc_run(int N, int R, int Q, const int32_t *row_ptr, const int32_t *col_idx
         }
         for (int k = 0; k < sweeps_per_swap; ++k) {
             *sweep += 1u;
-            for (int c = 0; c < Q; ++c)
-                orc_metropolis_sites(N, R, row_ptr, col_idx, theta, sites + class_ptr[c],
-                                     class_ptr[c + 1] - class_ptr[c], beta_slot, w_slot, seed,
-                                     *sweep, sample, NULL, NULL);
-            for (int o = 0; o < or_per_sweep; ++o)
-                for (int c = 0; c < Q; ++c)
+            if (order == 1) {
+                /* interleaved order: per colour class, Metropolis and then the
+                 * over-relaxation of its sites; every update leaves the Gibbs measure invariant, so
+                 * any fixed order of the same updates is a valid chain. */
+                for (int c = 0; c < Q; ++c) {
+                    orc_metropolis_sites(N, R, row_ptr, col_idx, theta, sites + class_ptr[c],
+                                         class_ptr[c + 1] - class_ptr[c], beta_slot, w_slot, seed,
+                                         *sweep, sample, NULL, NULL);
                     orc_overrelax_sites(N, R, row_ptr, col_idx, theta, sites + class_ptr[c],
                                         class_ptr[c + 1] - class_ptr[c], NULL);
+                }
+            } else {
+                for (int c = 0; c < Q; ++c)
+                    orc_metropolis_sites(N, R, row_ptr, col_idx, theta, sites + class_ptr[c],
+                                         class_ptr[c + 1] - class_ptr[c], beta_slot, w_slot, seed,
+                                         *sweep, sample, NULL, NULL);
+                for (int o = 0; o < or_per_sweep; ++o)
+                    for (int c = 0; c < Q; ++c)
+                        orc_overrelax_sites(N, R, row_ptr, col_idx, theta, sites + class_ptr[c],
+                                            class_ptr[c + 1] - class_ptr[c], NULL);
+            }
             if (measure_every > 0 && (*sweep % (uint32_t)measure_every) == 0u) {
                 orc_measure(N, R, row_ptr, col_idx, theta, E, Mx, My);
                 orc_accumulate(N, R, E, Mx, My, temp_of_slot, acc);
@@ -511,4 +525,14 @@ void orc_run(int N, int R, int Q, const int32_t *row_ptr, const int32_t *col_idx
     }
     free(beta_f); free(w_f); free(beta_slot); free(w_slot);
     free(E); free(Mx); free(My); free(sites); free(dec);
+}
+
+void orc_run(int N, int R, int Q, const int32_t *row_ptr, const int32_t *col_idx,
+             const int32_t *class_ptr, float *theta, const double *T, int32_t *temp_of_slot,
+             int32_t *slot_of_temp, uint64_t seed, uint32_t sample, uint32_t *sweep,
+             uint32_t *round, int n_cycles, int sweeps_per_swap, int or_per_sweep,
+             int measure_every, double *acc, int64_t *swap_attempts, int64_t *swap_accepts) {
+    orc_run_order(N, R, Q, row_ptr, col_idx, class_ptr, theta, T, temp_of_slot, slot_of_temp, seed,
+                  sample, sweep, round, n_cycles, sweeps_per_swap, or_per_sweep, measure_every, 0, acc,
+                  swap_attempts, swap_accepts);
 }

@@ -125,6 +125,15 @@ void orc_run(int N, int R, int Q, const int32_t *row_ptr, const int32_t *col_idx
              int measure_every, double *acc /*[R][ORC_NACC]*/, int64_t *swap_attempts,
              int64_t *swap_accepts);
 
+/* the same with the order of a sweep as a parameter: 0 = as orc_run, 1 = interleaved by colour (per colour
+ * class: Metropolis, then over-relaxation of its sites; needs or_per_sweep == 1) */
+void orc_run_order(int N, int R, int Q, const int32_t *row_ptr, const int32_t *col_idx,
+                   const int32_t *class_ptr, float *theta, const double *T, int32_t *temp_of_slot,
+                   int32_t *slot_of_temp, uint64_t seed, uint32_t sample, uint32_t *sweep,
+                   uint32_t *round, int n_cycles, int sweeps_per_swap, int or_per_sweep,
+                   int measure_every, int order, double *acc, int64_t *swap_attempts,
+                   int64_t *swap_accepts);
+
 #ifdef __cplusplus
 }
 #endif

@@ -41,6 +41,8 @@ SYMBOLS = {
     "xy_set_tuning": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]),
     "xy_metropolis_colour": (C.c_int, [C.c_void_p, C.c_int, C.c_uint32]),
     "xy_overrelax_colour": (C.c_int, [C.c_void_p, C.c_int]),
+    "xy_metor_colour": (C.c_int, [C.c_void_p, C.c_int, C.c_uint32]),
+    "xy_set_order": (C.c_int, [C.c_void_p, C.c_int]),
     "xy_get_theta": (C.c_int, [C.c_void_p, C.c_void_p]),
     "xy_set_theta": (C.c_int, [C.c_void_p, C.c_void_p]),
     "xy_get_labels": (C.c_int, [C.c_void_p, C.c_void_p]),
@@ -211,6 +213,14 @@ def xy_metropolis_colour(pt, colour, sweep):
     _check(lib().xy_metropolis_colour(pt, colour, sweep))
 
 
+def xy_metor_colour(pt, colour, sweep):
+    _check(lib().xy_metor_colour(pt, colour, sweep))
+
+
+def xy_set_order(pt, order):
+    _check(lib().xy_set_order(pt, order))
+
+
 def xy_overrelax_colour(pt, colour):
     _check(lib().xy_overrelax_colour(pt, colour))
 
@@ -339,6 +349,8 @@ class Ensemble:
         xy_set_tuning(self.pt, balance, pdl, l2_persist, fuse_measure, cta_shape)
     def metropolis_colour(self, c, sweep): xy_metropolis_colour(self.pt, c, sweep)
     def overrelax_colour(self, c): xy_overrelax_colour(self.pt, c)
+    def metor_colour(self, c, sweep): xy_metor_colour(self.pt, c, sweep)
+    def set_order(self, order): xy_set_order(self.pt, order)
     def get_theta(self, out=None): return xy_get_theta(self.pt, (self.S, self.N, self.R), out)
     def set_theta(self, th): xy_set_theta(self.pt, th)
     def get_labels(self): return xy_get_labels(self.pt, (self.S, self.R))

@@ -60,7 +60,9 @@ template <int W>
 const void *phase_function(int G, bool single_block, int mode) {
     return mode == 0 ? phase_function_mode<0, W>(G, single_block)
          : mode == 1 ? phase_function_mode<1, W>(G, single_block)
-         : mode == 2 ? phase_function_mode<2, W>(G, single_block) : phase_function_mode<3, W>(G, single_block);
+         : mode == 2 ? phase_function_mode<2, W>(G, single_block)
+         : mode == 3 ? phase_function_mode<3, W>(G, single_block)
+         : mode == 4 ? phase_function_mode<4, W>(G, single_block) : phase_function_mode<5, W>(G, single_block);
 }
 
 }  // namespace
@@ -118,7 +120,8 @@ struct xy_pt {
     size_t l2_persist_bytes = 0, l2_window_max = 0;   // device limits (0 = not supported)
     int balance = 1;                 // cost-balanced share tables (1) or equal shares (0)
     int pdl = 1;                     // programmatic dependent launch edges between the k_phase launches
-    const void *phase_fn[2][4] = {};   // k_phase<G, CB, MODE, W>: [0] W = 8 warps per CTA, [1] W = 32
+    const void *phase_fn[2][6] = {};   // k_phase<G, CB, MODE, W>: [0] W = 8 warps per CTA, [1] W = 32
+    int order = 0;                   // 0 = Metropolis sweep then OR sweep, 1 = interleaved by colour (xy_set_order)
     int capacity_big = 0;            // co-resident 32-warp CTAs (one per SM)
     int cta_shape = 0;               // 0 = by class size, 1 = always 8-warp CTAs, 2 = always 32-warp CTAs
     int fuse_measure = 1;            // measured sweeps: the last over-relaxation sweep also produces E, Mx, My (MODE 3)
@@ -362,12 +365,35 @@ int sweep_group_fused(xy_pt *pt, int s0, int s1, bool accumulate) {
     return XY_OK;
 }
 
+// interleaved order: one sweep = for every colour class, Metropolis and then over-relaxation of each of its sites from
+// one gather (k_phase MODE 4; MODE 5 also produces E, Mx, My, converted by the launch of the last non-empty colour)
+int sweep_group_interleaved(xy_pt *pt, int s0, int s1, int sweep_offset, int measure /*0 none, 1 E only, 2 accumulate*/) {
+    const xy_graph *g = pt->g;
+    int last = -1;
+    for (int c = 0; c < g->q_max; ++c)
+        if (max_class_size(g, c, s0, s1) > 0) last = c;
+    for (int c = 0; c <= last; ++c) {
+        const int rc = launch_phase(pt, measure ? 5 : 4, c, s0, s1, true, sweep_offset, 0u,
+                                    (measure == 2 ? 1 : 0) | (measure && c == last ? 2 : 0));
+        if (rc != XY_OK) return rc;
+    }
+    if (measure && last < 0) return launch_measure(pt, s0, s1, measure == 2);
+    return XY_OK;
+}
+
 int issue_cycle(xy_pt *pt, int sps, int orps, int me, int phase, int group) {
     const int S = pt->g->S;
     for (int s0 = 0; s0 < S; s0 += group) {
         const int s1 = std::min(S, s0 + group);
         bool fresh = false;
         for (int k = 1; k <= sps; ++k) {
+            if (pt->order == 1) {
+                const bool measured = me > 0 && (phase + k) % me == 0;
+                const int rc = sweep_group_interleaved(pt, s0, s1, k, measured ? 2 : (k == sps ? 1 : 0));
+                if (rc != XY_OK) return rc;
+                fresh = measured || k == sps;
+                continue;
+            }
             int rc = sweep_group(pt, 0, s0, s1, true, k, 0u);
             if (rc != XY_OK) return rc;
             const bool measured = me > 0 && (phase + k) % me == 0;
@@ -399,6 +425,11 @@ int issue_sweeps(xy_pt *pt, int sps, int orps, int group) {
     for (int s0 = 0; s0 < S; s0 += group) {
         const int s1 = std::min(S, s0 + group);
         for (int k = 1; k <= sps; ++k) {
+            if (pt->order == 1) {
+                const int rc = sweep_group_interleaved(pt, s0, s1, k, 0);
+                if (rc != XY_OK) return rc;
+                continue;
+            }
             int rc = sweep_group(pt, 0, s0, s1, true, k, 0u);
             if (rc != XY_OK) return rc;
             for (int o = 0; o < orps; ++o)
@@ -700,7 +731,7 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
     pt->keys = xy::philox_key_schedule(pt->key0, pt->key1);
     pt->measure_chunk = std::max(256, ((N + 127) / 128 + 7) / 8 * 8);   // legacy measure partition: a function of N only
     if (pt->fast_G) {
-        for (int m = 0; m < 4; ++m) {
+        for (int m = 0; m < 6; ++m) {
             pt->phase_fn[0][m] = phase_function<xy::kWarpsSmall>(pt->fast_G, pt->col_blocks == 1, m);
             pt->phase_fn[1][m] = phase_function<xy::kWarpsBig>(pt->fast_G, pt->col_blocks == 1, m);
             for (int b = 0; b < 2; ++b) {
@@ -844,6 +875,28 @@ int xy_metropolis_colour(xy_pt *pt, int colour, uint32_t sweep) {
     return XY_OK;
 }
 
+int xy_metor_colour(xy_pt *pt, int colour, uint32_t sweep) {
+    if (!check_pt(pt) || colour < 0 || colour >= pt->g->q_max) return fail(XY_EINVAL, "bad handle or colour");
+    if (!pt->fast_G) return fail(XY_ESTATE, "the interleaved order needs a float2 kernel flavour (R = 2 * 2^k <= 64 or R % 64 == 0)");
+    pt->e_fresh = false;
+    const int group = auto_group(pt);
+    for (int s0 = 0; s0 < pt->g->S; s0 += group) {
+        const int rc = launch_phase(pt, 4, colour, s0, std::min(pt->g->S, s0 + group), false, 0, sweep, 0);
+        if (rc != XY_OK) return rc;
+    }
+    return XY_OK;
+}
+
+int xy_set_order(xy_pt *pt, int order) {
+    if (!check_pt(pt) || order < 0 || order > 1) return fail(XY_EINVAL, "bad handle or order not in {0, 1}");
+    if (order == 1 && !pt->fast_G)
+        return fail(XY_ESTATE, "the interleaved order needs a float2 kernel flavour (R = 2 * 2^k <= 64 or R % 64 == 0)");
+    XY_CUDA(cudaStreamSynchronize(pt->stream));
+    pt->order = order;
+    drop_graphs(pt);
+    return XY_OK;
+}
+
 int xy_overrelax_colour(xy_pt *pt, int colour) {
     if (!check_pt(pt) || colour < 0 || colour >= pt->g->q_max) return fail(XY_EINVAL, "bad handle or colour");
     pt->e_fresh = false;
@@ -978,6 +1031,7 @@ int xy_set_tuning(xy_pt *pt, int balance, int pdl, int l2_persist, int fuse_meas
 int xy_run(xy_pt *pt, int n_cycles, int sps, int orps, int me) {
     if (!check_pt(pt) || n_cycles < 0 || sps < 1 || orps < 0 || me < 0)
         return fail(XY_EINVAL, "need n_cycles >= 0, sweeps_per_swap >= 1, or_per_sweep >= 0, measure_every >= 0");
+    if (pt->order == 1 && orps != 1) return fail(XY_EINVAL, "the interleaved order needs or_per_sweep == 1");
     const int group = auto_group(pt);
     {
         const int rc = prepare_partitions(pt, group);
@@ -1001,6 +1055,7 @@ int xy_run(xy_pt *pt, int n_cycles, int sps, int orps, int me) {
 int xy_run_sweeps(xy_pt *pt, int n_blocks, int sps, int orps) {
     if (!check_pt(pt) || n_blocks < 0 || sps < 1 || orps < 0)
         return fail(XY_EINVAL, "need n_blocks >= 0, sweeps_per_block >= 1, or_per_sweep >= 0");
+    if (pt->order == 1 && orps != 1) return fail(XY_EINVAL, "the interleaved order needs or_per_sweep == 1");
     const int group = auto_group(pt);
     {
         const int rc = prepare_partitions(pt, group);

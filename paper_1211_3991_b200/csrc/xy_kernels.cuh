@@ -22,7 +22,7 @@ constexpr double kFix = 68719476736.0;          // 2^36: fixed-point scale of th
 constexpr double kInvFix = 1.0 / 68719476736.0;
 
 enum : uint32_t { kDomInit = 0u, kDomMetropolis = 1u, kDomSwap = 2u, kDomWalk = 4u };
-enum : int { kModeMetropolis = 0, kModeOverrelax = 1, kModeMeasure = 2, kModeOrMeasure = 3 };
+enum : int { kModeMetropolis = 0, kModeOverrelax = 1, kModeMeasure = 2, kModeOrMeasure = 3, kModeMetOr = 4, kModeMetOrMeasure = 5 };
 
 // ---- Philox4x32-10 (Salmon et al., SC'11), written from the round function -------------------------
 // ks[2r], ks[2r+1] = the round keys k0 + r W0, k1 + r W1 (W0 = 0x9E3779B9, W1 = 0xBB67AE85)

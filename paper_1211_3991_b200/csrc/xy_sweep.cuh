@@ -135,6 +135,12 @@ template <> struct PairAcc<kModeOrMeasure> {
     }
 };
 
+// interleaved order (xy_set_order): Metropolis and then over-relaxation of the SAME site from
+// ONE gather.  Same-colour sites share no bond, so the neighbours do not change between the two updates, and the local
+// field h = sum_j (cos th_j, sin th_j) serves both: sum_j sin(mid - th_j) = sin(mid) h_x - cos(mid) h_y.
+template <> struct PairAcc<kModeMetOr> : PairAcc<kModeOverrelax> {};
+template <> struct PairAcc<kModeMetOrMeasure> : PairAcc<kModeOrMeasure> {};
+
 // fixed-point (scale 2^19) bond energy of one slot of a site: -E_i = cos th_i l_x + sin th_i l_y, |.| <= nlow.
 // Explicit fma/mul so that the measure kernel and the fused over-relaxation kernel round identically.
 __device__ __forceinline__ float site_energy(float c, float s, float lx, float ly) {
@@ -306,7 +312,10 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
 
     float2 nbeta = make_float2(0.f, 0.f), w = make_float2(0.f, 0.f);
     uint32_t c2 = 0;
-    if constexpr (MODE == kModeMetropolis) {
+    constexpr bool kMet = MODE == kModeMetropolis || MODE == kModeMetOr || MODE == kModeMetOrMeasure;
+    constexpr bool kFusedMetOr = MODE == kModeMetOr || MODE == kModeMetOrMeasure;
+    constexpr bool kTally = MODE == kModeMeasure || MODE == kModeOrMeasure || MODE == kModeMetOrMeasure;
+    if constexpr (kMet) {
         const float2 b = __ldcg(reinterpret_cast<const float2 *>(a.beta_slot) + static_cast<size_t>(s) * R2 + x.q);
         nbeta = make_float2(-b.x, -b.y);
         w = __ldcg(reinterpret_cast<const float2 *>(a.w_slot) + static_cast<size_t>(s) * R2 + x.q);
@@ -315,7 +324,7 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
 
     // Metropolis proposal of site i (both slots of the lane): th' = th + w (u1 - 1/2), half = (th' - th)/2
     auto begin = [&](int i, int nlow, const float2 own, PairAcc<MODE> &acc, float2 &thp, float2 &u2) {
-        if constexpr (MODE == kModeMetropolis) {
+        if constexpr (kMet) {
             uint32_t r[4];
             philox4x32_10(static_cast<uint32_t>(i), sweep, c2, kDomMetropolis, a.keys, r);
             // u = (k + 1/2) 2^-23 with k = x >> 9 (R11), every step exact:
@@ -326,10 +335,9 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
             // R5: delta = fp32(w * (u1 - 1/2)), th' = fp32(th + delta): two roundings.  Scalar mul.rn / add.rn on purpose:
             // ptxas contracts mul.rn.f32x2 + add.rn.f32x2 into one FFMA2 (single rounding, 1 ulp off in 11 % of the moves)
             thp = make_float2(__fadd_rn(own.x, __fmul_rn(w.x, u1mh.x)), __fadd_rn(own.y, __fmul_rn(w.y, u1mh.y)));
-            acc.mid = add2(own, mul2(sub2(thp, own), make_float2(0.5f, 0.5f)));
-        } else if constexpr (MODE == kModeOrMeasure) {
-            acc.nlow = nlow;
+            if constexpr (MODE == kModeMetropolis) acc.mid = add2(own, mul2(sub2(thp, own), make_float2(0.5f, 0.5f)));
         }
+        if constexpr (MODE == kModeOrMeasure || MODE == kModeMetOrMeasure) acc.nlow = nlow;
     };
     // measure by-product of one site: fixed-point bond energy (lower neighbours) and magnetisation of both slots
     // The per-lane partial sums are 32-bit.  A site adds at most 2^22 per quantity (one "unit"), or 2^24 to the energy
@@ -384,6 +392,25 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
             out.x = overrelax_finish(own.x, acc.hx.x, acc.hy.x);
             out.y = overrelax_finish(own.y, acc.hx.y, acc.hy.y);
             if (UNI || valid) lb[static_cast<unsigned long long>(static_cast<uint32_t>(i) * R2)] = out;
+        } else if constexpr (kFusedMetOr) {
+            // Metropolis from the local field: dE = 2 sin((th'-th)/2) (sin(mid) h_x - cos(mid) h_y), then the
+            // over-relaxation of the (possibly moved) spin about the same h
+            const float2 half = mul2(sub2(thp, own), make_float2(0.5f, 0.5f));
+            const float2 mid = add2(own, half);
+            float smx, cmx, smy, cmy;
+            __sincosf(mid.x, &smx, &cmx);
+            __sincosf(mid.y, &smy, &cmy);
+            const float2 ss = make_float2(__fmaf_rn(smx, acc.hx.x, -__fmul_rn(cmx, acc.hy.x)),
+                                          __fmaf_rn(smy, acc.hx.y, -__fmul_rn(cmy, acc.hy.y)));
+            const float2 sh = make_float2(__sinf(half.x), __sinf(half.y));
+            const float2 arg = mul2(nbeta, mul2(add2(sh, sh), ss));
+            float2 out;
+            out.x = overrelax_finish(metropolis_select(own.x, thp.x, u2.x, __expf(arg.x)), acc.hx.x, acc.hy.x);
+            out.y = overrelax_finish(metropolis_select(own.y, thp.y, u2.y, __expf(arg.y)), acc.hx.y, acc.hy.y);
+            if (UNI || valid) {
+                lb[static_cast<unsigned long long>(static_cast<uint32_t>(i) * R2)] = out;
+                if constexpr (MODE == kModeMetOrMeasure) tally(out, acc.lx, acc.ly, nlow);
+            }
         } else if constexpr (MODE == kModeOrMeasure) {
             float2 out;
             out.x = overrelax_finish(own.x, acc.hx.x, acc.hy.x);
@@ -512,7 +539,7 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
         }
         __syncwarp();
         i0 += msite;
-        if constexpr (MODE == kModeMeasure || MODE == kModeOrMeasure) {
+        if constexpr (kTally) {
             if (units >= 320 && i0 < w1) {      // a chunk adds at most 128 units: the partial sums stay below 448 * 2^22 < 2^31
                 flush_partial();
                 units = 0;
@@ -553,6 +580,8 @@ __device__ __forceinline__ void sweep_finalize(const TileArgs &a, int s, bool ac
 // MODE 0 / 1: Metropolis / over-relaxation on colour a.t.colour; MODE 2: measure (a.t.accumulate bit 0), the last CTA
 // of the sample converts the fixed-point sums; MODE 3: over-relaxation that also adds the class's share of E, Mx, My
 // to the fixed-point sums (the measurement costs no extra gather), converted by the launch of the sweep's last colour.
+// MODE 4 / 5 (interleaved order, xy_set_order): Metropolis and then over-relaxation of every site of the class from one
+// gather, without / with the measurement by-product.
 #ifdef XY_TRACE   // tuning builds only (_work): per-warp time stamps of the last k_phase launch
 __device__ unsigned long long g_trace[8192][4];
 __device__ __forceinline__ unsigned long long trace_now() {
@@ -587,7 +616,7 @@ __global__ void __launch_bounds__(W * 32, kSmPerWarpSlots / W) k_phase(const Swe
     x.ring_s = static_cast<uint32_t>(__cvta_generic_to_shared(x.ring_l));
 
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    const PhasePrep P = sweep_prep<G, CB, W>(a, x, MODE == kModeOrMeasure ? kModeOverrelax : MODE, a.t.colour);
+    const PhasePrep P = sweep_prep<G, CB, W>(a, x, MODE == kModeMeasure ? kModeMeasure : kModeOverrelax, a.t.colour);
     __syncwarp();
     asm volatile("griddepcontrol.wait;" ::: "memory");      // the predecessor's theta / beta_slot / fx are final
 
@@ -606,7 +635,7 @@ __global__ void __launch_bounds__(W * 32, kSmPerWarpSlots / W) k_phase(const Swe
     }
 #endif
 
-    if constexpr (MODE == kModeMeasure || MODE == kModeOrMeasure) {
+    if constexpr (MODE == kModeMeasure || MODE == kModeOrMeasure || MODE == kModeMetOrMeasure) {
         __syncthreads();
         long long *s_red = reinterpret_cast<long long *>(&s_w[0]);
 #pragma unroll

@@ -95,3 +95,36 @@ def lockstep_overrelax(ens, graphs, colour, samples=None, site_subset=None, rng=
 
 def graphs_of_levy(g):
     return [(g.row_ptr[s], g.col_idx[s], g.class_ptr(s)) for s in range(g.S)]
+
+
+def lockstep_metor(ens, graphs, T, seed, colour, sweep, samples=None, site_subset=None, sample_base=0, rng=None):
+    """interleaved order: Metropolis then over-relaxation of one colour class in one launch, against the oracle's
+    two calls from the same pre-state.  Sites whose Metropolis decision is near threshold (R6) are excluded and
+    counted; the rest must satisfy the |h|-weighted over-relaxation bar (R7)."""
+    pre = ens.get_theta()
+    labels = ens.get_labels()
+    ens.metor_colour(colour, sweep)
+    post = ens.get_theta()
+    stats = dict(updates=0, near=0, bad=0, illcond=0, accepted=0)
+    for s in (range(ens.S) if samples is None else samples):
+        rp, ci, cp = graphs[s]
+        lo, hi = (int(cp[colour]), int(cp[colour + 1])) if colour + 1 < len(cp) else (0, 0)
+        assert np.array_equal(post[s, :lo], pre[s, :lo]) and np.array_equal(post[s, hi:], pre[s, hi:])
+        sites = np.arange(lo, hi, dtype=np.int32)
+        if site_subset is not None and len(sites) > site_subset:
+            sites = np.sort(rng.choice(sites, site_subset, replace=False)).astype(np.int32)
+        if len(sites) == 0:
+            continue
+        bs, ws = slot_params(T, labels[s])
+        ref = pre[s].copy()
+        margin, acc = O.metropolis_sites(rp, ci, ref, sites, bs, ws, seed, sweep, sample_base + s, want_margin=True)
+        hn = O.overrelax_sites(rp, ci, ref, sites, want_hnorm=True)
+        err = circ(post[s, sites], ref[sites])
+        scaled = err * np.minimum(1.0, hn)
+        near = margin < BAND
+        stats["updates"] += err.size
+        stats["near"] += int(near.sum())
+        stats["accepted"] += int(acc.sum())
+        stats["illcond"] += int(((err > TOL) & (scaled <= TOL) & ~near).sum())
+        stats["bad"] += int(((scaled > TOL) & ~near).sum())
+    return stats

@@ -14,13 +14,13 @@ SEED = 0x5EED1234
 NSIG = 4.5
 
 
-def run_blocks(g, T, n_blocks, cycles_per_block, burn_cycles, seed=SEED, sweeps_per_swap=10, or_per_sweep=1):
+def run_blocks(g, T, n_blocks, cycles_per_block, burn_cycles, seed=SEED, sweeps_per_swap=10, or_per_sweep=1, order=0):
     ch = O.Chain(g["row_ptr"], g["col_idx"], g["class_ptr"], T, seed)
-    ch.run(burn_cycles, sweeps_per_swap, or_per_sweep, 1)
+    ch.run(burn_cycles, sweeps_per_swap, or_per_sweep, 1, order)
     blocks = []
     for _ in range(n_blocks):
         ch.reset_acc()
-        ch.run(cycles_per_block, sweeps_per_swap, or_per_sweep, 1)
+        ch.run(cycles_per_block, sweeps_per_swap, or_per_sweep, 1, order)
         blocks.append(ch.acc.copy())
     return np.array(blocks), ch
 
@@ -170,3 +170,31 @@ def test_specific_heat_two_estimators_agree():
     z = np.abs(cf - cd) / np.sqrt(sf ** 2 + sd ** 2 + (0.01 * cf) ** 2)     # 1 %: truncation of the 3-point derivative
     assert np.all(z < NSIG), (cf, cd, sf, sd)
     assert np.all(sf < 0.08 * cf) and np.all(cf > 0.05)
+
+
+@pytest.mark.parametrize("name", ["K3", "paw", "K4"])
+def test_interleaved_order_samples_the_same_gibbs_measure(name):
+    """per colour class Metropolis then over-relaxation (orc_run_order, order = 1) is a different
+    chain with the same stationary distribution: the quadrature pins must hold for it too."""
+    N, edges = CF.SMALL_GRAPHS[name]
+    betas = np.array([2.0, 1.0, 0.5])
+    g = G.colour_major(N, edges)
+    blocks, _ = run_blocks(g, 1 / betas, 40, 100, 50, order=1)
+    q = [CF.quadrature(N, edges, b) for b in betas]
+    check(blocks, lambda m: m[..., S.E_], [x["E"] for x in q], f"{name} E")
+    check(blocks, S.obs_var_e(), [x["varE"] for x in q], f"{name} varE")
+    check(blocks, S.obs_absm(), [x["absm"] for x in q], f"{name} |m|")
+    check(blocks, S.obs_m4(), [x["m4"] for x in q], f"{name} m4")
+
+
+def test_interleaved_order_ring_closed_form_and_differs_from_default():
+    N = 16
+    T = np.array([0.5, 1.0, 2.0, 4.0])
+    g = G.colour_major(N, G.ring_edges(N))
+    blocks, ch = run_blocks(g, T, 40, 40, 40, order=1)
+    exact = np.array([CF.ring(N, 1 / t) for t in T])
+    check(blocks, S.obs_energy(N), exact[:, 0], "ring interleaved e")
+    check(blocks, S.obs_m2(), exact[:, 1], "ring interleaved m2")
+    a = O.Chain(g["row_ptr"], g["col_idx"], g["class_ptr"], T, SEED); a.run(1, 2, 1, 1, 0)
+    b = O.Chain(g["row_ptr"], g["col_idx"], g["class_ptr"], T, SEED); b.run(1, 2, 1, 1, 1)
+    assert not np.array_equal(a.theta, b.theta)                   # genuinely another order
