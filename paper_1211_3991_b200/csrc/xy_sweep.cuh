@@ -592,7 +592,7 @@ __device__ __forceinline__ unsigned long long trace_now() {
 #endif
 
 template <int G, int CB, int MODE, int W>
-__global__ void __launch_bounds__(W * 32, kSmPerWarpSlots / W) k_phase(const SweepArgs a) {
+__global__ void __launch_bounds__(W * 32, W == 24 ? 1 : kSmPerWarpSlots / W) k_phase(const SweepArgs a) {
     extern __shared__ __align__(16) unsigned char s_raw[];
     SweepWarp *s_w = reinterpret_cast<SweepWarp *>(s_raw);
     __shared__ int s_last;
