@@ -135,3 +135,26 @@ def test_interleaved_equilibrium_config1_vs_oracle():
     z = np.abs(np.concatenate(zs))
     print(f"\ninterleaved config 1 vs oracle: {z.size} comparisons, max |z| {z.max():.2f}, > 3 sigma {int((z > 3).sum())}")
     assert z.max() < 4.5 and (z > 3).sum() <= 2
+
+
+def test_interleaved_full_size_config4_sampled_lockstep():
+    """BASELINE config 4 at full size in the launch configuration bench.py times: sampled sites of every colour class."""
+    w = workloads.CONFIGS[4]
+    g = levy.build(w.L, w.rho, w.z, w.seed, S=w.S)
+    T = w.temperatures()
+    ens = U.ensemble_from_levy(g, T, SEED); ens.set_order(1)
+    graphs = U.graphs_of_levy(g)
+    rng = np.random.default_rng(4)
+    ens.run(2, w.sweeps_per_swap, 1, 1)
+    tot = dict(updates=0, near=0, bad=0, illcond=0, accepted=0)
+    for c in range(int(g.n_colours.max())):
+        st = U.lockstep_metor(ens, graphs, T, SEED, c, 21, samples=[1, 6], site_subset=96, rng=rng)
+        assert st["bad"] == 0, st
+        for k in tot: tot[k] += st[k]
+    print(f"\n[interleaved full size cfg 4] {tot}")
+    assert tot["updates"] > 40000 and tot["near"] <= 5 + 2e-4 * tot["updates"]
+    E = ens.get_energy()
+    th = ens.get_theta()
+    Eo, _, _ = O.measure(g.row_ptr[1], g.col_idx[1], th[1])
+    assert np.all(np.abs(E[1] - Eo) <= 4e-7 * 3 * w.N)
+    ens.close()
