@@ -307,3 +307,26 @@ def test_degenerate_graphs_isolated_sites_and_unequal_colour_counts():
         Eo, _, _ = O.measure(gd["row_ptr"], gd["col_idx"], th[s])
         assert np.allclose(E[s], Eo, atol=1e-5)
     ens.close()
+
+
+@pytest.mark.parametrize("order", [0, 1])
+def test_checkpoint_resume_is_bit_identical(order):
+    """counter-based Philox makes (theta, labels, sweep, round) a complete restartable state:
+    run 2n cycles == run n cycles, save, restore into a NEW ensemble, run n cycles."""
+    g = small_levy(16, 3.5, 3, sample_base=4)
+    T = O.geometric_temperatures(16, 1.0, 4.0)
+    a = U.ensemble_from_levy(g, T, SEED, sample_base=4); a.set_order(order)
+    b = U.ensemble_from_levy(g, T, SEED, sample_base=4); b.set_order(order)
+    a.run(6, 5, 1, 2)
+    b.run(3, 5, 1, 2)
+    th, lab = b.get_theta(), b.get_labels()
+    sw, rd, _, _ = b.get_counters()
+    b.close()
+    c = U.ensemble_from_levy(g, T, SEED + 99, sample_base=4)      # wrong seed on purpose: only the key matters ...
+    c.close()
+    c = U.ensemble_from_levy(g, T, SEED, sample_base=4); c.set_order(order)
+    c.set_theta(th); c.set_labels(lab); c.set_counters(sw, rd)
+    c.run(3, 5, 1, 2)
+    assert np.array_equal(a.get_theta(), c.get_theta()) and np.array_equal(a.get_labels(), c.get_labels())
+    assert a.get_counters()[:2] == c.get_counters()[:2]
+    a.close(); c.close()
