@@ -1,5 +1,6 @@
-// xy_sweep.cuh -- the colour-class kernel k_phase<G, CB, MODE>: Metropolis / over-relaxation update of one colour
-// class, or the E / M reduction over all sites, for one group of samples.
+// xy_sweep.cuh -- the colour-class kernel k_phase<G, CB, MODE, W>: Metropolis and/or over-relaxation update of one
+// colour class (optionally with the E / M measurement as a by-product), or the stand-alone E / M reduction over all
+// sites, for one group of samples.
 //
 // Work layout: theta[S][N][R] fp32, replica fastest.  A lane owns TWO adjacent slots (one float2, one Philox4x32-10
 // call per site: words (x0,x1) feed the even slot, (x2,x3) the odd one), G = R/2 lanes cover a site (G = 32 and
@@ -9,17 +10,21 @@
 // (one contiguous CSR run) staged in the warp's slice of shared memory, pre-scaled by the site stride.  Same-colour
 // sites share no bond, so the gathers of row t+1 never read what row t stores: they are issued BEFORE
 // row t is computed, as cp.async (LDGSTS) copies of the lane's own 8 bytes into a per-warp ring in shared memory --
-// in-flight data costs no registers (64 per thread, 32 warps per SM, no spills), each lane reads back only what it
-// copied itself (cp.async.wait_group, no cross-lane synchronisation), and the Philox / sin / exp work of row t
-// covers the latency of row t+1.  When SPW > 1 the sites of a row have different degrees: the loops run to the row
-// maximum and lanes whose site has fewer neighbours are predicated off (no memory request is made for them).
+// in-flight data costs no registers (64 per thread and 32 warps per SM for the update modes, without spills; 80
+// registers and 24 warps for the modes that also measure), each lane reads back only what it copied itself
+// (cp.async.wait_group, no cross-lane synchronisation), and the Philox / sin / exp work of row t covers the latency
+// of row t+1.  When SPW > 1 the sites of a row have different degrees: the loops run to the row maximum and lanes
+// whose site has fewer neighbours are predicated off (no memory request is made for them).
+//
+// Modes: 0 Metropolis, 1 over-relaxation, 2 measure, 3 over-relaxation + measurement by-product, 4 Metropolis then
+// over-relaxation of the same site from one gather (interleaved order, xy_set_order), 5 = 4 + measurement by-product.
 //
 // The launches of a PT cycle are captured in a CUDA graph with PROGRAMMATIC DEPENDENT LAUNCH edges (see k_phase).
 // A persistent cooperative variant (all phases of a cycle in one launch, per-sample barriers) was built and measured
-// in round 1 and removed: it lost to the per-phase launches at every BASELINE config (DESIGN.md section 12).
+// in round 1 and removed: it lost to the per-phase launches at every BASELINE config (DESIGN.md 7.6).
 //
 // PAPER.md:444,:454 (coloured single-spin Metropolis), :460 (over-relaxation, ref 66), :167-181 (E, m),
-// :460-472 (parallel tempering); readings R5-R11 in DESIGN.md.
+// :460-472 (parallel tempering); readings R5-R11, R20 in DESIGN.md.
 #pragma once
 #include "xy_kernels.cuh"
 
