@@ -90,3 +90,17 @@ def test_workload_recipes():
     assert T[0] == 1.5 and abs(T[-1] - 4.0) < 1e-12 and np.allclose(T[1:] / T[:-1], (4.0 / 1.5) ** (1 / 63))
     assert np.allclose(O.geometric_temperatures(w.R, w.T_min, w.T_max), T, rtol=1e-15)
     assert workloads.lscan(64).L == 64 and workloads.lscan(64).R * workloads.lscan(64).S == 512
+
+
+def test_colour_count_within_the_papers_bound_at_z4():
+    """at z = 4 the number of colours is never larger than 6 for N <= 2^16 (tests/golden/paper_values.txt)."""
+    import os
+    bound = None
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "paper_values.txt")):
+        f = line.split()
+        if f and f[0] == "colours_max_z4":
+            bound = int(f[1])
+    assert bound == 6
+    for L, rho in ((64, 0.0), (64, 2.5), (128, 3.5), (64, 4.5), (256, 3.0)):
+        g = levy.build(L, rho, 4, 0x12113991, S=2)
+        assert int(g.n_colours.max()) <= bound, (L, rho, g.n_colours)

@@ -11,7 +11,16 @@ from paper_1211_3991_b200 import binding as B
 from paper_1211_3991_b200 import levy, workloads
 
 pytestmark = pytest.mark.gpu
-TC_ER_Z4 = 1.9361
+def paper_value(name):
+    import os
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "paper_values.txt")):
+        f = line.split()
+        if f and f[0] == name:
+            return float(f[1])
+    raise KeyError(name)
+
+
+TC_ER_Z4 = paper_value("tc_erdos_renyi_z4")          # 1.9361
 
 
 def binder(L, T, order):
