@@ -75,6 +75,7 @@ struct xy_graph {
     int32_t *class_ptr = nullptr;
     std::vector<int32_t> h_class_ptr;  // [S][q_stride]
     std::vector<uint32_t> h_deg;       // [S][N] degree | n_lower << 16 (host copy of rec.y, for the share tables)
+    std::vector<long long> h_off;      // [S+1] first col_idx entry of every sample
     size_t bytes_per_sample = 0;       // rec + col_idx (average), for the schedule heuristic
     int Lx = 0, Ly = 0;                // lattice extents of the site coordinates (0 = none set)
     uint32_t *coords = nullptr;        // [S][N] x | y << 16
@@ -126,7 +127,7 @@ struct xy_pt {
     int capacity_big = 0;            // co-resident 32-warp CTAs (one per SM)
     int cta_shape = 0;               // 0 = by class size, 1 = always 8-warp CTAs, 2 = always 32-warp CTAs
     int fuse_measure = 1;            // measured sweeps: the last over-relaxation sweep also produces E, Mx, My (MODE 3)
-    std::map<int, int32_t *> parts;  // warps per sample -> device [S][q_stride][nw + 1] cost-balanced share tables
+    std::map<int, int4 *> parts;     // warps per sample -> device [S][q_stride][nw] share tables {i0, w1, start0, n_run}
     int sweep_capacity = 0;          // co-resident CTAs of k_phase on this device: the grid is one such wave
     int measure_chunk = 256;  // sites per CTA of the generic measure kernel
     int samples_per_group = 0;  // 0 = automatic
@@ -168,16 +169,19 @@ xy::TileArgs tile_args(const xy_pt *pt, int colour, int s0) {
 // (and, at colour index q_max, of the measure pass over all sites), balanced by cost = const + degree.  Integer
 // bookkeeping only; the kernels give the same results for any partition (sites of a class are independent, the
 // measure sums are exact integers). ----
-int get_partition(xy_pt *pt, int nw, const int32_t **out) {
+int get_partition(xy_pt *pt, int nw, const int4 **out) {
     auto it = pt->parts.find(nw);
     if (it != pt->parts.end()) { *out = it->second; return XY_OK; }
     const xy_graph *g = pt->g;
     const int S = g->S, N = g->N, QS = g->q_stride;
-    std::vector<int32_t> h(static_cast<size_t>(S) * QS * (nw + 1));
-    std::vector<long long> pre(static_cast<size_t>(N) + 1);
+    std::vector<int4> h(static_cast<size_t>(S) * QS * nw);
+    std::vector<long long> pre(static_cast<size_t>(N) + 1), rowoff(static_cast<size_t>(N) + 1);
+    std::vector<int> cut(static_cast<size_t>(nw) + 1);
     for (int s = 0; s < S; ++s) {
         const uint32_t *dg = g->h_deg.data() + static_cast<size_t>(s) * N;
         const int32_t *cp = g->h_class_ptr.data() + static_cast<size_t>(s) * QS;
+        rowoff[0] = g->h_off[s];
+        for (int i = 0; i < N; ++i) rowoff[i + 1] = rowoff[i] + static_cast<long long>(dg[i] & 0xffffu);
         for (int c = 0; c < QS; ++c) {
             const bool meas = c == QS - 1;
             const int cbeg = meas ? 0 : cp[c], cend = meas ? N : cp[c + 1];
@@ -187,20 +191,30 @@ int get_partition(xy_pt *pt, int nw, const int32_t **out) {
                 pre[i - cbeg + 1] = pre[i - cbeg] + (meas ? 10 + nlow : 12 + deg);
             }
             const long long total = pre[cend - cbeg];
-            int32_t *row = h.data() + (static_cast<size_t>(s) * QS + c) * (nw + 1);
             int pos = 0;
             for (int k = 0; k <= nw; ++k) {
                 const long long target = (total * k + nw / 2) / nw;
                 while (pos < cend - cbeg && pre[pos] < target) ++pos;
-                row[k] = cbeg + pos;
+                cut[k] = cbeg + pos;
             }
-            row[0] = cbeg; row[nw] = cend;
+            cut[0] = cbeg; cut[nw] = cend;
+            int4 *row = h.data() + (static_cast<size_t>(s) * QS + c) * nw;
+            for (int k = 0; k < nw; ++k) {
+                // the share's first chunk as the kernel will cut it (chunk_fit): the longest prefix of <= 32 sites whose
+                // neighbour ids fit the staging slice -- so the ids can be staged without waiting for rec[]
+                const int i0 = cut[k], w1 = cut[k + 1];
+                const int nsite = std::min(32, w1 - i0);
+                int msite = 0;
+                while (msite < nsite && rowoff[i0 + msite + 1] - rowoff[i0] <= xy::kStageCap) ++msite;
+                const int n_run = msite > 0 ? static_cast<int>(rowoff[i0 + msite] - rowoff[i0]) : 0;
+                row[k] = make_int4(i0, w1, i0 < w1 ? static_cast<int>(rowoff[i0]) : 0, n_run);
+            }
         }
     }
-    int32_t *d = nullptr;
+    int4 *d = nullptr;
     const int rc = dev_alloc(&d, h.size());
     if (rc != XY_OK) return rc;
-    const cudaError_t e = cudaMemcpy(d, h.data(), h.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    const cudaError_t e = cudaMemcpy(d, h.data(), h.size() * sizeof(int4), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { cudaFree(d); return fail(XY_ECUDA, std::string("share table upload: ") + cudaGetErrorString(e)); }
     pt->parts[nw] = d;
     *out = d;
@@ -456,7 +470,7 @@ int prepare_partitions(xy_pt *pt, int group) {
         for (int c = 0; c <= g->q_max; ++c) {
             const int nmax = c == g->q_max ? g->N : max_class_size(g, c, s0, s1);
             if (nmax == 0) continue;
-            const int32_t *unused = nullptr;
+            const int4 *unused = nullptr;
             for (int mode : {0, 3}) {      // the update shapes and the measuring shape
                 if (c == g->q_max && mode == 3) continue;
                 const SweepGrid sg = sweep_grid(pt, s1 - s0, nmax, c == g->q_max ? 2 : mode);
@@ -575,6 +589,7 @@ int xy_graph_load(int S, int N, const int32_t *row_ptr, const int32_t *col_idx, 
         std::vector<int32_t> h_col(static_cast<size_t>(off[S]));   // neighbour lists, ascending per site
         g->h_class_ptr.assign(static_cast<size_t>(S) * g->q_stride, 0);
         g->h_deg.assign(static_cast<size_t>(S) * N, 0u);
+        g->h_off = off;
         for (int s = 0; s < S; ++s) {
             const int32_t *rp = row_ptr + static_cast<size_t>(s) * (N + 1);
             const int32_t *col = colour + static_cast<size_t>(s) * N;

@@ -223,8 +223,9 @@ __device__ __forceinline__ void sweep_consume(ACC &acc, const float2 *row0, int 
 // ---- arguments: the shared TileArgs plus the share table ---------------------------------------------------------
 struct SweepArgs {
     TileArgs t;
-    const int32_t *part;           // [S][q_stride][nw + 1] cost-balanced first site of every warp's share (colour q_max =
-                                   // the measure pass over all sites), nw = warps per sample and column block; nullptr = equal shares
+    const int4 *part;              // [S][q_stride][nw] per warp {first site, end site, first col_idx entry and number of
+                                   // staged ids of the share's first chunk}: cost-balanced shares (colour q_max = the
+                                   // measure pass over all sites), nw = warps per sample and column block; nullptr = equal shares
 };
 
 // per-thread constants of a launch
@@ -273,8 +274,13 @@ __device__ __forceinline__ PhasePrep sweep_prep(const SweepArgs &sa, const Sweep
     const int nw = gridDim.x * W, gw = blockIdx.x * W + x.warp;
     const int cidx = mode == kModeMeasure ? a.q_stride - 1 : colour;
     if (sa.part) {      // cost-balanced shares (host-computed: cost = const + degree)
-        const int32_t *pp = sa.part + (static_cast<size_t>(x.s) * a.q_stride + cidx) * (nw + 1) + gw;
-        P.i0 = pp[0]; P.w1 = pp[1];
+        const int4 e = __ldg(sa.part + (static_cast<size_t>(x.s) * a.q_stride + cidx) * nw + gw);
+        P.i0 = e.x; P.w1 = e.y;
+        if (P.i0 < P.w1) {      // rec[] and the ids of the first chunk in parallel: two dependent latencies, not three
+            if (x.lane < min(32, P.w1 - P.i0)) P.rc = x.rec[P.i0 + x.lane];
+            if (e.w > 0) chunk_stage(a.col_idx + e.z, x.sidx, x.lane, e.w, R2);
+        }
+        return P;
     } else {            // contiguous equal shares (whole rows)
         int cbeg = 0, cend = a.N;
         if (mode != kModeMeasure) {
