@@ -50,6 +50,15 @@ int xy_levy_build(int L, double rho, int z, uint64_t seed, uint32_t sample_base,
                   int n_threads, int32_t *row_ptr, int32_t *col_idx, int32_t *colour,
                   int32_t *new_to_old, int32_t *n_colours, int64_t *n_draws);
 
+/* The same with FREE boundary conditions (Fig. 14: bond lengths up to L sqrt 2 instead of
+ * [L/2] sqrt 2): plain Euclidean distance on the open L x L lattice.  A bond is drawn by choosing i uniformly and a
+ * displacement (dx, dy) in [-(L-1), L-1]^2 \ {0} with P ~ |d|^-rho (one fp64 CDF summed in index order
+ * d = (dy+L-1)(2L-1) + (dx+L-1)); a partner outside the lattice or a duplicate bond discards the whole draw, so the
+ * accepted bonds are distributed ~ r_ij^-rho over the pairs that exist (DESIGN R21).  L <= 2048. */
+int xy_levy_build_fbc(int L, double rho, int z, uint64_t seed, uint32_t sample_base, int S,
+                  int n_threads, int32_t *row_ptr, int32_t *col_idx, int32_t *colour,
+                  int32_t *new_to_old, int32_t *n_colours, int64_t *n_draws);
+
 /* Smallest-last greedy colouring of any symmetric CSR graph; returns Q (>= 0) or a negative error. */
 int xy_colour_smallest_last(int N, const int32_t *row_ptr, const int32_t *col_idx,
                             int32_t *colour /*[N]*/);

@@ -37,6 +37,8 @@ def lib():
         L.orc_levy_edges.argtypes = [C.c_int, C.c_double, C.c_int, C.c_uint64, C.c_uint32, _i32p,
                                      C.c_int64]
         L.orc_levy_edges.restype = C.c_int64
+        L.orc_levy_edges_fbc.argtypes = L.orc_levy_edges.argtypes
+        L.orc_levy_edges_fbc.restype = C.c_int64
         L.orc_csr_from_edges.argtypes = [C.c_int, C.c_int, _i32p, _i32p, _i32p]
         L.orc_csr_from_edges.restype = None
         L.orc_colour_smallest_last.argtypes = [C.c_int, _i32p, _i32p, _i32p]
@@ -107,10 +109,11 @@ def slot_uniforms(seed, domain, site, sweep, sample, slot):
     return a.value, b.value
 
 
-def levy_edges(L, rho, z, seed, sample, max_draws=1 << 40):
+def levy_edges(L, rho, z, seed, sample, max_draws=1 << 40, boundary="periodic"):
     N = L * L
     edges = np.zeros((N * z // 2, 2), np.int32)
-    draws = lib().orc_levy_edges(L, float(rho), z, seed, sample, edges, max_draws)
+    fn = lib().orc_levy_edges if boundary == "periodic" else lib().orc_levy_edges_fbc
+    draws = fn(L, float(rho), z, seed, sample, edges, max_draws)
     if draws < 0:
         raise RuntimeError("orc_levy_edges failed")
     return edges, int(draws)

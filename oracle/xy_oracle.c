@@ -137,6 +137,56 @@ int64_t orc_levy_edges(int L, double rho, int z, uint64_t seed, uint32_t sample,
     return k;
 }
 
+/* Free boundary conditions ("r up to L sqrt 2"; DESIGN R21), definition level: site i uniform;
+ * displacement (dx, dy) in [-(L-1), L-1]^2 without the null vector, P ~ (dx^2 + dy^2)^(-rho/2), by a linear scan of
+ * the cumulative sum in index order d = (dy+L-1)(2L-1) + (dx+L-1); partner outside the lattice or duplicate bond:
+ * the whole draw is discarded. */
+int64_t orc_levy_edges_fbc(int L, double rho, int z, uint64_t seed, uint32_t sample, int32_t *edges,
+                           int64_t max_draws) {
+    const int N = L * L, W = 2 * L - 1;
+    const int64_t n_bonds = (int64_t)N * z / 2;
+    if (N > 16384 || ((int64_t)N * z) % 2 != 0) return -1;
+    uint8_t *present = (uint8_t *)calloc(((size_t)N * N + 7) / 8, 1);
+    if (!present) return -1;
+    double total = 0.0;
+    for (int d = 0; d < W * W; ++d) {
+        const int dx = d % W - (L - 1), dy = d / W - (L - 1);
+        if (dx != 0 || dy != 0) total += pow((double)(dx * dx + dy * dy), -0.5 * rho);
+    }
+    uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    int64_t have = 0, k = 0;
+    while (have < n_bonds) {
+        if (k >= max_draws) { free(present); return -1; }
+        uint32_t ctr[4] = {(uint32_t)k, (uint32_t)((uint64_t)k >> 32), sample, ORC_DOMAIN_GRAPH};
+        uint32_t x[4];
+        orc_philox4x32_10(ctr, key, x);
+        ++k;
+        int i = (int)(((uint64_t)x[0] * (uint64_t)N) >> 32);
+        uint64_t m53 = ((uint64_t)x[1] << 21) | ((uint64_t)x[2] >> 11);
+        double target = (((double)m53 + 0.5) * 1.1102230246251565e-16) * total;
+        double run = 0.0;
+        int d = W * W - 1;
+        for (int dd = 0; dd < W * W; ++dd) {
+            const int dx = dd % W - (L - 1), dy = dd / W - (L - 1);
+            if (dx != 0 || dy != 0) run += pow((double)(dx * dx + dy * dy), -0.5 * rho);
+            if (run > target) { d = dd; break; }
+        }
+        int xi = i % L, yi = i / L;
+        int xj = xi + d % W - (L - 1), yj = yi + d / W - (L - 1);
+        if (xj < 0 || xj >= L || yj < 0 || yj >= L || (xj == xi && yj == yi)) continue;
+        int j = yj * L + xj;
+        int a = i < j ? i : j, b = i < j ? j : i;
+        size_t bit = (size_t)a * N + b;
+        if (present[bit >> 3] & (1u << (bit & 7))) continue;
+        present[bit >> 3] |= (uint8_t)(1u << (bit & 7));
+        edges[2 * have] = i;
+        edges[2 * have + 1] = j;
+        ++have;
+    }
+    free(present);
+    return k;
+}
+
 void orc_csr_from_edges(int N, int n_edges, const int32_t *edges, int32_t *row_ptr,
                         int32_t *col_idx) {
     if (N <= 0) return;

@@ -43,6 +43,9 @@ void orc_slot_uniforms(uint64_t seed, uint32_t domain, uint32_t site, uint32_t s
 /* returns number of Philox draws consumed (>=E_b) or -1 on failure; edges[2*e], edges[2*e+1] */
 int64_t orc_levy_edges(int L, double rho, int z, uint64_t seed, uint32_t sample,
                        int32_t *edges /*[N*z/2][2]*/, int64_t max_draws);
+/* free boundary conditions (DESIGN R21): plain Euclidean distance on the open lattice */
+int64_t orc_levy_edges_fbc(int L, double rho, int z, uint64_t seed, uint32_t sample,
+                           int32_t *edges /*[N*z/2][2]*/, int64_t max_draws);
 /* symmetric CSR with ascending neighbour lists from an edge list */
 void orc_csr_from_edges(int N, int n_edges, const int32_t *edges, int32_t *row_ptr /*[N+1]*/,
                         int32_t *col_idx /*[2*n_edges]*/);

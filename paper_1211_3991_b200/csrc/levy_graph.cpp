@@ -149,7 +149,25 @@ void renumber(int N, const int32_t *row_ptr, const int32_t *col_idx, const int32
 struct Cdf {
     std::vector<double> run;  // run[d] = sum_{d'=1..d} w_d', run[0] = 0
     double total = 0.0;
+    bool fbc = false;         // free boundaries: displacements (dx, dy) in [-(L-1), L-1]^2, plain Euclidean distance
 };
+
+// free boundary conditions (r up to L sqrt 2): run[] over the (2L-1)^2 displacement vectors in index
+// order d = (dy + L-1)(2L-1) + (dx + L-1) + 1, the null vector has weight 0 (DESIGN R21)
+Cdf make_cdf_fbc(int L, double rho) {
+    const int W = 2 * L - 1;
+    Cdf c;
+    c.fbc = true;
+    c.run.assign(static_cast<size_t>(W) * W + 1, 0.0);
+    double s = 0.0;
+    for (int d = 0; d < W * W; ++d) {
+        const int dx = d % W - (L - 1), dy = d / W - (L - 1);
+        if (dx != 0 || dy != 0) s += std::pow(static_cast<double>(dx * dx + dy * dy), -0.5 * rho);
+        c.run[static_cast<size_t>(d) + 1] = s;
+    }
+    c.total = s;
+    return c;
+}
 
 Cdf make_cdf(int L, double rho) {
     const int N = L * L;
@@ -185,11 +203,23 @@ int build_one(int L, int z, uint64_t seed, uint32_t sample, const Cdf &cdf, int3
         const int i = static_cast<int>((static_cast<uint64_t>(x[0]) * static_cast<uint64_t>(N)) >> 32);
         const uint64_t m53 = (static_cast<uint64_t>(x[1]) << 21) | (static_cast<uint64_t>(x[2]) >> 11);
         const double target = ((static_cast<double>(m53) + 0.5) * 1.1102230246251565e-16) * cdf.total;
-        // first d in [1, N-1] with run[d] > target
-        int d = static_cast<int>(std::upper_bound(cdf.run.begin() + 1, cdf.run.end(), target) - cdf.run.begin());
-        if (d > N - 1) d = N - 1;
         const int xi = i % L, yi = i / L;
-        const int j = ((yi + d / L) % L) * L + (xi + d % L) % L;
+        int j;
+        if (cdf.fbc) {
+            // first d in [1, W^2] with run[d] > target; displacement index d - 1; a partner outside the lattice
+            // discards the whole draw (pairs are drawn with P ~ r^-rho among the pairs that exist)
+            const int W = 2 * L - 1;
+            int d = static_cast<int>(std::upper_bound(cdf.run.begin() + 1, cdf.run.end(), target) - cdf.run.begin());
+            if (d > W * W) d = W * W;
+            const int xj = xi + (d - 1) % W - (L - 1), yj = yi + (d - 1) / W - (L - 1);
+            if (xj < 0 || xj >= L || yj < 0 || yj >= L || (xj == xi && yj == yi)) continue;
+            j = yj * L + xj;
+        } else {
+            // first d in [1, N-1] with run[d] > target
+            int d = static_cast<int>(std::upper_bound(cdf.run.begin() + 1, cdf.run.end(), target) - cdf.run.begin());
+            if (d > N - 1) d = N - 1;
+            j = ((yi + d / L) % L) * L + (xi + d % L) % L;
+        }
         if (!present.insert(static_cast<uint32_t>(i), static_cast<uint32_t>(j))) continue;
         bonds.emplace_back(i, j);
     }
@@ -216,9 +246,9 @@ extern "C" {
 
 const char *xy_levy_last_error(void) { return g_err.c_str(); }
 
-int xy_levy_build(int L, double rho, int z, uint64_t seed, uint32_t sample_base, int S, int n_threads,
-                  int32_t *row_ptr, int32_t *col_idx, int32_t *colour, int32_t *new_to_old,
-                  int32_t *n_colours, int64_t *n_draws) {
+static int levy_build_impl(bool fbc, int L, double rho, int z, uint64_t seed, uint32_t sample_base, int S, int n_threads,
+                           int32_t *row_ptr, int32_t *col_idx, int32_t *colour, int32_t *new_to_old,
+                           int32_t *n_colours, int64_t *n_draws) {
     try {
         if (L < 2 || L > 16384 || z < 1 || S < 0 || !(rho >= 0.0) || !std::isfinite(rho))
             return fail(XY_LEVY_EINVAL, "need 2 <= L <= 16384, z >= 1, S >= 0, finite rho >= 0");
@@ -227,7 +257,8 @@ int xy_levy_build(int L, double rho, int z, uint64_t seed, uint32_t sample_base,
         if (N * z / 2 > N * (N - 1) / 2) return fail(XY_LEVY_EINVAL, "more bonds than pairs");
         if (N * z > 0x7fffffffll) return fail(XY_LEVY_EINVAL, "nnz exceeds int32");
         if (S > 0 && (!row_ptr || !col_idx || !colour)) return fail(XY_LEVY_EINVAL, "null output array");
-        const Cdf cdf = make_cdf(L, rho);
+        if (fbc && L > 2048) return fail(XY_LEVY_EINVAL, "free boundaries: L <= 2048");
+        const Cdf cdf = fbc ? make_cdf_fbc(L, rho) : make_cdf(L, rho);
         if (!(cdf.total > 0.0) || !std::isfinite(cdf.total)) return fail(XY_LEVY_EINVAL, "degenerate weights");
         int nt = n_threads > 0 ? n_threads : static_cast<int>(std::thread::hardware_concurrency());
         nt = std::max(1, std::min(nt, S));
@@ -266,6 +297,20 @@ int xy_levy_build(int L, double rho, int z, uint64_t seed, uint32_t sample_base,
     } catch (...) {
         return fail(XY_LEVY_EINVAL, "unexpected exception");
     }
+}
+
+int xy_levy_build(int L, double rho, int z, uint64_t seed, uint32_t sample_base, int S, int n_threads,
+                  int32_t *row_ptr, int32_t *col_idx, int32_t *colour, int32_t *new_to_old,
+                  int32_t *n_colours, int64_t *n_draws) {
+    return levy_build_impl(false, L, rho, z, seed, sample_base, S, n_threads, row_ptr, col_idx, colour, new_to_old,
+                           n_colours, n_draws);
+}
+
+int xy_levy_build_fbc(int L, double rho, int z, uint64_t seed, uint32_t sample_base, int S, int n_threads,
+                      int32_t *row_ptr, int32_t *col_idx, int32_t *colour, int32_t *new_to_old,
+                      int32_t *n_colours, int64_t *n_draws) {
+    return levy_build_impl(true, L, rho, z, seed, sample_base, S, n_threads, row_ptr, col_idx, colour, new_to_old,
+                           n_colours, n_draws);
 }
 
 int xy_colour_smallest_last(int N, const int32_t *row_ptr, const int32_t *col_idx, int32_t *colour) {

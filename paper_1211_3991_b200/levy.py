@@ -21,6 +21,8 @@ def lib():
         L.xy_levy_build.argtypes = [C.c_int, C.c_double, C.c_int, C.c_uint64, C.c_uint32, C.c_int, C.c_int,
                                     _i32p, _i32p, _i32p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.xy_levy_build.restype = C.c_int
+        L.xy_levy_build_fbc.argtypes = L.xy_levy_build.argtypes
+        L.xy_levy_build_fbc.restype = C.c_int
         L.xy_colour_smallest_last.argtypes = [C.c_int, _i32p, _i32p, _i32p]
         L.xy_colour_smallest_last.restype = C.c_int
         L.xy_renumber_colour_major.argtypes = [C.c_int, _i32p, _i32p, _i32p, _i32p, _i32p, _i32p, _i32p]
@@ -62,7 +64,7 @@ class LevyGraphs:
         return np.searchsorted(self.colour[s], np.arange(Q + 1)).astype(np.int32)
 
 
-def build(L, rho, z, seed, S=1, sample_base=0, n_threads=0):
+def build(L, rho, z, seed, S=1, sample_base=0, n_threads=0, boundary="periodic"):
     N = L * L
     row_ptr = np.zeros((S, N + 1), np.int32)
     col_idx = np.zeros((S, N * z), np.int32)
@@ -70,7 +72,10 @@ def build(L, rho, z, seed, S=1, sample_base=0, n_threads=0):
     n2o = np.zeros((S, N), np.int32)
     nq = np.zeros(S, np.int32)
     nd = np.zeros(S, np.int64)
-    rc = lib().xy_levy_build(L, float(rho), z, seed, sample_base, S, n_threads, row_ptr.reshape(-1),
+    fn = lib().xy_levy_build if boundary == "periodic" else lib().xy_levy_build_fbc
+    if boundary not in ("periodic", "free"):
+        raise ValueError("boundary must be 'periodic' or 'free'")
+    rc = fn(L, float(rho), z, seed, sample_base, S, n_threads, row_ptr.reshape(-1),
                              col_idx.reshape(-1), colour.reshape(-1), n2o.ctypes.data, nq.ctypes.data,
                              nd.ctypes.data)
     if rc != 0:

@@ -104,3 +104,44 @@ def test_colour_count_within_the_papers_bound_at_z4():
     for L, rho in ((64, 0.0), (64, 2.5), (128, 3.5), (64, 4.5), (256, 3.0)):
         g = levy.build(L, rho, 4, 0x12113991, S=2)
         assert int(g.n_colours.max()) <= bound, (L, rho, g.n_colours)
+
+
+@pytest.mark.parametrize("L,rho,z,sample", [(8, 3.5, 6, 0), (16, 3.5, 6, 3), (12, 0.0, 4, 1), (16, 4.5, 4, 0)])
+def test_free_boundary_builder_matches_oracle_bit_exact(L, rho, z, sample):
+    N = L * L
+    g = levy.build(L, rho, z, SEED, S=1, sample_base=sample, boundary="free")
+    edges, draws = O.levy_edges(L, rho, z, SEED, sample, boundary="free")
+    rp, ci = O.csr_from_edges(N, edges)
+    colour, Q = O.colour_smallest_last(rp, ci)
+    n2o, rp2, ci2, c2 = O.renumber_colour_major(rp, ci, colour)
+    assert int(g.n_draws[0]) == draws and int(g.n_colours[0]) == Q
+    assert np.array_equal(g.new_to_old[0], n2o)
+    assert np.array_equal(g.row_ptr[0], rp2) and np.array_equal(g.col_idx[0], ci2) and np.array_equal(g.colour[0], c2)
+
+
+def test_free_boundary_structure():
+    """with free boundaries bonds reach beyond [L/2] sqrt 2 (up to L sqrt 2) and never wrap; the
+    bond-length law is ~ (number of pairs at that displacement) r^-rho; border sites have fewer bonds."""
+    L, rho, z = 32, 3.0, 6
+    g = levy.build(L, rho, z, SEED, S=8, boundary="free")
+    cnt = {}
+    for s in range(g.S):
+        rp, ci, lat = g.row_ptr[s], g.col_idx[s], g.new_to_old[s]
+        assert rp[-1] == L * L * z and O.colouring_is_proper(rp, ci, g.colour[s])
+        x, y = lat % L, lat // L
+        src = np.repeat(np.arange(L * L), np.diff(rp))
+        dx, dy = np.abs(x[src] - x[ci]), np.abs(y[src] - y[ci])
+        assert np.hypot(dx, dy).max() <= (L - 1) * np.sqrt(2) + 1e-9
+        for a, b in zip(dx, dy):
+            cnt[(a, b)] = cnt.get((a, b), 0) + 1
+        deg = np.diff(rp)
+        border = (x == 0) | (x == L - 1) | (y == 0) | (y == L - 1)
+        assert deg[border].mean() < deg[~border].mean()
+    assert max(np.hypot(a, b) for (a, b) in cnt) > (L // 2) * np.sqrt(2)        # longer than any periodic bond
+    # away from the saturated nearest-neighbour shell (bonds are drawn without replacement) the counts follow
+    # (number of pairs) r^-rho: displacement (3,0)+(0,3) against (4,0)+(0,4)
+    n3 = cnt[(3, 0)] + cnt[(0, 3)]; n4 = cnt[(4, 0)] + cnt[(0, 4)]
+    expect = ((L - 3) * 3.0 ** -rho) / ((L - 4) * 4.0 ** -rho)
+    assert abs(n3 / n4 - expect) < 0.25 * expect, (n3, n4, expect)
+    with pytest.raises(ValueError):
+        levy.build(8, 3.0, 6, SEED, boundary="helical")
