@@ -367,6 +367,7 @@ def main():
     else:
         ens.close()
     if world > 1:
+        dist.barrier()          # rank 0 may still be in its auxiliary measurements
         dist.destroy_process_group()
 
 
