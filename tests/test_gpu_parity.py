@@ -330,3 +330,79 @@ def test_checkpoint_resume_is_bit_identical(order):
     assert np.array_equal(a.get_theta(), c.get_theta()) and np.array_equal(a.get_labels(), c.get_labels())
     assert a.get_counters()[:2] == c.get_counters()[:2]
     a.close(); c.close()
+
+
+@pytest.mark.parametrize("R", [8, 64, 2])
+def test_hub_with_more_neighbours_than_the_staging_slice(R):
+    """a site whose degree (300, then 700) exceeds the 256 staged neighbour ids takes the block-wise path of the kernel:
+    Metropolis, over-relaxation, interleaved and measure parity on a star-with-chords graph; also R = 1024 slots."""
+    for n_leaves in (300, 700):
+        N = n_leaves + 1
+        edges = [(0, k) for k in range(1, N)] + [(k, k + 1) for k in range(1, N - 1, 2)]      # hub + a matching of the leaves
+        gd = G.colour_major(N, edges)
+        T = O.geometric_temperatures(R, 0.8, 3.0)
+        ens = U.ensemble_from_graph(gd, T, SEED, S=2)
+        graphs = [(gd["row_ptr"], gd["col_idx"], gd["class_ptr"])] * 2
+        Q = len(gd["class_ptr"]) - 1
+        deg = np.diff(gd["row_ptr"])
+
+        def overrelax_ok(c, interleaved, sweep):
+            """R7 with the field error written out: |dtheta| |h| <= 2 eps_h, eps_h = z 2^-21.4 (fast sincos), which is
+            the 1e-5 bar for the degrees of the BASELINE graphs (z <= 19) and scales with z for the hub."""
+            pre = ens.get_theta(); labels = ens.get_labels()
+            ens.metor_colour(c, sweep) if interleaved else ens.overrelax_colour(c)
+            post = ens.get_theta()
+            lo, hi = int(gd["class_ptr"][c]), int(gd["class_ptr"][c + 1])
+            sites = np.arange(lo, hi, dtype=np.int32)
+            for s in range(2):
+                ref = pre[s].copy()
+                near = np.zeros((len(sites), R), bool)
+                if interleaved:
+                    bs, ws = U.slot_params(T, labels[s])
+                    m, _ = O.metropolis_sites(gd["row_ptr"], gd["col_idx"], ref, sites, bs, ws, SEED, sweep, s, want_margin=True)
+                    near = m < U.BAND
+                hn = O.overrelax_sites(gd["row_ptr"], gd["col_idx"], ref, sites, want_hnorm=True)
+                err = U.circ(post[s, sites], ref[sites])
+                bar = np.maximum(1e-5, 2.0 * deg[sites] * 2.0 ** -21.4)[:, None]
+                assert np.all((err * np.minimum(1.0, hn) <= 1e-5) | (err * hn <= bar) | near), (c, s, float((err * hn).max()))
+
+        for sweep in (1, 2):
+            for c in range(Q):
+                assert U.lockstep_metropolis(ens, graphs, T, SEED, c, sweep)["bad"] == 0
+            for c in range(Q):
+                overrelax_ok(c, False, 0)
+            for c in range(Q):
+                overrelax_ok(c, True, sweep + 10)
+        out = ens.measure(want=True)
+        th = ens.get_theta(); lab = ens.get_labels()
+        for s in range(2):
+            E, Mx, My = O.measure(gd["row_ptr"], gd["col_idx"], th[s])
+            assert np.all(np.abs(out[s, lab[s], 0] - E) <= 4e-7 * len(edges) + 1e-4)
+            assert np.all(np.abs(out[s, lab[s], 1] - Mx) <= 2e-7 * N + 1e-5)
+        a = ens.read_accumulators().copy()
+        ens.run(2, 3, 1, 1)                                            # fused measurement on the same graph
+        E2 = ens.get_energy(); th = ens.get_theta()
+        for s in range(2):
+            E, _, _ = O.measure(gd["row_ptr"], gd["col_idx"], th[s])
+            assert np.all(np.abs(E2[s] - E) <= 4e-7 * len(edges) + 1e-4)
+        assert np.all(ens.read_accumulators()[..., 0] == a[..., 0] + 6)
+        ens.close()
+
+
+def test_thousand_replicas_sixteen_column_blocks():
+    g = small_levy(8, 3.5, 1)
+    R = 1024
+    T = O.geometric_temperatures(R, 1.0, 4.0)
+    ens = U.ensemble_from_levy(g, T, SEED)
+    assert np.array_equal(ens.get_theta()[0], O.init_theta(64, R, SEED, 0))
+    graphs = U.graphs_of_levy(g)
+    for c in range(int(g.n_colours.max())):
+        assert U.lockstep_metropolis(ens, graphs, T, SEED, c, 1)["bad"] == 0
+        assert U.lockstep_metor(ens, graphs, T, SEED, c, 2)["bad"] == 0
+    ens.run(2, 3, 1, 1)
+    E = ens.get_energy()[0]
+    Eo, _, _ = O.measure(g.row_ptr[0], g.col_idx[0], ens.get_theta()[0])
+    assert np.all(np.abs(E - Eo) <= 4e-7 * 192 + 1e-5)
+    with pytest.raises(B.XYError):
+        U.ensemble_from_levy(g, O.geometric_temperatures(1025, 1.0, 4.0), SEED)
+    ens.close()
