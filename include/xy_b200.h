@@ -32,6 +32,7 @@
  */
 #ifndef XY_B200_H
 #define XY_B200_H
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -79,6 +80,10 @@ int xy_graph_set_coords(xy_graph *g, int Lx, int Ly, const int32_t *x /*host*/, 
  * bit-exact against the oracle.  Runs on `stream` (cudaStream_t as void*, NULL = default) and synchronises it. */
 int xy_random_walk(const xy_graph *g, int n_walkers, const int32_t *start /*host*/, int n_steps, uint64_t seed,
                    uint32_t sample_base, void *stream, int64_t *hist_host);
+
+/* Device time in microseconds of the k_random_walk launch of the calling thread's last successful xy_random_walk call
+ * (CUDA events around the kernel alone, on that call's stream: no allocation, no copy).  XY_ESTATE if there was none. */
+int xy_random_walk_kernel_us(double *us_out);
 
 /* ---- PT ensemble ----
  * T [R] host, strictly positive, ascending (T = +inf allowed: beta = 0).  width [R] host or NULL;
@@ -130,6 +135,23 @@ int xy_run_sweeps(xy_pt *pt, int n_blocks, int sweeps_per_block, int or_per_swee
  * are bit-identical for every value.  0 = automatic (default), S = all samples per launch. */
 int xy_set_schedule(xy_pt *pt, int samples_per_group);
 
+/* Execution path of xy_run / xy_run_sweeps ("subsets ... processed sequentially on
+ * each MCS").  1 = one launch per colour class (k_phase) captured in a CUDA graph with programmatic-dependent-launch
+ * edges: right when a class fills the chip.  2 = one THREAD-BLOCK CLUSTER per sample (k_cycle): all colour classes of all
+ * sweeps of all requested cycles, the fused measurement and the swap round run in ONE launch, the classes separated by
+ * the hardware cluster barrier -- right when a class is a few hundred rows and a launch is latency-bound; needs
+ * R = 2 * 2^k <= 64, or_per_sweep >= 1 and fused measurement (else XY_ESTATE from xy_set_path / xy_run).  0 (default) =
+ * automatic: path 2 where it applies and the samples are small, else path 1.  Both paths give bit-identical angles,
+ * labels, accumulators and counters.  xy_get_path reports what xy_run(or_per_sweep) would use (1 or 2) and the cluster
+ * size (CTAs per sample; 0 for path 1); either output may be NULL. */
+int xy_set_path(xy_pt *pt, int path);
+int xy_get_path(xy_pt *pt, int or_per_sweep, int *path, int *cluster_size);
+
+/* The schedule in force: samples per launch group, and the bytes one group keeps live (its angles + its share of the
+ * graph tables) -- a group that fits the 126 MB L2 is served from L2 after the first sweep of a cycle.  Either output
+ * may be NULL. */
+int xy_get_schedule(xy_pt *pt, int *samples_per_group, int64_t *group_bytes);
+
 /* Tuning switches of the float2 kernel flavours (R = 2 * 2^k <= 64, R % 64 == 0); results are bit-identical for
  * every setting (tests/test_gpu_parity.py).  balance != 0: cost-balanced shares of a colour class per warp (default),
  * 0: equal shares.  pdl != 0: programmatic-dependent-launch edges between the colour-class launches (default).
@@ -161,6 +183,12 @@ int xy_metor_colour(xy_pt *pt, int colour, uint32_t sweep);
 /* ---- state access (all synchronise the stream) ---- */
 int xy_get_theta(xy_pt *pt, float *theta_host /*[S][N][R]*/);
 int xy_set_theta(xy_pt *pt, const float *theta_host /*[S][N][R]*/);
+/* Asynchronous upload of the whole state from PINNED host memory (cudaHostAlloc / torch pin_memory), one copy per sample
+ * group of the current schedule on a second stream owned by the handle; returns at once.  theta_host must stay valid
+ * and unchanged until the handle's stream has been synchronised.  The next xy_run orders each sample group's first
+ * launch after that group's copy only (samples never interact, Eq. 12), so the upload of group g+1 overlaps
+ * the sweeps of group g; every other call waits for the whole upload first.  Results are those of xy_set_theta. */
+int xy_set_theta_async(xy_pt *pt, const float *theta_host /*[S][N][R], pinned*/);
 int xy_get_labels(xy_pt *pt, int32_t *temp_of_slot_host /*[S][R]*/);
 int xy_set_labels(xy_pt *pt, const int32_t *temp_of_slot_host /*[S][R], a permutation per sample*/);
 /* energies per memory slot [S][R] (recomputed if stale; accumulators untouched) */
@@ -180,6 +208,15 @@ int xy_theta_device(xy_pt *pt, float **theta_dev);
 /* number of kernel launches (graph kernel nodes included) issued by this handle so far */
 int xy_launch_count(xy_pt *pt, int64_t *n_launches);
 int xy_synchronize(xy_pt *pt);
+
+/* ---- diagnostic: L2 bandwidth of this GPU (the roofline denominator when a sample group is L2-resident; BASELINE.json
+ * north_star "or L2 GB/s when the state fits in the 126 MB L2") ----
+ * Allocates a zero-filled buffer of `bytes` (1 MiB .. 4 GiB; 32 MiB is the survey's choice, well inside L2), and times
+ * `repeats` launches (CUDA events on `stream`, after two warm-up launches) of a hand-written read kernel that goes
+ * through the buffer 16 times with L1 bypassed: mode 0 = linear stream of 16-byte loads, mode 1 = random aligned
+ * 256-byte rows, 8 bytes per lane (the request shape of the neighbour gather at R = 64).  *gbs_out = the best launch's
+ * bytes read / time in GB/s.  Runs on the current device; synchronises `stream`; frees everything it allocated. */
+int xy_l2_bandwidth(size_t bytes, int mode, int repeats, void *stream /*cudaStream_t or NULL*/, double *gbs_out /*host*/);
 
 #ifdef __cplusplus
 }

@@ -3,7 +3,7 @@
   libxy_levy.so   host-only Levy-graph builder / colouring   (g++)
   libxy_b200.so   the C-ABI hot-path library, sm_100a only   (nvcc -gencode arch=compute_100a,code=sm_100a)
 
-Both are rebuilt only when a source is newer than the library.  __graft_entry__.build() calls
+Both are rebuilt only when a source is newer than the library (libxy_b200.so: per translation unit, objects in build/).  __graft_entry__.build() calls
 build_all(); the bindings call the per-library functions lazily and fail loudly if a build fails.
 """
 import os
@@ -57,14 +57,36 @@ def nvcc_path():
 
 
 def build_xy(force=False, verbose=False, extra_flags=()):
-    src = [os.path.join(CSRC, "xy_b200.cu")]
-    deps = _sources([(CSRC, (".cu", ".cuh", ".h")), (INCLUDE, (".h",))])
-    if force or _stale(XY_LIB, deps):
-        cmd = [nvcc_path(), *NVCC_ARCH, "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC",
-               "-shared", "-Xptxas", "-v" if verbose else "-O3", "-I", INCLUDE, "-I", CSRC,
-               *extra_flags, *src, "-o", XY_LIB, "-lcudart"]
+    """nvcc every csrc/*.cu into build/*.o (in parallel: the kernel instantiations are spread over xy_inst_*.cu so that
+    they compile side by side) and link libxy_b200.so.  An object is rebuilt when its source or any header is newer."""
+    from concurrent.futures import ThreadPoolExecutor
+    srcs = _sources([(CSRC, (".cu",))])
+    hdrs = _sources([(CSRC, (".cuh", ".h")), (INCLUDE, (".h",))])
+    objdir = os.path.join(PKG, "build")
+    os.makedirs(objdir, exist_ok=True)
+    nvcc = nvcc_path()
+    flags = [*NVCC_ARCH, "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v" if verbose else "-O3",
+             "-I", INCLUDE, "-I", CSRC, *extra_flags]
+
+    def compile_one(src):
+        obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
+        if force or _stale(obj, [src, *hdrs]):
+            cmd = [nvcc, *flags, "-c", src, "-o", obj]
+            if verbose:
+                print(" ".join(cmd), flush=True)
+            r = subprocess.run(cmd, capture_output=True, text=True)
+            if verbose or r.returncode != 0:
+                print(r.stdout + r.stderr, flush=True)
+            if r.returncode != 0:
+                raise RuntimeError(f"nvcc failed on {src}")
+        return obj
+
+    with ThreadPoolExecutor(max_workers=max(1, min(len(srcs), os.cpu_count() or 1))) as pool:
+        objs = list(pool.map(compile_one, srcs))
+    if force or _stale(XY_LIB, objs):
+        cmd = [nvcc, *NVCC_ARCH, "-shared", *objs, "-o", XY_LIB, "-lcudart"]
         if verbose:
-            print(" ".join(cmd))
+            print(" ".join(cmd), flush=True)
         subprocess.run(cmd, check=True)
     return XY_LIB
 

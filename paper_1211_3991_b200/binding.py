@@ -5,7 +5,6 @@ memory (the theta tensor) and the CUDA stream, nothing else.  There is no CPU fa
 cannot be built or loaded, or no CUDA device is present, the calls raise.
 """
 import ctypes as C
-import os
 
 import numpy as np
 
@@ -26,6 +25,10 @@ SYMBOLS = {
     "xy_measure_fourier": (C.c_int, [C.c_void_p, C.c_void_p]),
     "xy_read_fourier_accumulators": (C.c_int, [C.c_void_p, C.c_void_p]),
     "xy_random_walk": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_uint64, C.c_uint32, C.c_void_p, C.c_void_p]),
+    "xy_random_walk_kernel_us": (C.c_int, [C.POINTER(C.c_double)]),
+    "xy_set_path": (C.c_int, [C.c_void_p, C.c_int]),
+    "xy_get_path": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)]),
+    "xy_get_schedule": (C.c_int, [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int64)]),
     "xy_graph_info": (C.c_int, [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int64),
                                 C.POINTER(C.c_int), C.POINTER(C.c_int)]),
     "xy_pt_create": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_void_p,
@@ -45,6 +48,7 @@ SYMBOLS = {
     "xy_set_order": (C.c_int, [C.c_void_p, C.c_int]),
     "xy_get_theta": (C.c_int, [C.c_void_p, C.c_void_p]),
     "xy_set_theta": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "xy_set_theta_async": (C.c_int, [C.c_void_p, C.c_void_p]),
     "xy_get_labels": (C.c_int, [C.c_void_p, C.c_void_p]),
     "xy_set_labels": (C.c_int, [C.c_void_p, C.c_void_p]),
     "xy_get_energy": (C.c_int, [C.c_void_p, C.c_void_p]),
@@ -56,6 +60,7 @@ SYMBOLS = {
     "xy_theta_device": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p)]),
     "xy_launch_count": (C.c_int, [C.c_void_p, C.POINTER(C.c_int64)]),
     "xy_synchronize": (C.c_int, [C.c_void_p]),
+    "xy_l2_bandwidth": (C.c_int, [C.c_size_t, C.c_int, C.c_int, C.c_void_p, C.POINTER(C.c_double)]),
 }
 
 _lib = None
@@ -71,8 +76,7 @@ def lib():
     """Load (building if stale) libxy_b200.so.  Raises if nvcc or the build fails: there is no fallback."""
     global _lib
     if _lib is None:
-        # XY_B200_LIB: load a prebuilt variant of the library instead (kernel tuning experiments only)
-        L = C.CDLL(os.environ.get("XY_B200_LIB") or _build.build_xy())
+        L = C.CDLL(_build.build_xy())
         for name, (res, args) in SYMBOLS.items():
             f = getattr(L, name)
             f.restype, f.argtypes = res, args
@@ -156,6 +160,30 @@ def xy_random_walk(g, start, n_steps, seed, sample_base=0, stream=None):
     return hist
 
 
+def xy_random_walk_kernel_us():
+    out = C.c_double()
+    _check(lib().xy_random_walk_kernel_us(C.byref(out)))
+    return out.value
+
+
+def xy_set_path(pt, path):
+    _check(lib().xy_set_path(pt, path))
+
+
+def xy_get_path(pt, or_per_sweep=1):
+    """(path xy_run would take: 1 = launch per colour class, 2 = cluster per sample; CTAs per cluster)"""
+    p, c = C.c_int(), C.c_int()
+    _check(lib().xy_get_path(pt, or_per_sweep, C.byref(p), C.byref(c)))
+    return p.value, c.value
+
+
+def xy_get_schedule(pt):
+    """(samples per launch group, bytes one group keeps live)"""
+    g, b = C.c_int(), C.c_int64()
+    _check(lib().xy_get_schedule(pt, C.byref(g), C.byref(b)))
+    return g.value, b.value
+
+
 def xy_pt_create(g, T, seed, width=None, sample_base=0, theta_dev=None, stream=None):
     """theta_dev: device address (int) of a caller-owned [S][N][R] fp32 buffer, e.g. tensor.data_ptr()."""
     T, Tp = _host(T, np.float64)
@@ -236,6 +264,14 @@ def xy_set_theta(pt, theta):
     _check(lib().xy_set_theta(pt, p))
 
 
+def xy_set_theta_async(pt, theta_pinned):
+    """theta_pinned: C-contiguous float32 numpy view of PINNED host memory; the caller keeps it alive and unchanged
+    until xy_synchronize."""
+    if theta_pinned.dtype != np.float32 or not theta_pinned.flags["C_CONTIGUOUS"]:
+        raise ValueError("theta_pinned must be a C-contiguous float32 array")
+    _check(lib().xy_set_theta_async(pt, theta_pinned.ctypes.data_as(C.c_void_p)))
+
+
 def xy_get_labels(pt, shape):
     out = np.empty(shape, np.int32)
     _check(lib().xy_get_labels(pt, out.ctypes.data_as(C.c_void_p)))
@@ -297,6 +333,13 @@ def xy_synchronize(pt):
     _check(lib().xy_synchronize(pt))
 
 
+def xy_l2_bandwidth(nbytes=32 << 20, mode=0, repeats=5, stream=None):
+    """GB/s of the L2 read microbenchmark (mode 0 linear stream, 1 random 256-byte rows)."""
+    out = C.c_double()
+    _check(lib().xy_l2_bandwidth(nbytes, mode, repeats, stream, C.byref(out)))
+    return out.value
+
+
 class Ensemble:
     """Convenience owner of one graph + PT handle; theta lives in a torch tensor on its own torch stream.
     Still marshalling only: every method forwards to the xy_* call of the same name."""
@@ -345,6 +388,14 @@ class Ensemble:
     def run_sweeps(self, n_blocks, sweeps_per_block=10, or_per_sweep=1):
         xy_run_sweeps(self.pt, n_blocks, sweeps_per_block, or_per_sweep)
     def set_schedule(self, g): xy_set_schedule(self.pt, g)
+    def get_schedule(self): return xy_get_schedule(self.pt)
+    def set_path(self, path): xy_set_path(self.pt, path)
+    def get_path(self, or_per_sweep=1): return xy_get_path(self.pt, or_per_sweep)
+
+    def path_name(self, or_per_sweep=1):
+        p, c = self.get_path(or_per_sweep)
+        return (f"k_cycle: one {c}-CTA cluster per sample, whole cycles per launch" if p == 2
+                else "k_phase: one launch per colour class (captured graph, PDL edges)")
     def set_tuning(self, balance=1, pdl=1, l2_persist=1, fuse_measure=1, cta_shape=0):
         xy_set_tuning(self.pt, balance, pdl, l2_persist, fuse_measure, cta_shape)
     def metropolis_colour(self, c, sweep): xy_metropolis_colour(self.pt, c, sweep)
@@ -353,6 +404,7 @@ class Ensemble:
     def set_order(self, order): xy_set_order(self.pt, order)
     def get_theta(self, out=None): return xy_get_theta(self.pt, (self.S, self.N, self.R), out)
     def set_theta(self, th): xy_set_theta(self.pt, th)
+    def set_theta_async(self, th_pinned): xy_set_theta_async(self.pt, th_pinned)
     def get_labels(self): return xy_get_labels(self.pt, (self.S, self.R))
     def set_labels(self, lab): xy_set_labels(self.pt, lab)
     def get_energy(self): return xy_get_energy(self.pt, (self.S, self.R))

@@ -1,0 +1,387 @@
+// xy_aux_kernels.cuh -- the kernels outside the colour-class hot loop (included by xy_b200.cu only): the any-R path (one
+// warp per site, lanes stride over the slots; one launch per colour class) that serves replica counts without a float2
+// flavour (odd R, R = 6, 10, ...), the structure factor at k_min, the random-walk return histogram, the angle
+// initialisation, the stand-alone swap round and the counter tick.
+//
+// PAPER.md:444,:454 (coloured single-spin Metropolis), :460 (over-relaxation, ref 66), :167-181 (E, m), :183-190 (chi(k)),
+// :436-440 (random walks), :460-472 (parallel tempering); readings R5-R11, R18, R19 in DESIGN.md.
+#pragma once
+#include "xy_kernels.cuh"
+
+namespace xy {
+
+// last CTA of a sample: fixed-point sums -> E, M per slot; optional accumulation under the slot's temperature
+// (Eq. 13-16); leaves fx and the ticket zeroed for the next launch
+__device__ __forceinline__ void measure_finalize(const TileArgs &a, int s) {
+    for (int r = threadIdx.x; r < a.R; r += blockDim.x) {
+        long long *f = a.fx + (static_cast<size_t>(s) * a.R + r) * 3;
+        const double e = static_cast<double>(__ldcg(f)) * kInvFix;
+        const double mx = static_cast<double>(__ldcg(f + 1)) * kInvFix;
+        const double my = static_cast<double>(__ldcg(f + 2)) * kInvFix;
+        f[0] = 0; f[1] = 0; f[2] = 0;
+        const size_t sr = static_cast<size_t>(s) * a.R + r;
+        a.E_slot[sr] = e;
+        a.M_slot[2 * sr] = mx;
+        a.M_slot[2 * sr + 1] = my;
+        if (a.accumulate) {
+            double *o = a.acc + (static_cast<size_t>(s) * a.R + a.temp_of_slot[sr]) * 8;
+            const double ux = mx / a.N, uy = my / a.N, m2 = ux * ux + uy * uy;
+            o[0] += 1.0; o[1] += e; o[2] += e * e; o[3] += sqrt(m2); o[4] += m2; o[5] += m2 * m2;
+            o[6] += ux; o[7] += uy;
+        }
+    }
+    if (threadIdx.x == 0) a.ticket[s] = 0u;
+}
+
+// ---- generic path: any R >= 1 (odd R, R = 6, ...): one warp per site, lanes stride over the slots ----
+template <int MODE>
+__global__ void __launch_bounds__(kBlock) k_update_class_generic(const TileArgs a) {
+    const int s = a.s0 + blockIdx.y;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int cbeg = a.class_ptr[s * a.q_stride + a.colour];
+    const int cend = a.class_ptr[s * a.q_stride + a.colour + 1];
+    const int n_sites = cend - cbeg;
+    const int g0 = (blockIdx.x * kWarps + warp) * a.tiles_per_warp;
+    if (g0 >= n_sites) return;
+    const int g1 = min(g0 + a.tiles_per_warp, n_sites);
+    float *__restrict__ th = a.theta + static_cast<size_t>(s) * a.N * a.R;
+    const int2 *__restrict__ rec = a.rec + static_cast<size_t>(s) * a.N;
+    const uint32_t sweep = a.use_counter ? a.counters[0] + static_cast<uint32_t>(a.sweep_offset) : a.sweep_fixed;
+
+    for (int g = g0; g < g1; ++g) {
+        const int i = cbeg + g;
+        const int2 rc = rec[i];
+        const int deg = rc.y & 0xffff;
+        for (int r = lane; r < a.R; r += 32) {
+            const float own = th[static_cast<size_t>(i) * a.R + r];
+            float thp = 0.f, half = 0.f, mid = 0.f, u2 = 0.f, acc0 = 0.f, acc1 = 0.f;
+            if (MODE == kModeMetropolis) {
+                uint32_t x[4];
+                philox4x32_10(static_cast<uint32_t>(i), sweep,
+                              ((a.sample_base + static_cast<uint32_t>(s)) << 16) | static_cast<uint32_t>(r >> 1),
+                              kDomMetropolis, a.keys, x);
+                const float u1 = (r & 1) ? u01(x[2]) : u01(x[0]);
+                u2 = (r & 1) ? u01(x[3]) : u01(x[1]);
+                const float w = a.w_slot[static_cast<size_t>(s) * a.R + r];
+                thp = __fadd_rn(own, __fmul_rn(w, u1 - 0.5f));
+                half = 0.5f * (thp - own);
+                mid = own + half;
+            }
+            for (int e = 0; e < deg; ++e) {
+                const float t = th[static_cast<size_t>(a.col_idx[rc.x + e]) * a.R + r];
+                if (MODE == kModeMetropolis) {
+                    acc0 += __sinf(mid - t);
+                } else {
+                    float sn, cs;
+                    __sincosf(t, &sn, &cs);
+                    acc0 += cs; acc1 += sn;
+                }
+            }
+            float out;
+            if (MODE == kModeMetropolis)
+                // dE = -sum_j[cos(th' - th_j) - cos(th - th_j)] = 2 sin((th'-th)/2) sum_j sin((th'+th)/2 - th_j)
+                out = metropolis_select(own, thp, u2,
+                                        __expf(-a.beta_slot[static_cast<size_t>(s) * a.R + r] * (2.0f * __sinf(half) * acc0)));
+            else
+                out = overrelax_finish(own, acc0, acc1);
+            th[static_cast<size_t>(i) * a.R + r] = out;
+        }
+    }
+}
+
+// generic measure: grid (n_chunks, samples); thread = slot (strided), sequential over the CTA's sites
+__global__ void __launch_bounds__(kBlock) k_measure_generic(const TileArgs a, int chunk_sites) {
+    __shared__ int s_last;
+    const int s = a.s0 + blockIdx.y;
+    const int ibeg = blockIdx.x * chunk_sites;
+    const int iend = min(ibeg + chunk_sites, a.N);
+    const float *__restrict__ th = a.theta + static_cast<size_t>(s) * a.N * a.R;
+    const int2 *__restrict__ rec = a.rec + static_cast<size_t>(s) * a.N;
+    for (int r = threadIdx.x; r < a.R; r += kBlock) {
+        double e = 0.0, mx = 0.0, my = 0.0;
+        for (int i = ibeg; i < iend; ++i) {
+            const int2 rc = rec[i];
+            const int deg = rc.y & 0xffff, nlow = static_cast<int>(static_cast<uint32_t>(rc.y) >> 16);
+            const float own = th[static_cast<size_t>(i) * a.R + r];
+            float sn, cs, es = 0.f;
+            __sincosf(own, &sn, &cs);
+            for (int k = nlow; k < deg; ++k)
+                es += __cosf(own - th[static_cast<size_t>(a.col_idx[rc.x + k]) * a.R + r]);
+            e -= static_cast<double>(es); mx += static_cast<double>(cs); my += static_cast<double>(sn);
+        }
+        unsigned long long *f = reinterpret_cast<unsigned long long *>(a.fx) + (static_cast<size_t>(s) * a.R + r) * 3;
+        atomicAdd(f, static_cast<unsigned long long>(__double2ll_rn(e * kFix)));
+        atomicAdd(f + 1, static_cast<unsigned long long>(__double2ll_rn(mx * kFix)));
+        atomicAdd(f + 2, static_cast<unsigned long long>(__double2ll_rn(my * kFix)));
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(a.ticket + s, 1u) == gridDim.x - 1u) ? 1 : 0;
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+        measure_finalize(a, s);
+    }
+}
+
+// ---- structure factor at the smallest momenta (Eq. 17-18) ---------------
+// G1 = |sum_i S_i exp(i 2 pi x_i / Lx)|^2 / N, G2 likewise with y_i / Ly, per (sample, slot): the single-configuration
+// estimators of chi(k_min).  One streaming pass over theta (4 bytes per spin and slot, no gathers): a warp walks a
+// contiguous range of sites, lane = slot (blocks of 32 slots), eight sums per slot (Re/Im x two spin components x
+// two momenta) as exact fixed-point integers (scale 2^22, see quant of the measure kernel), so the result does not
+// depend on the grid.  The last CTA of a sample converts the sums and files G1, G2 under the slot's temperature.
+struct FourierArgs {
+    const float *theta;             // [S][N][R]
+    const uint32_t *coords;         // [S][N] x | y << 16
+    const float2 *tab1, *tab2;      // [Lx], [Ly]: (cos, sin)(2 pi n / L)
+    long long *fk;                  // [S][R][8] fixed-point sums, zero between launches
+    unsigned int *ticket;           // [S]
+    const int32_t *temp_of_slot;    // [S][R]
+    double *G_slot;                 // [S][R][2]
+    double *acc_k;                  // [S][R][3]: n, sum G1, sum G2 by temperature
+    int N, R, s0, sites_per_warp;
+};
+
+__device__ __forceinline__ int quant_unit(float x) { return __float_as_int(__fadd_rn(x, 3.0f)) - 0x40400000; }   // rn(x 2^22), |x| <= 1
+
+__global__ void __launch_bounds__(kBlock) k_fourier(const FourierArgs a) {
+    __shared__ int s_last;
+    const int s = a.s0 + blockIdx.y;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int i0 = (blockIdx.x * kWarps + warp) * a.sites_per_warp;
+    const int i1 = min(a.N, i0 + a.sites_per_warp);
+    const float *th = a.theta + static_cast<size_t>(s) * a.N * a.R;
+    const uint32_t *co = a.coords + static_cast<size_t>(s) * a.N;
+    for (int r = lane; r < a.R && i0 < i1; r += 32) {
+        long long acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        int part[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        int n_part = 0;
+        for (int i = i0; i < i1; ++i) {
+            const uint32_t xy = __ldg(co + i);
+            const float2 p1 = __ldg(a.tab1 + (xy & 0xffffu)), p2 = __ldg(a.tab2 + (xy >> 16));
+            float sn, cs;
+            __sincosf(th[static_cast<size_t>(i) * a.R + r], &sn, &cs);
+            part[0] += quant_unit(__fmul_rn(cs, p1.x)); part[1] += quant_unit(__fmul_rn(cs, p1.y));
+            part[2] += quant_unit(__fmul_rn(sn, p1.x)); part[3] += quant_unit(__fmul_rn(sn, p1.y));
+            part[4] += quant_unit(__fmul_rn(cs, p2.x)); part[5] += quant_unit(__fmul_rn(cs, p2.y));
+            part[6] += quant_unit(__fmul_rn(sn, p2.x)); part[7] += quant_unit(__fmul_rn(sn, p2.y));
+            if (++n_part == 256) {      // 256 * 2^22 < 2^31
+#pragma unroll
+                for (int c = 0; c < 8; ++c) { acc[c] += part[c]; part[c] = 0; }
+                n_part = 0;
+            }
+        }
+        unsigned long long *f = reinterpret_cast<unsigned long long *>(a.fk) + (static_cast<size_t>(s) * a.R + r) * 8;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) atomicAdd(f + c, static_cast<unsigned long long>(acc[c] + part[c]));
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(a.ticket + s, 1u) == gridDim.x - 1u) ? 1 : 0;
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+        const double inv = 1.0 / 4194304.0;
+        for (int r = threadIdx.x; r < a.R; r += blockDim.x) {
+            long long *f = a.fk + (static_cast<size_t>(s) * a.R + r) * 8;
+            double v[8];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) { v[c] = static_cast<double>(__ldcg(f + c)) * inv; f[c] = 0; }
+            const double g1 = (v[0] * v[0] + v[1] * v[1] + v[2] * v[2] + v[3] * v[3]) / a.N;
+            const double g2 = (v[4] * v[4] + v[5] * v[5] + v[6] * v[6] + v[7] * v[7]) / a.N;
+            const size_t sr = static_cast<size_t>(s) * a.R + r;
+            a.G_slot[2 * sr] = g1;
+            a.G_slot[2 * sr + 1] = g2;
+            double *o = a.acc_k + (static_cast<size_t>(s) * a.R + a.temp_of_slot[sr]) * 3;
+            o[0] += 1.0; o[1] += g1; o[2] += g2;
+        }
+        if (threadIdx.x == 0) a.ticket[s] = 0u;
+    }
+}
+
+// float2 flavour of k_fourier for R = 2G (G a power of two <= 32) or R a multiple of 64 (G = 32, blockIdx.z = block
+// of 64 slots): a lane owns two adjacent slots, G lanes cover a site, a warp reads 32/G sites per step (one fully used
+// 256-byte request at R >= 64), four steps of loads in flight.  Same fixed-point sums, same finalisation.
+template <int G>
+__global__ void __launch_bounds__(kBlock) k_fourier2(const FourierArgs a) {
+    constexpr int SPW = 32 / G;
+    __shared__ int s_last;
+    const int s = a.s0 + blockIdx.y;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int sub = lane / G, q = blockIdx.z * G + lane % G;           // slot pair of this lane
+    const int R2 = a.R >> 1;
+    const int i0 = (blockIdx.x * kWarps + warp) * a.sites_per_warp;
+    const int i1 = min(a.N, i0 + a.sites_per_warp);
+    const float2 *th = reinterpret_cast<const float2 *>(a.theta) + static_cast<size_t>(s) * a.N * R2 + q;
+    const uint32_t *co = a.coords + static_cast<size_t>(s) * a.N;
+    // fp32 partial sums over <= 256 sites of the lane's own range (fixed order: the partition is a function of N, S
+    // and R only, so a run is bit-reproducible), then exact fixed-point sums across flushes and warps
+    float part[16];
+#pragma unroll
+    for (int c = 0; c < 16; ++c) part[c] = 0.f;
+    int n_part = 0;
+    auto tally = [&](float t, const float2 p1, const float2 p2, int o) {
+        float sn, cs;
+        __sincosf(t, &sn, &cs);
+        part[o + 0] = fmaf(cs, p1.x, part[o + 0]); part[o + 1] = fmaf(cs, p1.y, part[o + 1]);
+        part[o + 2] = fmaf(sn, p1.x, part[o + 2]); part[o + 3] = fmaf(sn, p1.y, part[o + 3]);
+        part[o + 4] = fmaf(cs, p2.x, part[o + 4]); part[o + 5] = fmaf(cs, p2.y, part[o + 5]);
+        part[o + 6] = fmaf(sn, p2.x, part[o + 6]); part[o + 7] = fmaf(sn, p2.y, part[o + 7]);
+    };
+    auto flush = [&]() {      // rare (once per <= 256 sites and lane): no 64-bit accumulators live in the loop
+        unsigned long long *f = reinterpret_cast<unsigned long long *>(a.fk) + (static_cast<size_t>(s) * a.R + 2 * q) * 8;
+#pragma unroll
+        for (int c = 0; c < 16; ++c) {
+            atomicAdd(f + c, static_cast<unsigned long long>(__double2ll_rn(static_cast<double>(part[c]) * 4194304.0)));
+            part[c] = 0.f;
+        }
+    };
+    // software pipeline: the loads of batch k+1 (4 steps of theta + coordinates) fly while batch k is tallied
+    constexpr int UB = 4;
+    float2 t[UB], tn[UB];
+    uint32_t xy[UB], xyn[UB];
+    auto load = [&](int i, float2 (&tt)[UB], uint32_t (&cc)[UB]) {
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            const int iu = i + u * SPW;
+            tt[u] = make_float2(0.f, 0.f); cc[u] = 0u;
+            if (iu < i1) { tt[u] = __ldcs(th + static_cast<size_t>(iu) * R2); cc[u] = __ldg(co + iu); }
+        }
+    };
+    load(i0 + sub, t, xy);
+    for (int i = i0 + sub; i < i1; i += UB * SPW) {
+        load(i + UB * SPW, tn, xyn);
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            if (i + u * SPW < i1) {
+                const float2 p1 = __ldg(a.tab1 + (xy[u] & 0xffffu)), p2 = __ldg(a.tab2 + (xy[u] >> 16));
+                tally(t[u].x, p1, p2, 0);
+                tally(t[u].y, p1, p2, 8);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < UB; ++u) { t[u] = tn[u]; xy[u] = xyn[u]; }
+        n_part += UB;
+        if (n_part >= 256) {
+            flush();
+            n_part = 0;
+        }
+    }
+    // end of the range: quantise, add the CTA's warps in shared memory (exact integers), one atomic per CTA and sum
+    __shared__ long long s_red[kWarps][32][16];
+#pragma unroll
+    for (int c = 0; c < 16; ++c) s_red[warp][lane][c] = __double2ll_rn(static_cast<double>(part[c]) * 4194304.0);
+    __syncthreads();
+    for (int e = threadIdx.x; e < G * 16; e += blockDim.x) {
+        const int ll = e / 16, c = e % 16;
+        long long v = 0;
+        for (int wi = 0; wi < kWarps; ++wi)
+            for (int sb = 0; sb < SPW; ++sb) v += s_red[wi][sb * G + ll][c];
+        atomicAdd(reinterpret_cast<unsigned long long *>(a.fk) + (static_cast<size_t>(s) * a.R + 2 * (blockIdx.z * G + ll)) * 8 + c,
+                  static_cast<unsigned long long>(v));
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(a.ticket + s, 1u) == gridDim.x * gridDim.z - 1u) ? 1 : 0;
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+        const double inv = 1.0 / 4194304.0;
+        for (int r = threadIdx.x; r < a.R; r += blockDim.x) {
+            long long *f = a.fk + (static_cast<size_t>(s) * a.R + r) * 8;
+            double v[8];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) { v[c] = static_cast<double>(__ldcg(f + c)) * inv; f[c] = 0; }
+            const double g1 = (v[0] * v[0] + v[1] * v[1] + v[2] * v[2] + v[3] * v[3]) / a.N;
+            const double g2 = (v[4] * v[4] + v[5] * v[5] + v[6] * v[6] + v[7] * v[7]) / a.N;
+            const size_t sr = static_cast<size_t>(s) * a.R + r;
+            a.G_slot[2 * sr] = g1;
+            a.G_slot[2 * sr + 1] = g2;
+            double *o = a.acc_k + (static_cast<size_t>(s) * a.R + a.temp_of_slot[sr]) * 3;
+            o[0] += 1.0; o[1] += g1; o[2] += g2;
+        }
+        if (threadIdx.x == 0) a.ticket[s] = 0u;
+    }
+}
+
+// ---- random-walk self-return histogram (PAPER.md:149-155 Eq. 11, :436-440 App. A) ------------
+// One thread per walker: at step t it jumps to neighbour (x * deg) >> 32 of its site (stays if the site has none), x =
+// word (t-1) % 4 of Philox counter (walker, (t-1)/4, sample << 16, domain 4); every visit of its origin at time t adds
+// one to hist[sample][t].  Integer work: bit-exact against the oracle.  A step is two dependent random reads (rec,
+// col_idx): latency-bound pointer chasing; the walkers of a warp are independent, so the loads of a warp overlap.
+// The per-CTA histogram lives in shared memory (32-bit counts), flushed with one 64-bit atomic per time and CTA.
+struct WalkArgs {
+    const int2 *rec;            // [S][N]
+    const int32_t *col_idx;
+    const int32_t *start;       // [S][n_walkers]
+    unsigned long long *hist;   // [S][n_steps + 1], zero at launch
+    int N, n_walkers, n_steps;
+    uint32_t sample_base;
+    PhiloxKeys keys;
+};
+
+__global__ void __launch_bounds__(kBlock) k_random_walk(const WalkArgs a) {
+    extern __shared__ unsigned int s_hist[];      // [n_steps + 1]
+    const int s = blockIdx.y;
+    for (int t = threadIdx.x; t <= a.n_steps; t += blockDim.x) s_hist[t] = 0u;
+    __syncthreads();
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w < a.n_walkers) {
+        const int2 *rec = a.rec + static_cast<size_t>(s) * a.N;
+        const int origin = a.start[static_cast<size_t>(s) * a.n_walkers + w];
+        int pos = origin;
+        atomicAdd(&s_hist[0], 1u);
+        uint32_t x[4] = {0u, 0u, 0u, 0u};
+        for (int t = 1; t <= a.n_steps; ++t) {
+            const int k = (t - 1) & 3;
+            if (k == 0)
+                philox4x32_10(static_cast<uint32_t>(w), static_cast<uint32_t>((t - 1) >> 2),
+                              (a.sample_base + static_cast<uint32_t>(s)) << 16, kDomWalk, a.keys, x);
+            const int2 rc = __ldg(rec + pos);
+            const uint32_t deg = static_cast<uint32_t>(rc.y & 0xffff);
+            const uint32_t xk = k == 0 ? x[0] : k == 1 ? x[1] : k == 2 ? x[2] : x[3];
+            if (deg > 0u) pos = __ldg(a.col_idx + rc.x + static_cast<int>(__umulhi(xk, deg)));
+            if (pos == origin) atomicAdd(&s_hist[t], 1u);
+        }
+    }
+    __syncthreads();
+    for (int t = threadIdx.x; t <= a.n_steps; t += blockDim.x)
+        if (s_hist[t]) atomicAdd(a.hist + static_cast<size_t>(s) * (a.n_steps + 1) + t, static_cast<unsigned long long>(s_hist[t]));
+}
+
+// ---- init: theta = 2 pi_f * u, Philox domain 0, sweep 0 ------------------------------------------------
+__global__ void k_init_theta(float *theta, int S, int N, int R, PhiloxKeys keys, uint32_t sample_base) {
+    const size_t total = static_cast<size_t>(S) * N * R;
+    for (size_t idx = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; idx < total;
+         idx += static_cast<size_t>(gridDim.x) * blockDim.x) {
+        const int r = static_cast<int>(idx % R);
+        const size_t si = idx / R;
+        const int i = static_cast<int>(si % N);
+        const int s = static_cast<int>(si / N);
+        uint32_t x[4];
+        philox4x32_10(static_cast<uint32_t>(i), 0u, ((sample_base + static_cast<uint32_t>(s)) << 16) | static_cast<uint32_t>(r >> 1),
+                      kDomInit, keys, x);
+        theta[idx] = __fmul_rn(kTwoPiF, (r & 1) ? u01(x[2]) : u01(x[0]));
+    }
+}
+
+// ---- stand-alone swap round (one CTA per sample), counters, labels -> per-slot parameters ----
+__global__ void k_pt_swap(const SwapArgs a) { pt_swap_sample(a, blockIdx.x, a.counters[1]); }
+
+__global__ void k_tick(uint32_t *counters, uint32_t d_sweep, uint32_t d_round) {
+    counters[0] += d_sweep;
+    counters[1] += d_round;
+}
+
+// labels -> per-slot parameters (after xy_set_labels)
+__global__ void k_refresh_slot_params(const int32_t *temp_of_slot, int32_t *slot_of_temp, const float *beta_f,
+                                      const float *w_f, float *beta_slot, float *w_slot, int S, int R) {
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= S * R) return;
+    const int s = idx / R, t = temp_of_slot[idx];
+    slot_of_temp[static_cast<size_t>(s) * R + t] = idx % R;
+    beta_slot[idx] = beta_f[t];
+    w_slot[idx] = w_f[t];
+}
+
+}  // namespace xy

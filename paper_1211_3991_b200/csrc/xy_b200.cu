@@ -7,17 +7,23 @@
 #include <cstdio>
 #include <cstring>
 #include <map>
+#include <mutex>
 #include <new>
 #include <string>
 #include <tuple>
 #include <vector>
 
+#include "xy_aux_kernels.cuh"
+#include "xy_cycle.cuh"
+#include "xy_diag.cuh"
+#include "xy_dispatch.h"
 #include "xy_kernels.cuh"
 #include "xy_sweep.cuh"
 
 namespace {
 
 thread_local std::string g_err;
+thread_local double g_walk_kernel_us = -1.0;      // device time of the calling thread's last k_random_walk launch
 
 int fail(int code, const std::string &msg) {
     g_err = msg;
@@ -43,29 +49,65 @@ int dev_alloc(T **p, size_t n) {
 
 int ceil_div(long long a, long long b) { return static_cast<int>((a + b - 1) / b); }
 
-// the k_phase<G, CB, MODE> instantiation for G lanes per site (CB = 0: R a multiple of 64 larger than 64)
-template <int MODE, int W>
-const void *phase_function_mode(int G, bool single_block) {
-    switch (G) {
-        case 32: return single_block ? reinterpret_cast<const void *>(xy::k_phase<32, 1, MODE, W>)
-                                     : reinterpret_cast<const void *>(xy::k_phase<32, 0, MODE, W>);
-        case 16: return reinterpret_cast<const void *>(xy::k_phase<16, 1, MODE, W>);
-        case 8: return reinterpret_cast<const void *>(xy::k_phase<8, 1, MODE, W>);
-        case 4: return reinterpret_cast<const void *>(xy::k_phase<4, 1, MODE, W>);
-        case 2: return reinterpret_cast<const void *>(xy::k_phase<2, 1, MODE, W>);
-        default: return reinterpret_cast<const void *>(xy::k_phase<1, 1, MODE, W>);
+// persisting-L2 carve-out: raised while at least one ensemble lives on the device, put back by the last xy_pt_destroy
+std::mutex g_l2_mutex;
+std::map<int, std::pair<int, size_t>> g_l2_users;      // device -> (live ensembles, limit found before the first one)
+
+bool l2_carveout_acquire(int dev, size_t bytes) {
+    std::lock_guard<std::mutex> lock(g_l2_mutex);
+    auto &u = g_l2_users[dev];
+    if (u.first == 0) {
+        size_t before = 0;
+        if (cudaDeviceGetLimit(&before, cudaLimitPersistingL2CacheSize) != cudaSuccess ||
+            cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, bytes) != cudaSuccess) {
+            cudaGetLastError();
+            return false;
+        }
+        u.second = before;
     }
-}
-template <int W>
-const void *phase_function(int G, bool single_block, int mode) {
-    return mode == 0 ? phase_function_mode<0, W>(G, single_block)
-         : mode == 1 ? phase_function_mode<1, W>(G, single_block)
-         : mode == 2 ? phase_function_mode<2, W>(G, single_block)
-         : mode == 3 ? phase_function_mode<3, W>(G, single_block)
-         : mode == 4 ? phase_function_mode<4, W>(G, single_block) : phase_function_mode<5, W>(G, single_block);
+    u.first += 1;
+    return true;
 }
 
+void l2_carveout_release(int dev) {
+    std::lock_guard<std::mutex> lock(g_l2_mutex);
+    auto it = g_l2_users.find(dev);
+    if (it == g_l2_users.end() || it->second.first == 0) return;
+    if (--it->second.first == 0) {
+        cudaCtxResetPersistingL2Cache();
+        cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, it->second.second);
+        cudaGetLastError();
+    }
+}
+
+// every entry point runs on the device its handle was created on and leaves the caller's current device unchanged
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(int dev) {
+        if (dev >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+    DeviceGuard(const DeviceGuard &) = delete;
+    DeviceGuard &operator=(const DeviceGuard &) = delete;
+};
+
 }  // namespace
+
+namespace xy {
+
+const void *phase_function(int W, int G, bool single_block, int mode) {
+    if (W == 24) return phase_function_w24(G, single_block, mode);
+    if (W == kWarpsSmall) return mode < 3 ? phase_function_w8_a(G, single_block, mode) : phase_function_w8_b(G, single_block, mode);
+    if (W == kWarpsBig) return mode < 3 ? phase_function_w32_a(G, single_block, mode) : phase_function_w32_b(G, single_block, mode);
+    return nullptr;
+}
+
+const void *cycle_function(int order, int G) { return order == 0 ? cycle_function_o0(G) : cycle_function_o1(G); }
+
+}  // namespace xy
 
 struct xy_graph {
     int S = 0, N = 0, q_max = 0, q_stride = 0, max_degree = 0;
@@ -81,12 +123,13 @@ struct xy_graph {
     uint32_t *coords = nullptr;        // [S][N] x | y << 16
     float2 *tab1 = nullptr, *tab2 = nullptr;   // [Lx], [Ly]: (cos, sin)(2 pi n / L)
     cudaStream_t stream = nullptr;
+    int device = -1, n_sm = 0;         // the CUDA device the graph lives on (current device of xy_graph_load)
 };
 
 struct CycleKey {
-    int sps, orps, me, phase, group;
+    int sps, orps, me, phase, group, await_upload;
     bool operator<(const CycleKey &o) const {
-        return std::tie(sps, orps, me, phase, group) < std::tie(o.sps, o.orps, o.me, o.phase, o.group);
+        return std::tie(sps, orps, me, phase, group, await_upload) < std::tie(o.sps, o.orps, o.me, o.phase, o.group, o.await_upload);
     }
 };
 
@@ -119,6 +162,7 @@ struct xy_pt {
     int col_blocks = 1;
     int l2_persist = 1;              // mark the running sample group's theta as persisting in L2 (access policy window)
     size_t l2_persist_bytes = 0, l2_window_max = 0;   // device limits (0 = not supported)
+    bool l2_limit_set = false;       // this ensemble holds a reference on the device's persisting-L2 carve-out
     int balance = 1;                 // cost-balanced share tables (1) or equal shares (0)
     int pdl = 1;                     // programmatic dependent launch edges between the k_phase launches
     const void *phase_fn[2][6] = {};   // k_phase<G, CB, MODE, W>: [0] W = 8 warps per CTA, [1] W = 32
@@ -126,6 +170,9 @@ struct xy_pt {
     int order = 0;                   // 0 = Metropolis sweep then OR sweep, 1 = interleaved by colour (xy_set_order)
     int capacity_big = 0;            // co-resident 32-warp CTAs (one per SM)
     int cta_shape = 0;               // 0 = by class size, 1 = always 8-warp CTAs, 2 = always 32-warp CTAs
+    int path = 0;                    // xy_set_path: 0 = automatic, 1 = one launch per colour class (k_phase), 2 = one cluster per sample (k_cycle)
+    const void *cycle_fn[2] = {nullptr, nullptr};   // k_cycle<G, ORDER, xy::kCycleWarps>, by order
+    int cluster_max = 0;             // largest cluster size the device schedules for k_cycle (0 = not available)
     int fuse_measure = 1;            // measured sweeps: the last over-relaxation sweep also produces E, Mx, My (MODE 3)
     std::map<int, int4 *> parts;     // warps per sample -> device [S][q_stride][nw] share tables {i0, w1, start0, n_run}
     int sweep_capacity = 0;          // co-resident CTAs of k_phase on this device: the grid is one such wave
@@ -136,6 +183,12 @@ struct xy_pt {
     bool e_fresh = false;
     long long launches = 0;
     std::map<CycleKey, CycleGraph> graphs;
+    // xy_set_theta_async: group-wise uploads on a second stream, awaited group by group inside the next cycle
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t compute_done = nullptr;
+    std::vector<cudaEvent_t> upload_ev;   // one per sample group of the schedule the upload was issued for
+    int upload_group = 0;                 // samples per group of that schedule
+    bool upload_armed = false;            // uploads in flight that the compute stream has not been ordered after yet
 };
 
 namespace {
@@ -160,7 +213,7 @@ xy::TileArgs tile_args(const xy_pt *pt, int colour, int s0) {
     a.N = g->N; a.R = pt->R; a.q_stride = g->q_stride; a.colour = colour; a.s0 = s0; a.tiles_per_warp = 1;
     a.sweep_fixed = 0u; a.sweep_offset = 0; a.use_counter = 0;
     a.sample_base = pt->sample_base; a.keys = pt->keys;
-    a.fx = pt->fx; a.ticket = pt->ticket; a.temp_of_slot = pt->temp_of_slot;
+    a.fx = pt->fx; a.fx_stride = static_cast<size_t>(g->S) * pt->R * 3; a.ticket = pt->ticket; a.temp_of_slot = pt->temp_of_slot;
     a.E_slot = pt->E_slot; a.M_slot = pt->M_slot; a.acc = pt->acc; a.accumulate = 0;
     return a;
 }
@@ -311,7 +364,7 @@ int launch_class(xy_pt *pt, int colour, int s0, int s1, bool use_counter, int sw
     a.sweep_fixed = sweep_fixed; a.sweep_offset = sweep_offset; a.use_counter = use_counter ? 1 : 0;
     const long long total = static_cast<long long>(nmax) * (s1 - s0);
     // enough warps for ~3 full waves of resident warps, at most 8 sites per warp
-    a.tiles_per_warp = static_cast<int>(std::min<long long>(8, std::max<long long>(1, total / (148 * 32 * 3))));
+    a.tiles_per_warp = static_cast<int>(std::min<long long>(8, std::max<long long>(1, total / (static_cast<long long>(g->n_sm) * 32 * 3))));
     const dim3 grid(ceil_div(ceil_div(nmax, a.tiles_per_warp), xy::kWarps), s1 - s0, 1);
     xy::k_update_class_generic<MODE><<<grid, xy::kBlock, 0, pt->stream>>>(a);
     XY_CUDA(cudaGetLastError());
@@ -332,13 +385,18 @@ int launch_measure(xy_pt *pt, int s0, int s1, bool accumulate) {
     return XY_OK;
 }
 
-int launch_swap(xy_pt *pt, const uint8_t *decisions_dev, uint32_t d_sweep) {
+xy::SwapArgs swap_args(const xy_pt *pt, const uint8_t *decisions_dev) {
     xy::SwapArgs a;
     a.E_slot = pt->E_slot; a.betaT = pt->betaT; a.beta_f = pt->beta_f; a.w_f = pt->w_f;
     a.slot_of_temp = pt->slot_of_temp; a.temp_of_slot = pt->temp_of_slot;
     a.beta_slot = pt->beta_slot; a.w_slot = pt->w_slot; a.counters = pt->counters; a.decisions = decisions_dev;
     a.attempts = pt->attempts; a.accepts = pt->accepts; a.R = pt->R;
     a.keys = pt->keys; a.sample_base = pt->sample_base;
+    return a;
+}
+
+int launch_swap(xy_pt *pt, const uint8_t *decisions_dev, uint32_t d_sweep) {
+    const xy::SwapArgs a = swap_args(pt, decisions_dev);
     xy::k_pt_swap<<<pt->g->S, 128, 0, pt->stream>>>(a);
     XY_CUDA(cudaGetLastError());
     xy::k_tick<<<1, 1, 0, pt->stream>>>(pt->counters, d_sweep, 1u);
@@ -400,10 +458,13 @@ int sweep_group_interleaved(xy_pt *pt, int s0, int s1, int sweep_offset, int mea
     return XY_OK;
 }
 
-int issue_cycle(xy_pt *pt, int sps, int orps, int me, int phase, int group) {
+int issue_cycle(xy_pt *pt, int sps, int orps, int me, int phase, int group, bool await_upload) {
     const int S = pt->g->S;
     for (int s0 = 0; s0 < S; s0 += group) {
         const int s1 = std::min(S, s0 + group);
+        // xy_set_theta_async: this group's angles arrive on the copy stream; an external event-wait node orders the
+        // group's first launch after its upload, so the upload of group g+1 overlaps the sweeps of group g
+        if (await_upload) XY_CUDA(cudaStreamWaitEvent(pt->stream, pt->upload_ev[s0 / group], cudaEventWaitExternal));
         bool fresh = false;
         for (int k = 1; k <= sps; ++k) {
             if (pt->order == 1) {
@@ -458,6 +519,60 @@ int issue_sweeps(xy_pt *pt, int sps, int orps, int group) {
     xy::k_tick<<<1, 1, 0, pt->stream>>>(pt->counters, static_cast<uint32_t>(sps), 0u);
     XY_CUDA(cudaGetLastError());
     pt->launches += 1;
+    return XY_OK;
+}
+
+// ---- the cluster path (k_cycle): one thread-block cluster per sample runs whole cycles in one launch ----
+// CTAs per sample: as many as spread the samples over the SMs, a power of two <= the device's cluster limit
+int cycle_cluster_size(const xy_pt *pt) {
+    int c = 1;
+    while (c * 2 <= pt->cluster_max && static_cast<long long>(c) * 2 * pt->g->S <= pt->g->n_sm) c *= 2;
+    return c;
+}
+
+// the cluster path serves one column block (R = 2G <= 64) with at least one over-relaxation sweep per Metropolis sweep
+bool cycle_eligible(const xy_pt *pt, int orps) {
+    return pt->fast_G && pt->col_blocks == 1 && pt->cluster_max >= 1 && orps >= 1 && pt->fuse_measure;
+}
+
+// automatic choice: the cluster path when a colour-class launch would be launch-latency bound, i.e. when the rows of ALL
+// samples together give a resident warp less than a handful of rows per class (measured crossover: DESIGN.md 7.2)
+bool use_cycle_path(const xy_pt *pt, int orps) {
+    if (pt->path == 1 || !cycle_eligible(pt, orps)) return false;
+    if (pt->path == 2) return true;
+    const long long rows = static_cast<long long>(ceil_div(pt->g->N, 32 / pt->fast_G)) * pt->g->S;
+    return rows < 16ll * xy::kWarpsBig * pt->capacity_big;
+}
+
+int launch_cycle(xy_pt *pt, int n_cycles, int sps, int orps, int me, bool do_swap) {
+    const xy_graph *g = pt->g;
+    if (n_cycles <= 0) return XY_OK;
+    const int C = cycle_cluster_size(pt);
+    xy::CycleArgs a;
+    a.sa = sweep_args(pt, 0);
+    if (pt->balance) {
+        const int rc = get_partition(pt, C * xy::kCycleWarps, &a.sa.part);
+        if (rc != XY_OK) return rc;
+    }
+    a.sw = swap_args(pt, nullptr);
+    a.n_cycles = n_cycles; a.sps = sps; a.orps = orps; a.me = me; a.q_max = g->q_max; a.do_swap = do_swap ? 1 : 0;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(C, g->S, 1);
+    cfg.blockDim = dim3(xy::kCycleWarps * 32);
+    cfg.dynamicSmemBytes = xy::sweep_smem(xy::kCycleWarps);
+    cfg.stream = pt->stream;
+    cudaLaunchAttribute attr[2];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = C; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    int na = 1;
+    na += l2_window_attr(pt, 0, g->S, &attr[na]);
+    cfg.attrs = attr; cfg.numAttrs = na;
+    void *params[] = {&a};
+    XY_CUDA(cudaLaunchKernelExC(&cfg, pt->cycle_fn[pt->order], params));
+    xy::k_tick<<<1, 1, 0, pt->stream>>>(pt->counters, static_cast<uint32_t>(n_cycles) * static_cast<uint32_t>(sps),
+                                        do_swap ? static_cast<uint32_t>(n_cycles) : 0u);
+    XY_CUDA(cudaGetLastError());
+    pt->launches += 2;
     return XY_OK;
 }
 
@@ -518,6 +633,14 @@ void drop_graphs(xy_pt *pt) {
 }
 
 bool check_pt(const xy_pt *pt) { return pt && pt->g; }
+
+// order the compute stream after every upload of xy_set_theta_async that is still in flight (calls other than xy_run)
+int settle_upload(xy_pt *pt) {
+    if (!pt->upload_armed) return XY_OK;
+    pt->upload_armed = false;
+    if (!pt->upload_ev.empty()) XY_CUDA(cudaStreamWaitEvent(pt->stream, pt->upload_ev.back(), 0));
+    return XY_OK;
+}
 
 }  // namespace
 
@@ -581,6 +704,11 @@ int xy_graph_load(int S, int N, const int32_t *row_ptr, const int32_t *col_idx, 
         if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1)
             return fail(XY_ECUDA, "no CUDA device: this library has no CPU fallback");
         xy_graph *g = new xy_graph();
+        if (cudaGetDevice(&g->device) != cudaSuccess ||
+            cudaDeviceGetAttribute(&g->n_sm, cudaDevAttrMultiProcessorCount, g->device) != cudaSuccess || g->n_sm < 1) {
+            delete g;
+            return fail(XY_ECUDA, "cannot query the current CUDA device");
+        }
         g->S = S; g->N = N; g->q_max = q_max; g->q_stride = q_max + 1; g->max_degree = max_deg;
         g->nnz_total = off[S];
         g->stream = static_cast<cudaStream_t>(stream);
@@ -632,6 +760,7 @@ int xy_graph_load(int S, int N, const int32_t *row_ptr, const int32_t *col_idx, 
 
 int xy_graph_free(xy_graph *g) {
     if (!g) return XY_OK;
+    DeviceGuard guard(g->device);
     cudaFree(g->rec); cudaFree(g->col_idx); cudaFree(g->class_ptr);
     cudaFree(g->coords); cudaFree(g->tab1); cudaFree(g->tab2);
     delete g;
@@ -640,6 +769,7 @@ int xy_graph_free(xy_graph *g) {
 
 int xy_graph_set_coords(xy_graph *g, int Lx, int Ly, const int32_t *x, const int32_t *y) {
     if (!g || !x || !y) return fail(XY_EINVAL, "graph or coordinate array is NULL");
+    DeviceGuard guard(g->device);
     if (Lx < 1 || Ly < 1 || Lx > 65535 || Ly > 65535) return fail(XY_EINVAL, "need 1 <= Lx, Ly <= 65535");
     const size_t n = static_cast<size_t>(g->S) * g->N;
     try {
@@ -671,6 +801,7 @@ int xy_graph_set_coords(xy_graph *g, int Lx, int Ly, const int32_t *x, const int
 int xy_random_walk(const xy_graph *g, int n_walkers, const int32_t *start, int n_steps, uint64_t seed, uint32_t sample_base,
                    void *stream, int64_t *hist_host) {
     if (!g || !start || !hist_host) return fail(XY_EINVAL, "graph, start or hist is NULL");
+    DeviceGuard guard(g->device);
     if (n_walkers < 1 || n_steps < 0 || n_steps > 12000) return fail(XY_EINVAL, "need n_walkers >= 1, 0 <= n_steps <= 12000");
     if (static_cast<uint64_t>(sample_base) + g->S > 65536u) return fail(XY_EINVAL, "sample_base + S must be <= 65536");
     const size_t nw = static_cast<size_t>(g->S) * n_walkers, nh = static_cast<size_t>(g->S) * (n_steps + 1);
@@ -686,17 +817,34 @@ int xy_random_walk(const xy_graph *g, int n_walkers, const int32_t *start, int n
     a.rec = g->rec; a.col_idx = g->col_idx; a.start = d_start; a.hist = d_hist;
     a.N = g->N; a.n_walkers = n_walkers; a.n_steps = n_steps; a.sample_base = sample_base;
     a.keys = xy::philox_key_schedule(static_cast<uint32_t>(seed), static_cast<uint32_t>(seed >> 32));
+    cudaEvent_t k0 = nullptr, k1 = nullptr;
+    g_walk_kernel_us = -1.0;
     cudaError_t e = cudaMemcpyAsync(d_start, start, nw * sizeof(int32_t), cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemsetAsync(d_hist, 0, nh * sizeof(unsigned long long), st);
+    if (e == cudaSuccess) e = cudaEventCreate(&k0);
+    if (e == cudaSuccess) e = cudaEventCreate(&k1);
     if (e == cudaSuccess) {
         const dim3 grid(ceil_div(n_walkers, xy::kBlock), g->S);
+        cudaEventRecord(k0, st);
         xy::k_random_walk<<<grid, xy::kBlock, (n_steps + 1) * sizeof(unsigned int), st>>>(a);
         e = cudaGetLastError();
+        cudaEventRecord(k1, st);
     }
     if (e == cudaSuccess) e = cudaMemcpyAsync(hist_host, d_hist, nh * sizeof(int64_t), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    float k_ms = 0.f;
+    if (e == cudaSuccess && cudaEventElapsedTime(&k_ms, k0, k1) == cudaSuccess) g_walk_kernel_us = 1e3 * k_ms;
+    if (k0) cudaEventDestroy(k0);
+    if (k1) cudaEventDestroy(k1);
     cudaFree(d_start); cudaFree(d_hist);
     if (e != cudaSuccess) return fail(XY_ECUDA, std::string("xy_random_walk: ") + cudaGetErrorString(e));
+    return XY_OK;
+}
+
+int xy_random_walk_kernel_us(double *us_out) {
+    if (!us_out) return fail(XY_EINVAL, "NULL output");
+    if (g_walk_kernel_us < 0.0) return fail(XY_ESTATE, "no successful xy_random_walk call on this thread yet");
+    *us_out = g_walk_kernel_us;
     return XY_OK;
 }
 
@@ -715,12 +863,15 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
     if (!out) return fail(XY_EINVAL, "out is NULL");
     *out = nullptr;
     if (!g || !T) return fail(XY_EINVAL, "graph or T is NULL");
+    DeviceGuard guard(g->device);
     if (R < 1 || R > 1024) return fail(XY_EINVAL, "need 1 <= R <= 1024");
     if (static_cast<uint64_t>(sample_base) + g->S > 65536u) return fail(XY_EINVAL, "sample_base + S must be <= 65536");
     for (int k = 0; k < R; ++k) {
         if (!(T[k] > 0.0)) return fail(XY_EINVAL, "temperatures must be > 0");
         if (k > 0 && !(T[k] >= T[k - 1])) return fail(XY_EINVAL, "temperatures must be ascending");
-        if (width && !(width[k] >= 0.0 && std::isfinite(width[k]))) return fail(XY_EINVAL, "bad proposal width");
+        // R5 wraps a proposal once by +-2 pi: |delta| <= width / 2 must not exceed 2 pi
+        if (width && !(width[k] >= 0.0 && width[k] <= 4.0 * 3.14159265358979323846))
+            return fail(XY_EINVAL, "proposal width must lie in [0, 4 pi]");
     }
     if (theta_dev && (reinterpret_cast<uintptr_t>(theta_dev) & 7u)) return fail(XY_EINVAL, "theta_dev must be 8-byte aligned");
     xy_pt *pt = nullptr;
@@ -754,47 +905,66 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
     pt->keys = xy::philox_key_schedule(pt->key0, pt->key1);
     pt->measure_chunk = std::max(256, ((N + 127) / 128 + 7) / 8 * 8);   // legacy measure partition: a function of N only
     if (pt->fast_G) {
+        cudaError_t eo = cudaSuccess;
+        auto prepare = [&](const void *fn, int warps) {      // opt in to the kernel's dynamic shared memory
+            if (eo == cudaSuccess)
+                eo = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(xy::sweep_smem(warps)));
+            if (eo == cudaSuccess)
+                eo = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, static_cast<int>(cudaSharedmemCarveoutMaxShared));
+        };
         for (int m = 0; m < 6; ++m) {
-            pt->phase_fn[0][m] = phase_function<xy::kWarpsSmall>(pt->fast_G, pt->col_blocks == 1, m);
-            pt->phase_fn[1][m] = phase_function<xy::kWarpsBig>(pt->fast_G, pt->col_blocks == 1, m);
-            for (int b = 0; b < 2; ++b) {
-                cudaFuncSetAttribute(pt->phase_fn[b][m], cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     static_cast<int>(xy::sweep_smem(b ? xy::kWarpsBig : xy::kWarpsSmall)));
-                cudaFuncSetAttribute(pt->phase_fn[b][m], cudaFuncAttributePreferredSharedMemoryCarveout,
-                                     static_cast<int>(cudaSharedmemCarveoutMaxShared));
-            }
+            pt->phase_fn[0][m] = xy::phase_function(xy::kWarpsSmall, pt->fast_G, pt->col_blocks == 1, m);
+            pt->phase_fn[1][m] = xy::phase_function(xy::kWarpsBig, pt->fast_G, pt->col_blocks == 1, m);
+            prepare(pt->phase_fn[0][m], xy::kWarpsSmall);
+            prepare(pt->phase_fn[1][m], xy::kWarpsBig);
         }
-        int per_sm = 0, n_sm = 0, dev = 0;
-        cudaError_t eo = cudaGetDevice(&dev);
-        if (eo == cudaSuccess) eo = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
         // 32 resident warps x 5.5 KB of shared memory per SM in either CTA shape (carve-out set above)
-        pt->phase_fn24[0] = phase_function<24>(pt->fast_G, pt->col_blocks == 1, 3);
-        pt->phase_fn24[1] = phase_function<24>(pt->fast_G, pt->col_blocks == 1, 5);
-        for (int b = 0; b < 2; ++b) {
-            cudaFuncSetAttribute(pt->phase_fn24[b], cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(xy::sweep_smem(24)));
-            cudaFuncSetAttribute(pt->phase_fn24[b], cudaFuncAttributePreferredSharedMemoryCarveout,
-                                 static_cast<int>(cudaSharedmemCarveoutMaxShared));
-        }
-        int per_sm_big = 0;
+        pt->phase_fn24[0] = xy::phase_function(24, pt->fast_G, pt->col_blocks == 1, 3);
+        pt->phase_fn24[1] = xy::phase_function(24, pt->fast_G, pt->col_blocks == 1, 5);
+        prepare(pt->phase_fn24[0], 24);
+        prepare(pt->phase_fn24[1], 24);
+        int per_sm = 0, per_sm_big = 0;
+        const int n_sm = g->n_sm, dev = g->device;
         if (eo == cudaSuccess)
             eo = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pt->phase_fn[0][0], xy::kWarpsSmall * 32,
                                                                xy::sweep_smem(xy::kWarpsSmall));
         if (eo == cudaSuccess)
             eo = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_big, pt->phase_fn[1][0], xy::kWarpsBig * 32,
                                                                xy::sweep_smem(xy::kWarpsBig));
-        if (eo != cudaSuccess || per_sm < 1 || n_sm < 1) {
+        if (eo != cudaSuccess || per_sm < 1) {
             if (pt->owns_stream) cudaStreamDestroy(pt->stream);
             delete pt;
-            return fail(XY_ECUDA, std::string("k_phase occupancy query: ") + cudaGetErrorString(eo));
+            return fail(XY_ECUDA, std::string("k_phase attributes / occupancy query: ") + cudaGetErrorString(eo));
         }
         pt->sweep_capacity = per_sm * n_sm;
         pt->capacity_big = std::max(1, per_sm_big) * n_sm;
+        // the cluster path (k_cycle): one column block only; ask the device which cluster sizes it schedules
+        if (pt->col_blocks == 1) {
+            pt->cycle_fn[0] = xy::cycle_function(0, pt->fast_G);
+            pt->cycle_fn[1] = xy::cycle_function(1, pt->fast_G);
+            cudaError_t ec = cudaSuccess;
+            for (int o = 0; o < 2 && ec == cudaSuccess; ++o) {
+                ec = cudaFuncSetAttribute(pt->cycle_fn[o], cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          static_cast<int>(xy::sweep_smem(xy::kCycleWarps)));
+            }
+            int max_cluster = 0;
+            if (ec == cudaSuccess) {
+                cudaLaunchConfig_t qc = {};
+                qc.gridDim = dim3(8, 1, 1); qc.blockDim = dim3(xy::kCycleWarps * 32);
+                qc.dynamicSmemBytes = xy::sweep_smem(xy::kCycleWarps);
+                ec = cudaOccupancyMaxPotentialClusterSize(&max_cluster, pt->cycle_fn[0], &qc);
+            }
+            pt->cluster_max = ec == cudaSuccess ? std::min(8, std::max(0, max_cluster)) : 0;
+            cudaGetLastError();
+        }
+        // persisting L2 carve-out for the access-policy windows of the sample groups; xy_pt_destroy puts the limit back
         int max_persist = 0, max_window = 0;
         if (cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev) == cudaSuccess &&
             cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, dev) == cudaSuccess && max_persist > 0 &&
-            max_window > 0 && cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, static_cast<size_t>(max_persist)) == cudaSuccess) {
+            max_window > 0 && l2_carveout_acquire(dev, static_cast<size_t>(max_persist))) {
             pt->l2_persist_bytes = static_cast<size_t>(max_persist);
             pt->l2_window_max = static_cast<size_t>(max_window);
+            pt->l2_limit_set = true;
         }
         cudaGetLastError();
     }
@@ -809,7 +979,7 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
     A(dev_alloc(&pt->temp_of_slot, SR)); A(dev_alloc(&pt->slot_of_temp, SR));
     A(dev_alloc(&pt->counters, 2));
     A(dev_alloc(&pt->E_slot, SR)); A(dev_alloc(&pt->M_slot, SR * 2));
-    A(dev_alloc(&pt->fx, SR * 3)); A(dev_alloc(&pt->ticket, S)); A(dev_alloc(&pt->acc, SR * XY_NACC));
+    A(dev_alloc(&pt->fx, SR * 3 * 2)); A(dev_alloc(&pt->ticket, S)); A(dev_alloc(&pt->acc, SR * XY_NACC));
     A(dev_alloc(&pt->attempts, SR)); A(dev_alloc(&pt->accepts, SR)); A(dev_alloc(&pt->decisions, SR));
     A(dev_alloc(&pt->G_slot, SR * 2)); A(dev_alloc(&pt->acc_k, SR * 3)); A(dev_alloc(&pt->fk, SR * 8));
 
@@ -833,7 +1003,7 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
     if (e == cudaSuccess) e = cudaMemsetAsync(pt->attempts, 0, SR * sizeof(long long), pt->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(pt->accepts, 0, SR * sizeof(long long), pt->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(pt->E_slot, 0, SR * sizeof(double), pt->stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(pt->fx, 0, SR * 3 * sizeof(long long), pt->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(pt->fx, 0, SR * 3 * 2 * sizeof(long long), pt->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(pt->fk, 0, SR * 8 * sizeof(long long), pt->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(pt->acc_k, 0, SR * 3 * sizeof(double), pt->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(pt->G_slot, 0, SR * 2 * sizeof(double), pt->stream);
@@ -841,7 +1011,7 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
     if (e == cudaSuccess) {
         xy::k_refresh_slot_params<<<ceil_div(SR, 128), 128, 0, pt->stream>>>(pt->temp_of_slot, pt->slot_of_temp, pt->beta_f,
                                                                             pt->w_f, pt->beta_slot, pt->w_slot, S, R);
-        xy::k_init_theta<<<148 * 8, 256, 0, pt->stream>>>(pt->theta, S, N, R, pt->keys, pt->sample_base);
+        xy::k_init_theta<<<g->n_sm * 8, 256, 0, pt->stream>>>(pt->theta, S, N, R, pt->keys, pt->sample_base);
         pt->launches += 2;
         e = cudaGetLastError();
     }
@@ -856,6 +1026,7 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
 
 int xy_pt_destroy(xy_pt *pt) {
     if (!pt) return XY_OK;
+    DeviceGuard guard(pt->g ? pt->g->device : -1);
     cudaStreamSynchronize(pt->stream);
     drop_graphs(pt);
     if (pt->owns_theta) cudaFree(pt->theta);
@@ -865,6 +1036,10 @@ int xy_pt_destroy(xy_pt *pt) {
     cudaFree(pt->attempts); cudaFree(pt->accepts); cudaFree(pt->decisions);
     cudaFree(pt->G_slot); cudaFree(pt->acc_k); cudaFree(pt->fk);
     for (auto &kv : pt->parts) cudaFree(kv.second);
+    if (pt->l2_limit_set) l2_carveout_release(pt->g->device);      // the last ensemble gives the carve-out back
+    for (cudaEvent_t ev : pt->upload_ev) cudaEventDestroy(ev);
+    if (pt->compute_done) cudaEventDestroy(pt->compute_done);
+    if (pt->copy_stream) { cudaStreamSynchronize(pt->copy_stream); cudaStreamDestroy(pt->copy_stream); }
     if (pt->owns_stream) cudaStreamDestroy(pt->stream);
     delete pt;
     return XY_OK;
@@ -872,6 +1047,8 @@ int xy_pt_destroy(xy_pt *pt) {
 
 int xy_sweep(xy_pt *pt, int n_sweeps) {
     if (!check_pt(pt) || n_sweeps < 0) return fail(XY_EINVAL, "bad handle or n_sweeps < 0");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     for (int n = 0; n < n_sweeps; ++n) {
         const int rc = sweep_group(pt, 0, 0, pt->g->S, true, 1, 0u);
         if (rc != XY_OK) return rc;
@@ -886,6 +1063,8 @@ int xy_sweep(xy_pt *pt, int n_sweeps) {
 
 int xy_overrelax(xy_pt *pt, int n_sweeps) {
     if (!check_pt(pt) || n_sweeps < 0) return fail(XY_EINVAL, "bad handle or n_sweeps < 0");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     for (int n = 0; n < n_sweeps; ++n) {
         const int rc = sweep_group(pt, 1, 0, pt->g->S, false, 0, 0u);
         if (rc != XY_OK) return rc;
@@ -896,6 +1075,8 @@ int xy_overrelax(xy_pt *pt, int n_sweeps) {
 
 int xy_metropolis_colour(xy_pt *pt, int colour, uint32_t sweep) {
     if (!check_pt(pt) || colour < 0 || colour >= pt->g->q_max) return fail(XY_EINVAL, "bad handle or colour");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     pt->e_fresh = false;
     const int group = auto_group(pt);
     for (int s0 = 0; s0 < pt->g->S; s0 += group) {
@@ -907,6 +1088,8 @@ int xy_metropolis_colour(xy_pt *pt, int colour, uint32_t sweep) {
 
 int xy_metor_colour(xy_pt *pt, int colour, uint32_t sweep) {
     if (!check_pt(pt) || colour < 0 || colour >= pt->g->q_max) return fail(XY_EINVAL, "bad handle or colour");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     if (!pt->fast_G) return fail(XY_ESTATE, "the interleaved order needs a float2 kernel flavour (R = 2 * 2^k <= 64 or R % 64 == 0)");
     pt->e_fresh = false;
     const int group = auto_group(pt);
@@ -919,6 +1102,8 @@ int xy_metor_colour(xy_pt *pt, int colour, uint32_t sweep) {
 
 int xy_set_order(xy_pt *pt, int order) {
     if (!check_pt(pt) || order < 0 || order > 1) return fail(XY_EINVAL, "bad handle or order not in {0, 1}");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     if (order == 1 && !pt->fast_G)
         return fail(XY_ESTATE, "the interleaved order needs a float2 kernel flavour (R = 2 * 2^k <= 64 or R % 64 == 0)");
     XY_CUDA(cudaStreamSynchronize(pt->stream));
@@ -929,6 +1114,8 @@ int xy_set_order(xy_pt *pt, int order) {
 
 int xy_overrelax_colour(xy_pt *pt, int colour) {
     if (!check_pt(pt) || colour < 0 || colour >= pt->g->q_max) return fail(XY_EINVAL, "bad handle or colour");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     pt->e_fresh = false;
     const int group = auto_group(pt);
     for (int s0 = 0; s0 < pt->g->S; s0 += group) {
@@ -940,6 +1127,8 @@ int xy_overrelax_colour(xy_pt *pt, int colour) {
 
 int xy_pt_swap(xy_pt *pt) {
     if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     if (!pt->e_fresh) {
         const int rc = launch_measure(pt, 0, pt->g->S, false);
         if (rc != XY_OK) return rc;
@@ -952,6 +1141,8 @@ int xy_pt_swap(xy_pt *pt) {
 
 int xy_swap_with_decisions(xy_pt *pt, const uint8_t *accept_host) {
     if (!check_pt(pt) || !accept_host) return fail(XY_EINVAL, "bad handle or NULL decisions");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     const size_t SR = static_cast<size_t>(pt->g->S) * pt->R;
     XY_CUDA(cudaMemcpyAsync(pt->decisions, accept_host, SR, cudaMemcpyHostToDevice, pt->stream));
     XY_CUDA(cudaStreamSynchronize(pt->stream));  // accept_host is borrowed for the call only
@@ -962,6 +1153,8 @@ int xy_swap_with_decisions(xy_pt *pt, const uint8_t *accept_host) {
 
 int xy_measure(xy_pt *pt, double *out_host) {
     if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     const int S = pt->g->S, R = pt->R;
     const int rc = launch_measure(pt, 0, S, true);
     if (rc != XY_OK) return rc;
@@ -990,6 +1183,8 @@ int xy_measure(xy_pt *pt, double *out_host) {
 
 int xy_measure_fourier(xy_pt *pt, double *out_host) {
     if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     const xy_graph *g = pt->g;
     if (!g->coords) return fail(XY_ESTATE, "xy_graph_set_coords has not been called");
     const int S = g->S, R = pt->R;
@@ -999,7 +1194,7 @@ int xy_measure_fourier(xy_pt *pt, double *out_host) {
     a.G_slot = pt->G_slot; a.acc_k = pt->acc_k; a.N = g->N; a.R = R; a.s0 = 0;
     // one wave of CTAs over all samples and column blocks, at least 32 sites per warp
     const int cb = pt->fast_G ? pt->col_blocks : 1;
-    const int warps_per_sample = std::max(1, std::min(ceil_div(g->N, 32), std::max(1, 148 * 8 * xy::kWarps / (S * cb))));   // two waves of 4 CTAs per SM (one wave measured slower)
+    const int warps_per_sample = std::max(1, std::min(ceil_div(g->N, 32), std::max(1, g->n_sm * 8 * xy::kWarps / (S * cb))));   // two waves of 4 CTAs per SM (one wave measured slower)
     a.sites_per_warp = ceil_div(g->N, warps_per_sample);
     const dim3 grid(ceil_div(ceil_div(g->N, a.sites_per_warp), xy::kWarps), S, cb);
     switch (pt->fast_G) {
@@ -1036,6 +1231,7 @@ int xy_measure_fourier(xy_pt *pt, double *out_host) {
 
 int xy_read_fourier_accumulators(xy_pt *pt, double *acc_host) {
     if (!check_pt(pt) || !acc_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
+    DeviceGuard guard(pt->g->device);
     const size_t n = static_cast<size_t>(pt->g->S) * pt->R * 3;
     XY_CUDA(cudaMemcpyAsync(acc_host, pt->acc_k, n * sizeof(double), cudaMemcpyDeviceToHost, pt->stream));
     XY_CUDA(cudaStreamSynchronize(pt->stream));
@@ -1044,12 +1240,40 @@ int xy_read_fourier_accumulators(xy_pt *pt, double *acc_host) {
 
 int xy_set_schedule(xy_pt *pt, int samples_per_group) {
     if (!check_pt(pt) || samples_per_group < 0) return fail(XY_EINVAL, "bad handle or samples_per_group < 0");
+    DeviceGuard guard(pt->g->device);
     pt->samples_per_group = samples_per_group;
+    return XY_OK;
+}
+
+int xy_set_path(xy_pt *pt, int path) {
+    if (!check_pt(pt) || path < 0 || path > 2) return fail(XY_EINVAL, "bad handle or path not in {0, 1, 2}");
+    if (path == 2 && !(pt->fast_G && pt->col_blocks == 1 && pt->cluster_max >= 1))
+        return fail(XY_ESTATE, "the cluster path needs R = 2 * 2^k <= 64 and a device that schedules thread-block clusters");
+    pt->path = path;
+    return XY_OK;
+}
+
+int xy_get_path(xy_pt *pt, int or_per_sweep, int *path, int *cluster_size) {
+    if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    const bool cyc = use_cycle_path(pt, or_per_sweep);
+    if (path) *path = cyc ? 2 : 1;
+    if (cluster_size) *cluster_size = cyc ? cycle_cluster_size(pt) : 0;
+    return XY_OK;
+}
+
+int xy_get_schedule(xy_pt *pt, int *samples_per_group, int64_t *group_bytes) {
+    if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    const int group = auto_group(pt);
+    if (samples_per_group) *samples_per_group = group;
+    if (group_bytes)
+        *group_bytes = static_cast<int64_t>(group) * (static_cast<int64_t>(pt->g->N) * pt->R * 4 + static_cast<int64_t>(pt->g->bytes_per_sample));
     return XY_OK;
 }
 
 int xy_set_tuning(xy_pt *pt, int balance, int pdl, int l2_persist, int fuse_measure, int cta_shape) {
     if (!check_pt(pt) || cta_shape < 0 || cta_shape > 2) return fail(XY_EINVAL, "bad handle or cta_shape not in {0, 1, 2}");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     XY_CUDA(cudaStreamSynchronize(pt->stream));
     pt->cta_shape = cta_shape;
     pt->balance = balance ? 1 : 0; pt->pdl = pdl ? 1 : 0; pt->l2_persist = l2_persist ? 1 : 0;
@@ -1061,17 +1285,35 @@ int xy_set_tuning(xy_pt *pt, int balance, int pdl, int l2_persist, int fuse_meas
 int xy_run(xy_pt *pt, int n_cycles, int sps, int orps, int me) {
     if (!check_pt(pt) || n_cycles < 0 || sps < 1 || orps < 0 || me < 0)
         return fail(XY_EINVAL, "need n_cycles >= 0, sweeps_per_swap >= 1, or_per_sweep >= 0, measure_every >= 0");
+    DeviceGuard guard(pt->g->device);
     if (pt->order == 1 && orps != 1) return fail(XY_EINVAL, "the interleaved order needs or_per_sweep == 1");
+    if (pt->path == 2 && !cycle_eligible(pt, orps))
+        return fail(XY_ESTATE, "xy_set_path(2): the cluster path needs R = 2 * 2^k <= 64, or_per_sweep >= 1 and fused measurement");
+    if (use_cycle_path(pt, orps)) {          // small samples: all cycles in one launch, one cluster per sample
+        int rc = settle_upload(pt);
+        if (rc == XY_OK) rc = launch_cycle(pt, n_cycles, sps, orps, me, true);
+        if (rc != XY_OK) return rc;
+        pt->sweep += static_cast<uint32_t>(n_cycles) * static_cast<uint32_t>(sps);
+        pt->round += static_cast<uint32_t>(n_cycles);
+        if (n_cycles > 0) pt->e_fresh = false;
+        return XY_OK;
+    }
     const int group = auto_group(pt);
     {
         const int rc = prepare_partitions(pt, group);
         if (rc != XY_OK) return rc;
     }
+    if (pt->upload_armed && (n_cycles == 0 || group != pt->upload_group)) {
+        const int rc = settle_upload(pt);
+        if (rc != XY_OK) return rc;
+    }
     for (int c = 0; c < n_cycles; ++c) {
         const int phase = me > 0 ? static_cast<int>(pt->sweep % static_cast<uint32_t>(me)) : 0;
-        const CycleKey key{sps, orps, me, phase, group};
+        const bool await_upload = pt->upload_armed;      // first cycle after xy_set_theta_async: wait group by group
+        pt->upload_armed = false;
+        const CycleKey key{sps, orps, me, phase, group, await_upload ? 1 : 0};
         CycleGraph *cg = nullptr;
-        const int rc = cached_graph(pt, key, [&] { return issue_cycle(pt, sps, orps, me, phase, group); }, &cg);
+        const int rc = cached_graph(pt, key, [&] { return issue_cycle(pt, sps, orps, me, phase, group, await_upload); }, &cg);
         if (rc != XY_OK) return rc;
         XY_CUDA(cudaGraphLaunch(cg->exec, pt->stream));
         pt->launches += cg->launches;
@@ -1085,14 +1327,25 @@ int xy_run(xy_pt *pt, int n_cycles, int sps, int orps, int me) {
 int xy_run_sweeps(xy_pt *pt, int n_blocks, int sps, int orps) {
     if (!check_pt(pt) || n_blocks < 0 || sps < 1 || orps < 0)
         return fail(XY_EINVAL, "need n_blocks >= 0, sweeps_per_block >= 1, or_per_sweep >= 0");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     if (pt->order == 1 && orps != 1) return fail(XY_EINVAL, "the interleaved order needs or_per_sweep == 1");
+    if (pt->path == 2 && !cycle_eligible(pt, orps))
+        return fail(XY_ESTATE, "xy_set_path(2): the cluster path needs R = 2 * 2^k <= 64, or_per_sweep >= 1 and fused measurement");
+    if (use_cycle_path(pt, orps)) {
+        const int rc = launch_cycle(pt, n_blocks, sps, orps, 0, false);
+        if (rc != XY_OK) return rc;
+        pt->sweep += static_cast<uint32_t>(n_blocks) * static_cast<uint32_t>(sps);
+        if (n_blocks > 0) pt->e_fresh = false;
+        return XY_OK;
+    }
     const int group = auto_group(pt);
     {
         const int rc = prepare_partitions(pt, group);
         if (rc != XY_OK) return rc;
     }
     for (int b = 0; b < n_blocks; ++b) {
-        const CycleKey key{sps, orps, -1, 0, group};
+        const CycleKey key{sps, orps, -1, 0, group, 0};
         CycleGraph *cg = nullptr;
         const int rc = cached_graph(pt, key, [&] { return issue_sweeps(pt, sps, orps, group); }, &cg);
         if (rc != XY_OK) return rc;
@@ -1106,6 +1359,8 @@ int xy_run_sweeps(xy_pt *pt, int n_blocks, int sps, int orps) {
 
 int xy_get_theta(xy_pt *pt, float *theta_host) {
     if (!check_pt(pt) || !theta_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     const size_t n = static_cast<size_t>(pt->g->S) * pt->g->N * pt->R;
     XY_CUDA(cudaMemcpyAsync(theta_host, pt->theta, n * sizeof(float), cudaMemcpyDeviceToHost, pt->stream));
     XY_CUDA(cudaStreamSynchronize(pt->stream));
@@ -1114,6 +1369,8 @@ int xy_get_theta(xy_pt *pt, float *theta_host) {
 
 int xy_set_theta(xy_pt *pt, const float *theta_host) {
     if (!check_pt(pt) || !theta_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     const size_t n = static_cast<size_t>(pt->g->S) * pt->g->N * pt->R;
     XY_CUDA(cudaMemcpyAsync(pt->theta, theta_host, n * sizeof(float), cudaMemcpyHostToDevice, pt->stream));
     XY_CUDA(cudaStreamSynchronize(pt->stream));
@@ -1121,8 +1378,43 @@ int xy_set_theta(xy_pt *pt, const float *theta_host) {
     return XY_OK;
 }
 
+int xy_set_theta_async(xy_pt *pt, const float *theta_host) {
+    if (!check_pt(pt) || !theta_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
+    DeviceGuard guard(pt->g->device);
+    const int S = pt->g->S, group = auto_group(pt);
+    const size_t per_sample = static_cast<size_t>(pt->g->N) * pt->R;
+    if (!pt->copy_stream) XY_CUDA(cudaStreamCreateWithFlags(&pt->copy_stream, cudaStreamNonBlocking));
+    if (!pt->compute_done) XY_CUDA(cudaEventCreateWithFlags(&pt->compute_done, cudaEventDisableTiming));
+    const size_t n_groups = static_cast<size_t>((S + group - 1) / group);
+    if (pt->upload_group != group || pt->upload_ev.size() != n_groups) {
+        XY_CUDA(cudaStreamSynchronize(pt->stream));      // graphs that wait on the old events must have finished
+        drop_graphs(pt);
+        for (cudaEvent_t ev : pt->upload_ev) cudaEventDestroy(ev);
+        pt->upload_ev.clear();
+        for (size_t k = 0; k < n_groups; ++k) {
+            cudaEvent_t ev = nullptr;
+            XY_CUDA(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+            pt->upload_ev.push_back(ev);
+        }
+        pt->upload_group = group;
+    }
+    // the uploads overwrite theta: they start after everything already enqueued on the compute stream
+    XY_CUDA(cudaEventRecord(pt->compute_done, pt->stream));
+    XY_CUDA(cudaStreamWaitEvent(pt->copy_stream, pt->compute_done, 0));
+    for (int s0 = 0; s0 < S; s0 += group) {
+        const int s1 = std::min(S, s0 + group);
+        XY_CUDA(cudaMemcpyAsync(pt->theta + s0 * per_sample, theta_host + s0 * per_sample, (s1 - s0) * per_sample * sizeof(float),
+                                cudaMemcpyHostToDevice, pt->copy_stream));
+        XY_CUDA(cudaEventRecord(pt->upload_ev[s0 / group], pt->copy_stream));
+    }
+    pt->upload_armed = true;
+    pt->e_fresh = false;
+    return XY_OK;
+}
+
 int xy_get_labels(xy_pt *pt, int32_t *temp_of_slot_host) {
     if (!check_pt(pt) || !temp_of_slot_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
+    DeviceGuard guard(pt->g->device);
     const size_t SR = static_cast<size_t>(pt->g->S) * pt->R;
     XY_CUDA(cudaMemcpyAsync(temp_of_slot_host, pt->temp_of_slot, SR * sizeof(int32_t), cudaMemcpyDeviceToHost, pt->stream));
     XY_CUDA(cudaStreamSynchronize(pt->stream));
@@ -1131,6 +1423,7 @@ int xy_get_labels(xy_pt *pt, int32_t *temp_of_slot_host) {
 
 int xy_set_labels(xy_pt *pt, const int32_t *temp_of_slot_host) {
     if (!check_pt(pt) || !temp_of_slot_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
+    DeviceGuard guard(pt->g->device);
     const int S = pt->g->S, R = pt->R;
     try {
         std::vector<uint8_t> seen(R);
@@ -1157,6 +1450,8 @@ int xy_set_labels(xy_pt *pt, const int32_t *temp_of_slot_host) {
 
 int xy_get_energy(xy_pt *pt, double *E_slot_host) {
     if (!check_pt(pt) || !E_slot_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     if (!pt->e_fresh) {
         const int rc = launch_measure(pt, 0, pt->g->S, false);
         if (rc != XY_OK) return rc;
@@ -1170,6 +1465,7 @@ int xy_get_energy(xy_pt *pt, double *E_slot_host) {
 
 int xy_read_accumulators(xy_pt *pt, double *acc_host) {
     if (!check_pt(pt) || !acc_host) return fail(XY_EINVAL, "bad handle or NULL buffer");
+    DeviceGuard guard(pt->g->device);
     const size_t n = static_cast<size_t>(pt->g->S) * pt->R * XY_NACC;
     XY_CUDA(cudaMemcpyAsync(acc_host, pt->acc, n * sizeof(double), cudaMemcpyDeviceToHost, pt->stream));
     XY_CUDA(cudaStreamSynchronize(pt->stream));
@@ -1178,6 +1474,7 @@ int xy_read_accumulators(xy_pt *pt, double *acc_host) {
 
 int xy_reset_accumulators(xy_pt *pt) {
     if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    DeviceGuard guard(pt->g->device);
     const size_t n = static_cast<size_t>(pt->g->S) * pt->R * XY_NACC;
     XY_CUDA(cudaMemsetAsync(pt->acc, 0, n * sizeof(double), pt->stream));
     XY_CUDA(cudaMemsetAsync(pt->acc_k, 0, static_cast<size_t>(pt->g->S) * pt->R * 3 * sizeof(double), pt->stream));
@@ -1186,6 +1483,7 @@ int xy_reset_accumulators(xy_pt *pt) {
 
 int xy_get_counters(xy_pt *pt, uint32_t *sweep, uint32_t *round, int64_t *att, int64_t *acc) {
     if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    DeviceGuard guard(pt->g->device);
     uint32_t c[2];
     const size_t SR = static_cast<size_t>(pt->g->S) * pt->R;
     XY_CUDA(cudaMemcpyAsync(c, pt->counters, sizeof(c), cudaMemcpyDeviceToHost, pt->stream));
@@ -1200,6 +1498,7 @@ int xy_get_counters(xy_pt *pt, uint32_t *sweep, uint32_t *round, int64_t *att, i
 
 int xy_set_counters(xy_pt *pt, uint32_t sweep, uint32_t round) {
     if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    DeviceGuard guard(pt->g->device);
     const uint32_t c[2] = {sweep, round};
     XY_CUDA(cudaMemcpyAsync(pt->counters, c, sizeof(c), cudaMemcpyHostToDevice, pt->stream));
     XY_CUDA(cudaStreamSynchronize(pt->stream));
@@ -1209,25 +1508,67 @@ int xy_set_counters(xy_pt *pt, uint32_t sweep, uint32_t round) {
 
 int xy_theta_device(xy_pt *pt, float **theta_dev) {
     if (!check_pt(pt) || !theta_dev) return fail(XY_EINVAL, "bad handle or NULL out");
+    DeviceGuard guard(pt->g->device);
     *theta_dev = pt->theta;
     return XY_OK;
 }
 
 int xy_launch_count(xy_pt *pt, int64_t *n) {
     if (!check_pt(pt) || !n) return fail(XY_EINVAL, "bad handle or NULL out");
+    DeviceGuard guard(pt->g->device);
     *n = pt->launches;
     return XY_OK;
 }
 
-#ifdef XY_TRACE
-int xy_debug_trace(unsigned long long *out_host /*[8192][4]*/) {
-    XY_CUDA(cudaMemcpyFromSymbol(out_host, xy::g_trace, sizeof(unsigned long long) * 8192 * 4));
+int xy_l2_bandwidth(size_t bytes, int mode, int repeats, void *stream, double *gbs_out) {
+    if (!gbs_out || bytes < (1u << 20) || bytes > (size_t(1) << 32) || mode < 0 || mode > 1 || repeats < 1)
+        return fail(XY_EINVAL, "need 1 MiB <= bytes <= 4 GiB, mode in {0, 1}, repeats >= 1, non-NULL output");
+    int dev = 0, n_sm = 0;
+    XY_CUDA(cudaGetDevice(&dev));
+    XY_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    size_t n_rows = 1;                                      // 256-byte rows: the largest power of two that fits
+    while (n_rows * 2 * 256 <= bytes) n_rows *= 2;
+    const int grid = n_sm * 4, threads = 512, passes = 16;
+    const size_t n_vec = bytes / 16 / grid;                  // uint4 per CTA slice (stream mode)
+    const size_t moved = mode == 0 ? n_vec * 16 * grid * passes : n_rows * 256 * passes;
+    const int rows_per_warp = static_cast<int>((n_rows * passes / (static_cast<size_t>(grid) * (threads / 32)) + 7) / 8 * 8);
+    unsigned char *buf = nullptr;
+    unsigned *sink = nullptr;
+    int rc;
+    if ((rc = dev_alloc(&buf, bytes)) != XY_OK) return rc;
+    if ((rc = dev_alloc(&sink, 1)) != XY_OK) { cudaFree(buf); return rc; }
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaError_t e = cudaMemsetAsync(buf, 0, bytes, st);
+    if (e == cudaSuccess) e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    double best = 0.0;
+    for (int r = 0; r < repeats + 2 && e == cudaSuccess; ++r) {       // two untimed launches warm L2 and the clocks
+        e = cudaEventRecord(e0, st);
+        if (e != cudaSuccess) break;
+        if (mode == 0) xy::k_l2_stream<<<grid, threads, 0, st>>>(reinterpret_cast<const uint4 *>(buf), n_vec, passes, sink);
+        else xy::k_l2_gather<<<grid, threads, 0, st>>>(reinterpret_cast<const uint2 *>(buf), static_cast<uint32_t>(n_rows), rows_per_warp, sink);
+        e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaEventRecord(e1, st);
+        if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        const double bytes_done = mode == 0 ? static_cast<double>(moved)
+                                            : static_cast<double>(rows_per_warp) * grid * (threads / 32) * 256.0;
+        if (e == cudaSuccess && r >= 2 && ms > 0.f) best = std::max(best, bytes_done / (ms * 1e-3) * 1e-9);
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(buf); cudaFree(sink);
+    if (e != cudaSuccess) return fail(XY_ECUDA, std::string("xy_l2_bandwidth: ") + cudaGetErrorString(e));
+    *gbs_out = best;
     return XY_OK;
 }
-#endif
 
 int xy_synchronize(xy_pt *pt) {
     if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     XY_CUDA(cudaStreamSynchronize(pt->stream));
     return XY_OK;
 }

@@ -1,0 +1,25 @@
+// xy_dispatch.h -- host-side lookup of the k_phase / k_cycle instantiations.  The kernels are templates (xy_sweep.cuh,
+// xy_cycle.cuh); their instantiations are spread over several translation units (xy_inst_*.cu) so that the library
+// builds in parallel; xy_b200.cu only sees these function-pointer lookups.
+#pragma once
+
+namespace xy {
+
+constexpr int kCycleWarps = 16;      // warps per CTA of k_cycle (128 registers per thread, one CTA per SM)
+
+// k_phase<G, CB, MODE, W> for W in {8, 32} (MODE 0..5) and W = 24 (MODE 3, 5 only); CB = single_block ? 1 : 0 (G = 32 only).
+// nullptr for a combination that is not built.
+const void *phase_function(int W, int G, bool single_block, int mode);
+// k_cycle<G, ORDER, kCycleWarps>
+const void *cycle_function(int order, int G);
+
+// per translation unit
+const void *phase_function_w8_a(int G, bool single_block, int mode);    // modes 0, 1, 2
+const void *phase_function_w8_b(int G, bool single_block, int mode);    // modes 3, 4, 5
+const void *phase_function_w32_a(int G, bool single_block, int mode);
+const void *phase_function_w32_b(int G, bool single_block, int mode);
+const void *phase_function_w24(int G, bool single_block, int mode);     // modes 3, 5
+const void *cycle_function_o0(int G);
+const void *cycle_function_o1(int G);
+
+}  // namespace xy

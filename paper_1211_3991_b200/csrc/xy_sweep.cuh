@@ -20,8 +20,8 @@
 // over-relaxation of the same site from one gather (interleaved order, xy_set_order), 5 = 4 + measurement by-product.
 //
 // The launches of a PT cycle are captured in a CUDA graph with PROGRAMMATIC DEPENDENT LAUNCH edges (see k_phase).
-// A persistent cooperative variant (all phases of a cycle in one launch, per-sample barriers) was built and measured
-// in round 1 and removed: it lost to the per-phase launches at every BASELINE config.
+// Small samples run whole cycles in one launch instead: one thread-block cluster per sample with the hardware cluster
+// barrier between the colour classes (k_cycle, xy_cycle.cuh), built from the same sweep_prep / sweep_phase pieces.
 //
 // PAPER.md:444,:454 (coloured single-spin Metropolis), :460 (over-relaxation, ref 66), :167-181 (E, m),
 // :460-472 (parallel tempering); readings R5-R11, R20 in DESIGN.md.
@@ -236,6 +236,7 @@ struct SweepCtx {
     const float2 *ring_l;       // this lane's column of the warp's ring (generic pointer)
     uint32_t ring_s;            // same, shared-space address
     int s, lane, warp, sub, q;
+    long long *fx;              // the fixed-point sums the measuring modes add to ([S][R][3]; k_cycle alternates two buffers)
 };
 
 // what a warp stages BEFORE it waits for the preceding launch (graph data only, never theta): its share
@@ -356,7 +357,7 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
     // in global memory before 2^31 can be reached (rarely: same-address atomics are slow).  A site with more than 32
     // lower neighbours goes to the 64-bit sum directly.
     auto fx_lane = [&]() {      // this lane's six 64-bit sums (recomputed where needed: cold code, no live registers)
-        return reinterpret_cast<unsigned long long *>(a.fx) + (static_cast<size_t>(x.s) * a.R + 2 * x.q) * 3;
+        return reinterpret_cast<unsigned long long *>(x.fx) + (static_cast<size_t>(x.s) * a.R + 2 * x.q) * 3;
     };
     int units = 0;
     auto tally = [&](const float2 th, const float2 lx, const float2 ly, int nlow) {
@@ -463,7 +464,7 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
             // a single site with more neighbours than the staging slice: lane group 0 walks its ids in blocks
             const int ry = __shfl_sync(kFull, rc.y, 0);
             int deg = ry & 0xffff;
-            const int nlow = ry >> 16;
+            const int nlow = static_cast<int>(static_cast<uint32_t>(ry) >> 16);
             if constexpr (MODE == kModeMeasure) deg = nlow;      // lower neighbours only: the head of the list
             const int32_t *gidx = a.col_idx + start0;
             const bool valid = UNI || sub == 0;
@@ -491,6 +492,12 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
             __syncwarp();
             i0 += 1;
             staged = false;
+            if constexpr (kTally) {
+                if (units >= 320 && i0 < w1) {      // a run of hub sites must not overflow the 32-bit partial sums either
+                    flush_partial();
+                    units = 0;
+                }
+            }
             continue;
         }
 
@@ -509,7 +516,7 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
             st.i = i0 + m;
             st.deg = st.valid ? (ry & 0xffff) : 0;
             st.pos = rx;
-            st.nlow = st.valid ? (ry >> 16) : 0;
+            st.nlow = st.valid ? static_cast<int>(static_cast<uint32_t>(ry) >> 16) : 0;
             if constexpr (MODE == kModeMeasure) st.deg = st.nlow;   // bonds counted once: neighbours j < i are the head of the list
             return st;
         };
@@ -561,9 +568,9 @@ __device__ __forceinline__ void sweep_phase(const TileArgs &a, const SweepCtx &x
 
 // last CTA of a sample in a measure launch: fixed-point sums -> E, M per slot, optional accumulation under the
 // slot's temperature (Eq. 13-16); leaves fx zeroed for the next measure launch
-__device__ __forceinline__ void sweep_finalize(const TileArgs &a, int s, bool accumulate) {
+__device__ __forceinline__ void sweep_finalize(const TileArgs &a, long long *fx, int s, bool accumulate) {
     for (int r = threadIdx.x; r < a.R; r += blockDim.x) {
-        long long *f = a.fx + (static_cast<size_t>(s) * a.R + r) * 3;
+        long long *f = fx + (static_cast<size_t>(s) * a.R + r) * 3;
         const double e = -static_cast<double>(__ldcg(f)) * kInvScaleE;
         const double mx = static_cast<double>(__ldcg(f + 1)) * kInvScaleM;
         const double my = static_cast<double>(__ldcg(f + 2)) * kInvScaleM;
@@ -581,6 +588,27 @@ __device__ __forceinline__ void sweep_finalize(const TileArgs &a, int s, bool ac
     }
 }
 
+// the CTA's per-lane fixed-point partial sums -> one 64-bit atomic per (slot, quantity) and CTA; reuses the warps' ring
+// slices as scratch, so all warps of the CTA must have left sweep_phase (block-wide barriers inside)
+template <int G, int W>
+__device__ __forceinline__ void sweep_reduce_to_fx(const TileArgs &a, const SweepCtx &x, const int (&iacc)[6], SweepWarp *s_w) {
+    constexpr int SPW = 32 / G;
+    __syncthreads();
+    long long *s_red = reinterpret_cast<long long *>(&s_w[0]);
+#pragma unroll
+    for (int c = 0; c < 6; ++c) s_red[(x.warp * 32 + x.lane) * 6 + c] = static_cast<long long>(iacc[c]);
+    __syncthreads();
+    if (threadIdx.x < G * 6) {
+        const int ll = threadIdx.x / 6, c = threadIdx.x % 6;
+        long long v = 0;
+        for (int wi = 0; wi < W; ++wi)
+            for (int sb = 0; sb < SPW; ++sb) v += s_red[(wi * 32 + sb * G + ll) * 6 + c];
+        const int slot = 2 * (blockIdx.z * G + ll) + c / 3;
+        atomicAdd(reinterpret_cast<unsigned long long *>(x.fx) + (static_cast<size_t>(x.s) * a.R + slot) * 3 + c % 3,
+                  static_cast<unsigned long long>(v));
+    }
+}
+
 // ---- the kernel: one colour class (or the measure pass) per launch, so each mode gets its own register allocation
 // (64 registers, no spills) and the hardware does the grid-wide ordering between colour classes.  grid (x = CTAs per
 // sample and column block, y = samples of the group, z = blocks of 64 slots).
@@ -593,24 +621,12 @@ __device__ __forceinline__ void sweep_finalize(const TileArgs &a, int s, bool ac
 // to the fixed-point sums (the measurement costs no extra gather), converted by the launch of the sweep's last colour.
 // MODE 4 / 5 (interleaved order, xy_set_order): Metropolis and then over-relaxation of every site of the class from one
 // gather, without / with the measurement by-product.
-#ifdef XY_TRACE   // tuning builds only (_work): per-warp time stamps of the last k_phase launch
-__device__ unsigned long long g_trace[8192][4];
-__device__ __forceinline__ unsigned long long trace_now() {
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    return t;
-}
-#endif
 
 template <int G, int CB, int MODE, int W>
 __global__ void __launch_bounds__(W * 32, W == 24 ? 1 : kSmPerWarpSlots / W) k_phase(const SweepArgs a) {
     extern __shared__ __align__(16) unsigned char s_raw[];
     SweepWarp *s_w = reinterpret_cast<SweepWarp *>(s_raw);
     __shared__ int s_last;
-    constexpr int SPW = 32 / G;
-#ifdef XY_TRACE
-    const unsigned long long tr0 = trace_now();
-#endif
 
     SweepCtx x;
     x.s = a.t.s0 + blockIdx.y;
@@ -625,6 +641,7 @@ __global__ void __launch_bounds__(W * 32, W == 24 ? 1 : kSmPerWarpSlots / W) k_p
     x.sidx = s_w[x.warp].idx;
     x.ring_l = &s_w[x.warp].ring[0][0][x.lane];
     x.ring_s = static_cast<uint32_t>(__cvta_generic_to_shared(x.ring_l));
+    x.fx = a.t.fx;
 
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     const PhasePrep P = sweep_prep<G, CB, W>(a, x, MODE == kModeMeasure ? kModeMeasure : kModeOverrelax, a.t.colour);
@@ -633,34 +650,10 @@ __global__ void __launch_bounds__(W * 32, W == 24 ? 1 : kSmPerWarpSlots / W) k_p
 
     int iacc[6] = {0, 0, 0, 0, 0, 0};
     const uint32_t sweep = a.t.use_counter ? a.t.counters[0] + static_cast<uint32_t>(a.t.sweep_offset) : a.t.sweep_fixed;
-#ifdef XY_TRACE
-    const unsigned long long tr1 = trace_now();
-#endif
     sweep_phase<G, CB, MODE>(a.t, x, P, sweep, iacc);
-#ifdef XY_TRACE
-    if (x.lane == 0 && blockIdx.y == 0 && blockIdx.z == 0 && blockIdx.x * W + x.warp < 8192) {
-        unsigned long long *o = g_trace[blockIdx.x * W + x.warp];
-        unsigned smid;
-        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-        o[0] = tr0; o[1] = tr1; o[2] = trace_now(); o[3] = (static_cast<unsigned long long>(smid) << 32) | static_cast<unsigned>(P.w1 - P.i0);
-    }
-#endif
 
     if constexpr (MODE == kModeMeasure || MODE == kModeOrMeasure || MODE == kModeMetOrMeasure) {
-        __syncthreads();
-        long long *s_red = reinterpret_cast<long long *>(&s_w[0]);
-#pragma unroll
-        for (int c = 0; c < 6; ++c) s_red[(x.warp * 32 + x.lane) * 6 + c] = static_cast<long long>(iacc[c]);
-        __syncthreads();
-        if (threadIdx.x < G * 6) {
-            const int ll = threadIdx.x / 6, c = threadIdx.x % 6;
-            long long v = 0;
-            for (int wi = 0; wi < W; ++wi)
-                for (int sb = 0; sb < SPW; ++sb) v += s_red[(wi * 32 + sb * G + ll) * 6 + c];
-            const int slot = 2 * (blockIdx.z * G + ll) + c / 3;
-            atomicAdd(reinterpret_cast<unsigned long long *>(a.t.fx) + (static_cast<size_t>(x.s) * a.t.R + slot) * 3 + c % 3,
-                      static_cast<unsigned long long>(v));
-        }
+        sweep_reduce_to_fx<G, W>(a.t, x, iacc, s_w);
         // the sums are complete after the measure launch, or after the fused launch of the sweep's last colour
         // (a.t.accumulate bit 1); its last CTA converts them
         if (MODE == kModeMeasure || (a.t.accumulate & 2)) {
@@ -673,7 +666,7 @@ __global__ void __launch_bounds__(W * 32, W == 24 ? 1 : kSmPerWarpSlots / W) k_p
             __syncthreads();
             if (s_last) {
                 __threadfence();
-                sweep_finalize(a.t, x.s, (a.t.accumulate & 1) != 0);
+                sweep_finalize(a.t, x.fx, x.s, (a.t.accumulate & 1) != 0);
                 if (threadIdx.x == 0) a.t.ticket[x.s] = 0u;
             }
         }

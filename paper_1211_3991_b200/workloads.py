@@ -62,3 +62,10 @@ CONFIGS = {
 def lscan(L):
     """config 3's throughput scan: L in {32, 64, 128, 256} at 512 replica-samples (R=32 x S=16)."""
     return CONFIGS[3].scaled(name=f"config3b_L{L}_rho4.5_R32_S16", L=L)
+
+
+def square_lattice(L, R, T_min, T_max, S, name=None):
+    """rho -> infinity at z = 4 is the periodic square lattice, Q = 2 colours: the paper's KT
+    benchmark and, with L = 128, the shape of its timing experiment (Table III, PAPER.md:474-494:
+    square lattice, N = 2^14, PBC).  Built by the shared builder with rho = 100 (every other bond has weight <= 2^-50)."""
+    return Workload(name or f"square_L{L}_z4_R{R}_S{S}", L, 100.0, 4, R, T_min, T_max, S, 0)

@@ -26,24 +26,45 @@ def ensemble_from_graph(gd, T, seed, S=1, sample_base=0):
     return B.Ensemble(rp, ci, col, T, seed, sample_base=sample_base)
 
 
+class _Theta:
+    """theta of the ensemble on the host: the whole state (xy_get_theta), or -- for the full-size tests, where the state
+    is hundreds of MB -- only the samples asked for, read from the torch tensor the Ensemble owns (device memory is torch's
+    job; the stream is synchronised first)."""
+
+    def __init__(self, ens, samples):
+        if samples is None:
+            self.full, self.part = ens.get_theta(), None
+        else:
+            ens.synchronize()
+            self.full, self.part = None, {s: ens.theta[s].cpu().numpy() for s in samples}
+
+    def __getitem__(self, s):
+        return self.full[s] if self.part is None else self.part[s]
+
+
+def read_theta(ens, samples=None, sparse=False):
+    return _Theta(ens, samples if sparse else None)
+
+
 def slot_params(T, labels_s):
     beta_f, w_f = O.temperature_params(T)
     return beta_f[labels_s], w_f[labels_s]
 
 
-def lockstep_metropolis(ens, graphs, T, seed, colour, sweep, samples=None, site_subset=None, sample_base=0, rng=None):
+def lockstep_metropolis(ens, graphs, T, seed, colour, sweep, samples=None, site_subset=None, sample_base=0, rng=None,
+                        sparse=False):
     """Run Metropolis on one colour class on the GPU and on the oracle from the same pre-state.
     graphs: list of (row_ptr, col_idx, class_ptr) per sample.  Returns a dict of counts; raises on mismatch."""
-    pre = ens.get_theta()
+    pre = read_theta(ens, samples, sparse)
     labels = ens.get_labels()
     ens.metropolis_colour(colour, sweep)
-    post = ens.get_theta()
+    post = read_theta(ens, samples, sparse)
     stats = dict(updates=0, near=0, bad=0, maxerr=0.0, accepted=0, disagree_near=0)
     for s in (range(ens.S) if samples is None else samples):
         rp, ci, cp = graphs[s]
         lo, hi = (int(cp[colour]), int(cp[colour + 1])) if colour + 1 < len(cp) else (0, 0)
         # everything outside the class must be untouched, bit for bit
-        assert np.array_equal(post[s, :lo], pre[s, :lo]) and np.array_equal(post[s, hi:], pre[s, hi:])
+        assert np.array_equal(post[s][:lo], pre[s][:lo]) and np.array_equal(post[s][hi:], pre[s][hi:])
         sites = np.arange(lo, hi, dtype=np.int32)
         if site_subset is not None and len(sites) > site_subset:
             sites = np.sort(rng.choice(sites, site_subset, replace=False)).astype(np.int32)
@@ -52,7 +73,7 @@ def lockstep_metropolis(ens, graphs, T, seed, colour, sweep, samples=None, site_
         bs, ws = slot_params(T, labels[s])
         ref = pre[s].copy()
         margin, acc = O.metropolis_sites(rp, ci, ref, sites, bs, ws, seed, sweep, sample_base + s, want_margin=True)
-        err = circ(post[s, sites], ref[sites])
+        err = circ(post[s][sites], ref[sites])
         near = margin < BAND
         stats["updates"] += err.size
         stats["near"] += int(near.sum())
@@ -65,15 +86,15 @@ def lockstep_metropolis(ens, graphs, T, seed, colour, sweep, samples=None, site_
     return stats
 
 
-def lockstep_overrelax(ens, graphs, colour, samples=None, site_subset=None, rng=None):
-    pre = ens.get_theta()
+def lockstep_overrelax(ens, graphs, colour, samples=None, site_subset=None, rng=None, sparse=False):
+    pre = read_theta(ens, samples, sparse)
     ens.overrelax_colour(colour)
-    post = ens.get_theta()
+    post = read_theta(ens, samples, sparse)
     stats = dict(updates=0, illcond=0, bad=0, maxerr_scaled=0.0, maxerr_wellcond=0.0)
     for s in (range(ens.S) if samples is None else samples):
         rp, ci, cp = graphs[s]
         lo, hi = (int(cp[colour]), int(cp[colour + 1])) if colour + 1 < len(cp) else (0, 0)
-        assert np.array_equal(post[s, :lo], pre[s, :lo]) and np.array_equal(post[s, hi:], pre[s, hi:])
+        assert np.array_equal(post[s][:lo], pre[s][:lo]) and np.array_equal(post[s][hi:], pre[s][hi:])
         sites = np.arange(lo, hi, dtype=np.int32)
         if site_subset is not None and len(sites) > site_subset:
             sites = np.sort(rng.choice(sites, site_subset, replace=False)).astype(np.int32)
@@ -81,7 +102,7 @@ def lockstep_overrelax(ens, graphs, colour, samples=None, site_subset=None, rng=
             continue
         ref = pre[s].copy()
         hn = O.overrelax_sites(rp, ci, ref, sites, want_hnorm=True)
-        err = circ(post[s, sites], ref[sites])
+        err = circ(post[s][sites], ref[sites])
         scaled = err * np.minimum(1.0, hn)
         stats["updates"] += err.size
         stats["illcond"] += int(((err > TOL) & (scaled <= TOL)).sum())     # pass only through the |h| factor (R7)
@@ -97,19 +118,20 @@ def graphs_of_levy(g):
     return [(g.row_ptr[s], g.col_idx[s], g.class_ptr(s)) for s in range(g.S)]
 
 
-def lockstep_metor(ens, graphs, T, seed, colour, sweep, samples=None, site_subset=None, sample_base=0, rng=None):
+def lockstep_metor(ens, graphs, T, seed, colour, sweep, samples=None, site_subset=None, sample_base=0, rng=None,
+                   sparse=False):
     """interleaved order: Metropolis then over-relaxation of one colour class in one launch, against the oracle's
     two calls from the same pre-state.  Sites whose Metropolis decision is near threshold (R6) are excluded and
     counted; the rest must satisfy the |h|-weighted over-relaxation bar (R7)."""
-    pre = ens.get_theta()
+    pre = read_theta(ens, samples, sparse)
     labels = ens.get_labels()
     ens.metor_colour(colour, sweep)
-    post = ens.get_theta()
+    post = read_theta(ens, samples, sparse)
     stats = dict(updates=0, near=0, bad=0, illcond=0, accepted=0)
     for s in (range(ens.S) if samples is None else samples):
         rp, ci, cp = graphs[s]
         lo, hi = (int(cp[colour]), int(cp[colour + 1])) if colour + 1 < len(cp) else (0, 0)
-        assert np.array_equal(post[s, :lo], pre[s, :lo]) and np.array_equal(post[s, hi:], pre[s, hi:])
+        assert np.array_equal(post[s][:lo], pre[s][:lo]) and np.array_equal(post[s][hi:], pre[s][hi:])
         sites = np.arange(lo, hi, dtype=np.int32)
         if site_subset is not None and len(sites) > site_subset:
             sites = np.sort(rng.choice(sites, site_subset, replace=False)).astype(np.int32)
@@ -119,7 +141,7 @@ def lockstep_metor(ens, graphs, T, seed, colour, sweep, samples=None, site_subse
         ref = pre[s].copy()
         margin, acc = O.metropolis_sites(rp, ci, ref, sites, bs, ws, seed, sweep, sample_base + s, want_margin=True)
         hn = O.overrelax_sites(rp, ci, ref, sites, want_hnorm=True)
-        err = circ(post[s, sites], ref[sites])
+        err = circ(post[s][sites], ref[sites])
         scaled = err * np.minimum(1.0, hn)
         near = margin < BAND
         stats["updates"] += err.size

@@ -59,8 +59,9 @@ def test_lockstep_one_sweep_metropolis_and_overrelax(L, rho, R, S):
             assert st["bad"] == 0, st
     assert tot_m["updates"] == 3 * L * L * R * S and tot_o["updates"] == 3 * L * L * R * S
     assert 0.2 < tot_m["accepted"] / tot_m["updates"] < 0.95
-    assert tot_m["near"] <= 5 + 2e-4 * tot_m["updates"]              # expected ~2e-5 per update
-    assert tot_o["illcond"] <= 5 + 5e-3 * tot_o["updates"]           # <= 0.17 % at T = inf
+    assert tot_m["near"] <= 10 + 6e-5 * tot_m["updates"]             # expected 1e-5 .. 2e-5 per update (R6)
+    n_o = tot_o["updates"]
+    assert tot_o["illcond"] <= 3 + 1.7e-3 * n_o + 5 * np.sqrt(1.7e-3 * n_o)     # <= 0.17 % at T = inf, + 5 sigma
     print(f"\n[lockstep L={L} R={R} S={S}] metropolis {tot_m}  overrelax {tot_o}")
     th = ens.get_theta()
     assert th.min() >= 0.0 and th.max() <= np.float32(6.2831855)
@@ -69,7 +70,7 @@ def test_lockstep_one_sweep_metropolis_and_overrelax(L, rho, R, S):
 
 @pytest.mark.parametrize("R", [8, 2, 16, 32, 64, 128, 6])
 def test_metropolis_sweep_trajectory_config0(R):
-    """full Metropolis sweeps (all colours in one persistent launch) from an identical state: angles are
+    """full Metropolis sweeps (xy_sweep: one launch per colour class) from an identical state: angles are
     BIT-identical to the oracle's until the first near-threshold decision (R5: the accepted angle is the same
     fp32 number on both sides).  config 0's graph; R = 8 is config 0 itself, the other R cover every kernel flavour."""
     w = workloads.CONFIGS[0]
@@ -194,22 +195,47 @@ def test_run_equals_stepwise_calls_and_schedule_invariance():
     for e in (a, b, c): e.close()
 
 
-def test_run_matches_oracle_protocol_short():
-    """two full cycles on config 0 against orc_run: labels, counters and accumulated observables agree as long
-    as no decision was near threshold (angles are compared in lockstep elsewhere; here the protocol order,
-    measurement cadence and swap bookkeeping are what is checked)."""
-    w = workloads.CONFIGS[0]
-    g = levy.build(w.L, w.rho, w.z, w.seed, S=1)
-    T = w.temperatures()
-    ens = U.ensemble_from_levy(g, T, SEED)
-    ch = O.Chain(g.row_ptr[0], g.col_idx[0], g.class_ptr(0), T, SEED)
-    ens.run(1, 2, 1, 1); ch.run(1, 2, 1, 1)
-    acc = ens.read_accumulators()[0]
-    assert np.array_equal(acc[:, 0], ch.acc[:, 0])
-    assert np.allclose(acc[:, 1], ch.acc[:, 1], rtol=0, atol=2e-3)            # sum of 2 energies, chaotic drift small
-    assert np.allclose(acc[:, 4], ch.acc[:, 4], rtol=0, atol=1e-4)
-    assert np.array_equal(ens.get_labels()[0], ch.temp_of_slot)
-    assert U.circ(ens.get_theta()[0], ch.theta).mean() < 1e-3
+@pytest.mark.parametrize("order", [0, 1])
+def test_run_matches_oracle_protocol_full_cycles(order):
+    """xy_run against the oracle's protocol over FULL PT cycles (10 sweeps x (Metropolis, over-relaxation, measure) + a
+    swap round each): the order of the phases, the measurement cadence, the filing under temperatures and the swap
+    bookkeeping.  The chain is chaotic, so the comparison is exact only while no decision falls near its threshold:
+    tests/protocol.py replays the oracle's loop (bit-identical to orc_run_order, tests/test_oracle_equilibrium.py) and
+    reports the smallest decision margin so far; a seed is searched (deterministically) whose first cycles stay 1e-4
+    away from every threshold and that accepts a swap.  While that holds: labels bit-exact, accumulator counts exact,
+    angles within 1e-3 rad (a phase out of order moves angles by ~3 rad: checked on the oracle side, same file), energies
+    and m^2 sums within the fp32 drift.  Afterwards only the integer bookkeeping is compared."""
+    import protocol as P
+    L, R, sps = 8, 8, 10
+    g = small_levy(L, 3.5, 1)
+    T = O.geometric_temperatures(R, 1.0, 4.0)
+    rp, ci, cp = g.row_ptr[0], g.col_idx[0], g.class_ptr(0)
+    n_cycles = 4
+    for seed in range(2, 200):
+        h = P.run_with_margins(rp, ci, cp, T, seed, n_cycles, sps, 1, 1, order=order)
+        safe = [k for k in range(n_cycles) if min(h[k]["min_margin"], h[k]["min_swap_margin"]) > 1e-4]
+        if safe and any(not np.array_equal(h[k]["temp_of_slot"], np.arange(R)) for k in safe):
+            break
+    else:
+        pytest.fail("no seed with a threshold-free first cycle")
+    ens = U.ensemble_from_levy(g, T, seed)
+    ens.set_order(order)
+    worst = 0.0
+    for k in range(n_cycles):
+        ens.run(1, sps, 1, 1)
+        acc = ens.read_accumulators()[0]
+        sw, rd, att, accd = ens.get_counters()
+        assert (sw, rd) == ((k + 1) * sps, k + 1)
+        assert np.array_equal(acc[:, 0], h[k]["acc"][:, 0])
+        if k in safe:
+            assert np.array_equal(ens.get_labels()[0], h[k]["temp_of_slot"]), f"cycle {k}"
+            err = U.circ(ens.get_theta()[0], h[k]["theta"]).max()
+            worst = max(worst, err)
+            assert err < 1e-3, f"cycle {k}: max |dtheta| {err}"
+            assert np.allclose(acc[:, 1], h[k]["acc"][:, 1], rtol=0, atol=2e-2)
+            assert np.allclose(acc[:, 4], h[k]["acc"][:, 4], rtol=0, atol=2e-4)
+            assert np.allclose(acc[:, 6:8], h[k]["acc"][:, 6:8], rtol=0, atol=2e-3)
+    print(f"\n[protocol order {order}] seed {seed}: {len(safe)} threshold-free cycles compared, max |dtheta| {worst:.2e}")
     ens.close()
 
 
@@ -405,4 +431,88 @@ def test_thousand_replicas_sixteen_column_blocks():
     assert np.all(np.abs(E - Eo) <= 4e-7 * 192 + 1e-5)
     with pytest.raises(B.XYError):
         U.ensemble_from_levy(g, O.geometric_temperatures(1025, 1.0, 4.0), SEED)
+    ens.close()
+
+
+def test_free_boundary_levy_graph_lockstep_and_cycle():
+    """a FREE-boundary Levy sample (Fig. 14; DESIGN R21) through xy_graph_load: lockstep parity of
+    every colour class in all three update modes, then captured cycles and the energy against the oracle's fp64 sum."""
+    L, R, S = 16, 16, 2
+    g = levy.build(L, 3.0, 6, workloads.BASE_SEED, S=S, boundary="free")
+    lat = g.new_to_old[0]
+    x, y = lat % L, lat // L
+    d = np.hypot((x[:, None] - x[None, :]), (y[:, None] - y[None, :]))
+    rp, ci = g.row_ptr[0], g.col_idx[0]
+    blen = np.concatenate([d[i, ci[rp[i]:rp[i + 1]]] for i in range(L * L)])
+    assert blen.max() > (L // 2) * np.sqrt(2) and blen.max() <= (L - 1) * np.sqrt(2) + 1e-9      # longer than any periodic bond
+    T = O.geometric_temperatures(R, 1.0, 4.0)
+    ens = U.ensemble_from_levy(g, T, SEED)
+    graphs = U.graphs_of_levy(g)
+    ens.run(2, 10, 1, 1)
+    for c in range(int(g.n_colours.max())):
+        assert U.lockstep_metropolis(ens, graphs, T, SEED, c, 21)["bad"] == 0
+        assert U.lockstep_overrelax(ens, graphs, c)["bad"] == 0
+        assert U.lockstep_metor(ens, graphs, T, SEED, c, 22)["bad"] == 0
+    E = ens.get_energy(); th = ens.get_theta()
+    for s in range(S):
+        Eo, _, _ = O.measure(g.row_ptr[s], g.col_idx[s], th[s])
+        assert np.all(np.abs(E[s] - Eo) <= 4e-7 * 3 * L * L)
+    ens.close()
+
+
+@pytest.mark.parametrize("order", [0, 1])
+def test_sample_shards_reproduce_the_whole_ensemble_bit_for_bit(order):
+    """the path shards by graph sample with no data-path collective.  Rank r of a 2-rank job builds global
+    samples 4r .. 4r+3 (sample_base = 4r) and runs them alone; its angles, labels, accumulators and swap counters after
+    xy_run equal samples 4r .. 4r+3 of the single 8-sample ensemble bit for bit."""
+    L, R, S = 16, 16, 8
+    T = O.geometric_temperatures(R, 1.0, 4.0)
+    g = small_levy(L, 3.5, S)
+    whole = U.ensemble_from_levy(g, T, SEED)
+    whole.set_order(order)
+    whole.run(3, 10, 1, 1)
+    th, lab, acc = whole.get_theta(), whole.get_labels(), whole.read_accumulators()
+    _, _, att, accd = whole.get_counters()
+    whole.close()
+    for rank in (0, 1):
+        gs = small_levy(L, 3.5, S // 2, sample_base=rank * (S // 2))
+        assert np.array_equal(gs.col_idx, g.col_idx[rank * 4:rank * 4 + 4])
+        part = U.ensemble_from_levy(gs, T, SEED, sample_base=rank * (S // 2))
+        part.set_order(order)
+        part.run(3, 10, 1, 1)
+        sl = slice(rank * 4, rank * 4 + 4)
+        assert np.array_equal(part.get_theta(), th[sl])
+        assert np.array_equal(part.get_labels(), lab[sl])
+        assert np.array_equal(part.read_accumulators(), acc[sl])
+        _, _, a2, c2 = part.get_counters()
+        assert np.array_equal(a2, att[sl]) and np.array_equal(c2, accd[sl])
+        part.close()
+
+
+def test_run_of_hub_sites_does_not_overflow_the_fixed_point_partial_sums():
+    """sites with more neighbours than the staging slice take the one-site path of k_phase; a long run of them
+    in one warp's share (each adding up to 2^24 to the 32-bit partial energy sums) must be flushed like ordinary chunks.
+    140 consecutive hubs per warp, each with 32 lower and 240 higher neighbours, all spins aligned: E = -(number of
+    bonds) exactly (cos 0 = 1 in fp32 and in fixed point), in the stand-alone measure pass and in the fused modes."""
+    nA, nH, nB = 32, 1120, 240
+    N = nA + nH + nB
+    edges = [(a, nA + h) for a in range(nA) for h in range(nH)] + [(nA + h, nA + nH + b) for h in range(nH) for b in range(nB)]
+    rp, ci = G.csr_from_edges(N, edges)
+    col = np.concatenate([np.zeros(nA), np.ones(nH), np.full(nB, 2)]).astype(np.int32)      # already colour-major
+    S, R = 19, 1024                                  # 19 x 16 column blocks: one 8-warp CTA per (sample, block)
+    T = O.geometric_temperatures(R, 0.5, 1.0)
+    ens = B.Ensemble(np.tile(rp, (S, 1)), np.tile(ci, (S, 1)), np.tile(col, (S, 1)), T, SEED,
+                     width=np.zeros(R))               # zero proposal width: Metropolis never moves a spin
+    ens.set_tuning(cta_shape=1)
+    ens.set_theta(np.zeros((S, N, R), np.float32))
+    want = np.full((S, R), -float(len(edges)))
+    assert np.array_equal(ens.get_energy(), want)                      # stand-alone measure pass (MODE 2)
+    out = ens.measure(want=True)
+    assert np.array_equal(out[..., 0], want) and np.array_equal(out[..., 1], np.full((S, R), float(N)))
+    # fused measurement (MODE 3, then MODE 5): over-relaxation maps the aligned state onto itself (theta' = 2 * 0 - 0)
+    for order in (0, 1):
+        ens.set_order(order)
+        ens.run(1, 2, 1, 1)
+        assert np.array_equal(ens.get_energy(), want), order
+        assert not ens.get_theta().any()
     ens.close()

@@ -52,3 +52,48 @@ def test_erdos_renyi_z4_binder_crossing_at_the_analytic_tc(order):
     assert abs(cross[(64, 128)] - TC_ER_Z4) < 0.03
     assert abs(cross[(32, 64)] - TC_ER_Z4) < 0.06
     assert abs(cross[(64, 128)] - TC_ER_Z4) <= abs(cross[(32, 64)] - TC_ER_Z4) + 0.01     # converging with size
+
+
+TC_SQUARE = paper_value("tc_square_lattice")         # 0.8929
+ETA_KT = paper_value("eta_kt_at_tc")                 # 1/4,    PAPER.md:278 Eq. 27
+R_KT = paper_value("r_kt_log")                       # 1/16
+
+
+def test_square_lattice_kt_susceptibility_exponent_at_the_paper_tc():
+    """The paper's own benchmark of its algorithm: on the 2D square lattice (the rho = infinity
+    limit, z = 4, two colours) the susceptibility at T_c = 0.8929 scales as chi ~ L^(2 - eta)
+    (ln L)^(-2r) with eta = 1/4, r = 1/16 (Eq. 27); eta(T) = the exponent "numerically interpolating Eq. (27) at
+    different temperatures" grows with T, passes 1/4 at T_c, and chi stops growing with L in the vortex phase.
+    chi = N <m^2> (item (3): <m>^2 is negligible).  L = 16, 32, 64; 16 independent copies of the lattice."""
+    T = np.sort(np.append(np.linspace(0.70, 1.30, 15), TC_SQUARE))
+    k_c = int(np.where(T == TC_SQUARE)[0][0])
+    lnchi, err = {}, {}
+    for L in (16, 32, 64):
+        w = workloads.square_lattice(L, len(T), T[0], T[-1], 16)
+        g = levy.build(w.L, w.rho, w.z, w.seed, S=1)
+        assert int(g.n_colours[0]) == 2 and np.all(np.diff(g.row_ptr[0]) == 4)
+        ens = B.Ensemble(np.tile(g.row_ptr, (w.S, 1)), np.tile(g.col_idx, (w.S, 1)), np.tile(g.colour, (w.S, 1)), T, 0x2D0000 + L)
+        ens.run(2000, 10, 1, 1)
+        blocks = []
+        for _ in range(20):
+            ens.reset_accumulators()
+            ens.run(400, 10, 1, 1)
+            blocks.append(ens.read_accumulators().sum(0))             # pool the 16 copies of the same lattice
+        ens.close()
+        est, sig = S.jackknife(np.array(blocks), lambda m: np.log(L * L * m[..., S.M2_]))
+        lnchi[L], err[L] = est, sig
+    x = np.log(np.array([16.0, 32.0, 64.0]))
+    y = np.array([lnchi[L] + 2 * R_KT * np.log(np.log(L)) for L in (16, 32, 64)])        # Eq. 27 with the log factor removed
+    slope = ((x - x.mean())[:, None] * (y - y.mean(0))).sum(0) / ((x - x.mean()) ** 2).sum()
+    eta = 2.0 - slope
+    print("\nsquare lattice: T        " + " ".join(f"{t:6.3f}" for t in T))
+    print("                eta(T)   " + " ".join(f"{e:6.3f}" for e in eta))
+    print(f"eta at the paper's T_c = {TC_SQUARE}: {eta[k_c]:.4f} (paper / KT theory: {ETA_KT}); max jackknife sigma of ln chi {max(e.max() for e in err.values()):.1e}")
+    assert abs(eta[k_c] - ETA_KT) < 0.03
+    assert np.all(np.diff(eta) > -0.01)                  # eta grows with T
+    assert eta[0] < 0.20 and eta[-1] > 1.0               # spin-wave phase below, saturating chi above
+    # the temperature at which eta = 1/4 (the paper's "independent estimate" T_c = 0.894(5), PAPER.md:278)
+    k = int(np.where((eta[:-1] < ETA_KT) & (eta[1:] >= ETA_KT))[0][0])
+    t_eta = T[k] + (T[k + 1] - T[k]) * (ETA_KT - eta[k]) / (eta[k + 1] - eta[k])
+    print(f"T(eta = 1/4) = {t_eta:.4f}")
+    assert abs(t_eta - TC_SQUARE) < 0.03

@@ -198,3 +198,26 @@ def test_interleaved_order_ring_closed_form_and_differs_from_default():
     a = O.Chain(g["row_ptr"], g["col_idx"], g["class_ptr"], T, SEED); a.run(1, 2, 1, 1, 0)
     b = O.Chain(g["row_ptr"], g["col_idx"], g["class_ptr"], T, SEED); b.run(1, 2, 1, 1, 1)
     assert not np.array_equal(a.theta, b.theta)                   # genuinely another order
+
+
+@pytest.mark.parametrize("order", [0, 1])
+def test_protocol_replay_is_bit_identical_to_orc_run_and_order_sensitive(order):
+    """tests/protocol.py (the PT cycle spelled out with the single-step oracle calls, used by the GPU protocol test to
+    watch the decision margins) reproduces orc_run_order bit for bit; and running ONE phase out of order (over-relaxation
+    before Metropolis on the last colour) moves angles by O(1) within a cycle -- the GPU test's 1e-3 rad bar notices it."""
+    import protocol as P
+    from paper_1211_3991_b200 import levy, workloads
+    g = levy.build(8, 3.5, 6, workloads.BASE_SEED, S=1)
+    T = O.geometric_temperatures(8, 1.0, 4.0)
+    rp, ci, cp = g.row_ptr[0], g.col_idx[0], g.class_ptr(0)
+    h = P.run_with_margins(rp, ci, cp, T, 7, 3, 10, 1, 1, order=order)
+    ch = O.Chain(rp, ci, cp, T, 7)
+    ch.run(3, 10, 1, 1, order=order)
+    assert np.array_equal(h[-1]["theta"], ch.theta)
+    assert np.array_equal(h[-1]["temp_of_slot"], ch.temp_of_slot)
+    assert np.array_equal(h[-1]["acc"], ch.acc)
+    assert 0 < h[-1]["min_margin"] < 1e-2 and 0 < h[-1]["min_swap_margin"] < 1.0
+    if order == 0:
+        bad = P.run_with_margins(rp, ci, cp, T, 7, 1, 10, 1, 1, mutate="or_first_last_colour")
+        d = np.abs(bad[0]["theta"].astype(np.float64) - h[0]["theta"])
+        assert np.minimum(d, 2 * np.pi - d).max() > 1.0
