@@ -113,7 +113,7 @@ def oracle_replicas(w):
     return min(w.R, 16)
 
 
-def oracle_sample_run(w, n_steps, n_warmup, seed=0xBA5E):
+def oracle_sample_run(w, n_steps, n_warmup, seed=0xBA5E, reduce_colours=0):
     """The ONE cpu_baseline definition used by both arms: the oracle as it stands (gcc -O2, fp64, one thread pinned to
     one core) on graph sample 0 of workload w restricted to the first oracle_replicas(w) temperature slots; each step =
     one Metropolis sweep + or_per_sweep over-relaxation sweeps + one measurement + one swap round (orc_run_order with
@@ -122,7 +122,7 @@ def oracle_sample_run(w, n_steps, n_warmup, seed=0xBA5E):
     import oracle as O
     from paper_1211_3991_b200 import levy
     n_rep = oracle_replicas(w)
-    g = levy.build(w.L, w.rho, w.z, w.seed, S=1)
+    g = levy.build(w.L, w.rho, w.z, w.seed, S=1, reduce_colours=reduce_colours)
     T = w.temperatures()[:n_rep]
     ch = O.Chain(g.row_ptr[0], g.col_idx[0], g.class_ptr(0), T, seed)
     O.lib()
@@ -147,9 +147,9 @@ def oracle_sample_run(w, n_steps, n_warmup, seed=0xBA5E):
     return updates / dt * 1e-9, dt, what
 
 
-def workload_config(w, world, measure_every, colours, max_degree):
+def workload_config(w, world, measure_every, colours, max_degree, colouring, class_sizes):
     """the `config` object -- identical in both arms"""
-    return {"workload": w.name, "L": w.L, "N": w.N, "rho": w.rho, "z": w.z, "R": w.R, "S_per_gpu": w.S,
+    return {"colouring": colouring, "class_sizes_sample0": class_sizes, "workload": w.name, "L": w.L, "N": w.N, "rho": w.rho, "z": w.z, "R": w.R, "S_per_gpu": w.S,
             "T_min": w.T_min, "T_max": w.T_max, "sweeps_per_step": w.sweeps_per_swap, "or_per_sweep": w.or_per_sweep,
             "measure_every": measure_every, "colours": colours, "max_degree": max_degree,
             "step": "one PT cycle: sweeps_per_step x (Metropolis + OR + measure) + one swap round",
@@ -162,14 +162,15 @@ def run_reference(args, w, rank, world):
     """--impl reference: the oracle on the host cores (single pinned thread), a bounded sample per step."""
     if rank != 0:
         return
-    from paper_1211_3991_b200 import levy
-    g = levy.build(w.L, w.rho, w.z, w.seed, S=w.S)
-    val, dt, what = oracle_sample_run(w, args.steps, args.warmup)
+    from paper_1211_3991_b200 import levy, workloads
+    g = levy.build(w.L, w.rho, w.z, w.seed, S=w.S, reduce_colours=workloads.REDUCE_COLOURS if args.colouring == "reduced" else 0)
+    val, dt, what = oracle_sample_run(w, args.steps, args.warmup, reduce_colours=workloads.REDUCE_COLOURS if args.colouring == "reduced" else 0)
     model, cores = host_cpu()
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dt / max(args.steps, 1) * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(w, world, args.measure_every, int(g.n_colours.max()), int(np.diff(g.row_ptr, axis=1).max())),
+            "config": workload_config(w, world, args.measure_every, int(g.n_colours.max()), int(np.diff(g.row_ptr, axis=1).max()),
+                                      args.colouring, np.bincount(g.colour[0]).tolist()),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what, "steps": args.steps,
                              "seconds": dt, "host_cpu": model, "host_cores": cores},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -190,6 +191,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-interleaved", action="store_true", help="skip the interleaved-order measurement")
+    ap.add_argument("--colouring", default="reduced", choices=["reduced", "smallest-last"],
+                    help="reduced = smallest-last followed by the builder's colour-reducing local search (default)")
     ap.add_argument("--no-aux", action="store_true", help="skip every auxiliary stderr line")
     ap.add_argument("--no-lscan", action="store_true", help="skip config 3's L scan (auxiliary JSON lines on stderr)")
     ap.add_argument("--no-table3", action="store_true", help="skip the paper's Table III workload (auxiliary lines on stderr)")
@@ -226,7 +229,8 @@ def main():
 
     # ---- synthetic inputs: this rank's S samples (global ids rank*S ..), built by the shared builder ----
     sample_base = rank * w.S
-    g = levy.build(w.L, w.rho, w.z, w.seed, S=w.S, sample_base=sample_base)
+    reduce_colours = workloads.REDUCE_COLOURS if args.colouring == "reduced" else 0
+    g = levy.build(w.L, w.rho, w.z, w.seed, S=w.S, sample_base=sample_base, reduce_colours=reduce_colours)
     T = w.temperatures()
     seed = 0xB200_1211_3991
     ens = B.Ensemble(g.row_ptr, g.col_idx, g.colour, T, seed, sample_base=sample_base, device=f"cuda:{local_rank}")
@@ -375,7 +379,7 @@ def main():
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         per_step = (1 + orps) * w.N * oracle_replicas(w) / 2.4e6          # seconds, at the oracle's ~2.4e6 updates/s
         n_cpu = int(min(args.steps, max(2, 12.0 / per_step)))
-        v, dt, what = oracle_sample_run(w, n_cpu, 1)
+        v, dt, what = oracle_sample_run(w, n_cpu, 1, reduce_colours=reduce_colours)
         model, cores = host_cpu()
         cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt, "steps": n_cpu, "sample": what,
                "host_cpu": model, "host_cores": cores}
@@ -385,7 +389,8 @@ def main():
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic",
-                "config": workload_config(w, world, me, info["q_max"], info["max_degree"]),
+                "config": workload_config(w, world, me, info["q_max"], info["max_degree"], args.colouring,
+                                          np.bincount(g.colour[0]).tolist()),
                 "roofline": roofline, "roofline_streaming": streaming, "interleaved": interleaved, "cpu_baseline": cpu, "e2e": e2e,
                 "gpu_launches": int(launches), "clocks": clocks}
         print(json.dumps(line), flush=True)
@@ -439,7 +444,7 @@ def main():
     if rank == 0 and world == 1 and not args.no_aux and not args.no_lscan:
         for L in (32, 64, 128, 256):
             wl = workloads.lscan(L)
-            gl = levy.build(wl.L, wl.rho, wl.z, wl.seed, S=wl.S)
+            gl = levy.build(wl.L, wl.rho, wl.z, wl.seed, S=wl.S, reduce_colours=reduce_colours)
             el = B.Ensemble(gl.row_ptr, gl.col_idx, gl.colour, wl.temperatures(), seed)
             el.run(5, sps, orps, me)
             n = max(10, int(2000 * 64 * 64 / (L * L)))

@@ -59,9 +59,31 @@ int xy_levy_build_fbc(int L, double rho, int z, uint64_t seed, uint32_t sample_b
                   int n_threads, int32_t *row_ptr, int32_t *col_idx, int32_t *colour,
                   int32_t *new_to_old, int32_t *n_colours, int64_t *n_draws);
 
+/* xy_levy_build / xy_levy_build_fbc with one more step between the colouring and the renumbering: if
+ * reduce_moves_per_site > 0 the smallest-last colouring is passed through xy_colour_reduce (max_moves =
+ * reduce_moves_per_site * N, key = seed, sample = the global sample id) until it stops losing colours.  On the z = 6
+ * Levy graphs this keeps Q = 5 (they contain 5-cliques) but shrinks the fifth class from ~1.4 % of the sites to a few
+ * dozen, and evens out the other four.  The bonds are the same as without the step; only the colours -- and with them
+ * the site numbering -- differ.  free_boundaries != 0 selects the free-boundary construction. */
+int xy_levy_build_opt(int free_boundaries, int reduce_moves_per_site, int L, double rho, int z, uint64_t seed,
+                      uint32_t sample_base, int S, int n_threads, int32_t *row_ptr, int32_t *col_idx, int32_t *colour,
+                      int32_t *new_to_old, int32_t *n_colours, int64_t *n_draws);
+
 /* Smallest-last greedy colouring of any symmetric CSR graph; returns Q (>= 0) or a negative error. */
 int xy_colour_smallest_last(int N, const int32_t *row_ptr, const int32_t *col_idx,
                             int32_t *colour /*[N]*/);
+
+/* Fewer colours, or a smaller last colour class, by local search (any proper colouring is a correct
+ * result; PAPER.md:456 reports Q, :494 time ~ Q/2).  colour[] (in/out) must be a proper colouring with colours 0..Q-1.
+ * While Q > target_q: the sites of the last class are given the least conflicting of the other colours and a tabu /
+ * min-conflicts search (conflicting site chosen by Philox4x32-10 counter (move_lo, move_hi, sample, 5), key = seed; it
+ * takes its least conflicting non-tabu colour) repairs the monochromatic bonds.  If max_moves moves do not repair all of
+ * them (a graph with a Q-clique cannot lose its Q-th colour), conflicting sites without a free colour may go back to
+ * the last colour (never two neighbours): same Q, but a last class of a few sites instead of ~1.4 % of them.
+ * Deterministic.  Returns the final number of colours (>= target_q) or a negative error.  The result
+ * is always proper (tests/test_builder.py checks it with the oracle's checker). */
+int xy_colour_reduce(int N, const int32_t *row_ptr, const int32_t *col_idx, int32_t *colour /*[N] in/out*/, int target_q,
+                     uint64_t seed, uint32_t sample, int64_t max_moves);
 
 /* Colour-major renumbering of any coloured CSR graph (same outputs as the per-sample arrays above). */
 int xy_renumber_colour_major(int N, const int32_t *row_ptr, const int32_t *col_idx,

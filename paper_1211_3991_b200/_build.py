@@ -62,6 +62,8 @@ def build_xy(force=False, verbose=False, extra_flags=()):
     from concurrent.futures import ThreadPoolExecutor
     srcs = _sources([(CSRC, (".cu",))])
     hdrs = _sources([(CSRC, (".cuh", ".h")), (INCLUDE, (".h",))])
+    if not force and not _stale(XY_LIB, srcs + hdrs):
+        return XY_LIB
     objdir = os.path.join(PKG, "build")
     os.makedirs(objdir, exist_ok=True)
     nvcc = nvcc_path()

@@ -127,6 +127,132 @@ int colour_sl(int N, const int32_t *row_ptr, const int32_t *col_idx, int32_t *co
     return Q;
 }
 
+// Shrink (ideally: empty) the LAST colour class of a proper colouring with Q colours.  Smallest-last leaves ~1.4 % of
+// the sites in a fifth class at z = 6: a fifth sequential phase per sweep for almost no work (PAPER.md:456 Q, :494
+// time ~ Q/2).  The Levy graphs of the configs with rho >= 3 contain a few 5-cliques, so the fifth colour cannot go
+// away there -- but it is needed by a handful of sites, not by thousands.
+// Tabu / min-conflicts search: the sites of the last class (colour T = Q-1) take the least conflicting of the other
+// colours; then, while monochromatic bonds remain, a conflicting site (picked by the Philox stream of domain 5) moves
+// to its least conflicting colour < T that is not tabu (aspiration: a conflict-free colour is always allowed) and may
+// not move back for a few steps.  After max_moves such moves, at a moment when the search is near the fewest bad bonds
+// it has seen, the escape opens: a conflicting site without a conflict-free colour returns to colour T if none of its
+// neighbours holds it (late in the search such neighbours are pushed back below T first).  When no bad bond is left, sites of colour T that have a free colour leave it
+// again.  Returns T if the last class is empty (the graph is T-coloured), else Q with a proper Q-colouring whose last
+// class is small; if that is not smaller than the input's, or bad bonds remain after 4 max_moves moves, colour[] is
+// left untouched.  Deterministic in (graph, seed, sample).
+int colour_reduce_once(int N, const int32_t *row_ptr, const int32_t *col_idx, int32_t *colour, int Q, uint64_t seed,
+                       uint32_t sample, int64_t max_moves) {
+    if (Q < 3) return Q;
+    const int T = Q - 1;
+    std::vector<int32_t> col(colour, colour + N);
+    std::vector<int32_t> cnt(static_cast<size_t>(N) * Q, 0);      // cnt[v*Q + c] = neighbours of v with colour c
+    auto at = [&](int v, int c) -> int32_t & { return cnt[static_cast<size_t>(v) * Q + c]; };
+    auto bump = [&](int v, int c, int d) {
+        for (int e = row_ptr[v]; e < row_ptr[v + 1]; ++e) at(col_idx[e], c) += d;
+    };
+    int64_t last_class = 0;
+    for (int v = 0; v < N; ++v) {
+        if (col[v] < T) bump(v, col[v], +1);
+        else ++last_class;
+    }
+    for (int v = 0; v < N; ++v) {
+        if (col[v] < T) continue;
+        int best = 0;
+        for (int c = 1; c < T; ++c)
+            if (at(v, c) < at(v, best)) best = c;
+        col[v] = best;
+        bump(v, best, +1);
+    }
+    std::vector<int32_t> conf, where(N, -1);                       // the conflicting sites, and their position in conf
+    auto refresh = [&](int v) {
+        const bool bad = at(v, col[v]) > 0;
+        if (bad && where[v] < 0) { where[v] = static_cast<int32_t>(conf.size()); conf.push_back(v); }
+        else if (!bad && where[v] >= 0) {
+            const int32_t last = conf.back();
+            conf[where[v]] = last; where[last] = where[v];
+            conf.pop_back(); where[v] = -1;
+        }
+    };
+    auto move = [&](int v, int c) {
+        bump(v, col[v], -1);
+        col[v] = c;
+        bump(v, c, +1);
+        refresh(v);
+        for (int e = row_ptr[v]; e < row_ptr[v + 1]; ++e) refresh(col_idx[e]);
+    };
+    for (int v = 0; v < N; ++v) refresh(v);
+    std::vector<int64_t> tabu(static_cast<size_t>(N) * T, -1);     // move (v -> c) forbidden while it <= tabu
+    const uint32_t k0 = static_cast<uint32_t>(seed), k1 = static_cast<uint32_t>(seed >> 32);
+    size_t fewest = conf.size();                                   // fewest conflicting sites seen so far
+    bool escape = false;
+    for (int64_t it = 0; !conf.empty(); ++it) {
+        if (it >= 4 * max_moves) return Q;
+        fewest = std::min(fewest, conf.size());
+        // the escape opens after max_moves moves, at a moment when the search is (again) near its best state
+        if (!escape && (it >= 2 * max_moves || (it >= max_moves && conf.size() <= fewest + fewest / 8 + 1))) escape = true;
+        uint32_t x[4];
+        philox(static_cast<uint32_t>(it), static_cast<uint32_t>(static_cast<uint64_t>(it) >> 32), sample, 5u, k0, k1, x);
+        const int v = conf[(static_cast<uint64_t>(x[0]) * conf.size()) >> 32];
+        const int old = col[v];
+        int best = -1, n_best = 0;
+        for (int c = 0; c < T; ++c) {
+            if (c == old) continue;
+            const int32_t k = at(v, c);
+            if (tabu[static_cast<size_t>(v) * T + c] >= it && k > 0) continue;
+            if (best < 0 || k < at(v, best)) { best = c; n_best = 1; }
+            else if (k == at(v, best) && ((x[1] >> (n_best++ & 15)) & 1u)) best = c;
+        }
+        if (escape && (best < 0 || at(v, best) > 0) && (at(v, T) == 0 || it >= 3 * max_moves)) {
+            // no conflict-free colour: v takes the last colour; late in the search, neighbours that hold it are pushed
+            // back to their least conflicting colour below T first (they may become conflicting sites themselves)
+            for (int e = row_ptr[v]; e < row_ptr[v + 1] && at(v, T) > 0; ++e) {
+                const int u = col_idx[e];
+                if (col[u] != T) continue;
+                int bu = 0;
+                for (int c = 1; c < T; ++c)
+                    if (at(u, c) < at(u, bu)) bu = c;
+                move(u, bu);
+            }
+            move(v, T);
+            continue;
+        }
+        if (best < 0) continue;                                    // every other colour is tabu: draw again
+        tabu[static_cast<size_t>(v) * T + old] = it + 8 + (x[2] & 7u);
+        move(v, best);
+    }
+    int64_t left = 0;
+    for (int v = 0; v < N; ++v) {
+        if (col[v] < T) continue;
+        int c = 0;
+        while (c < T && at(v, c) > 0) ++c;
+        if (c < T) move(v, c);
+        else ++left;
+    }
+    if (left >= last_class) return Q;                              // no gain: keep the input
+    std::copy(col.begin(), col.end(), colour);
+    return left == 0 ? T : Q;
+}
+
+// colour_reduce_once until the number of colours reaches target_q or the last class stops shrinking (at most 8 rounds;
+// round r uses the Philox stream of sample + r * 2^16 so that a repeated search does not retrace the previous one)
+int colour_reduce(int N, const int32_t *row_ptr, const int32_t *col_idx, int32_t *colour, int Q, int target_q, uint64_t seed,
+                  uint32_t sample, int64_t max_moves) {
+    auto last_size = [&](int q) {
+        int64_t n = 0;
+        for (int v = 0; v < N; ++v) n += colour[v] == q - 1;
+        return n;
+    };
+    int64_t size = last_size(Q);
+    for (uint32_t round = 0; round < 8 && Q > target_q; ++round) {
+        const int q2 = colour_reduce_once(N, row_ptr, col_idx, colour, Q, seed, sample + (round << 16), max_moves);
+        const int64_t size2 = last_size(q2);
+        if (q2 == Q && size2 >= size) break;
+        Q = q2;
+        size = size2;
+    }
+    return Q;
+}
+
 void renumber(int N, const int32_t *row_ptr, const int32_t *col_idx, const int32_t *colour,
               int32_t *new_to_old, int32_t *row_ptr_new, int32_t *col_idx_new, int32_t *colour_new) {
     std::vector<int32_t> n2o(N), o2n(N);
@@ -184,7 +310,7 @@ Cdf make_cdf(int L, double rho) {
     return c;
 }
 
-int build_one(int L, int z, uint64_t seed, uint32_t sample, const Cdf &cdf, int32_t *row_ptr,
+int build_one(int L, int z, uint64_t seed, uint32_t sample, const Cdf &cdf, int reduce_moves_per_site, int32_t *row_ptr,
               int32_t *col_idx, int32_t *colour, int32_t *new_to_old, int32_t *n_colours,
               int64_t *n_draws, std::string &err) {
     const int N = L * L;
@@ -225,7 +351,10 @@ int build_one(int L, int z, uint64_t seed, uint32_t sample, const Cdf &cdf, int3
     }
     std::vector<int32_t> rp, ci, col(N);
     csr_from_bonds(N, bonds, rp, ci);
-    const int Q = colour_sl(N, rp.data(), ci.data(), col.data());
+    int Q = colour_sl(N, rp.data(), ci.data(), col.data());
+    // optional: fewer colours / a smaller last class by local search (colour_reduce_once), down to 3 colours at most
+    if (reduce_moves_per_site > 0) Q = colour_reduce(N, rp.data(), ci.data(), col.data(), Q, 3, seed, sample,
+                                                     static_cast<int64_t>(reduce_moves_per_site) * N);
     renumber(N, rp.data(), ci.data(), col.data(), new_to_old, row_ptr, col_idx, colour);
     if (n_colours) *n_colours = Q;
     if (n_draws) *n_draws = k;
@@ -246,8 +375,8 @@ extern "C" {
 
 const char *xy_levy_last_error(void) { return g_err.c_str(); }
 
-static int levy_build_impl(bool fbc, int L, double rho, int z, uint64_t seed, uint32_t sample_base, int S, int n_threads,
-                           int32_t *row_ptr, int32_t *col_idx, int32_t *colour, int32_t *new_to_old,
+static int levy_build_impl(bool fbc, int reduce_moves_per_site, int L, double rho, int z, uint64_t seed, uint32_t sample_base,
+                           int S, int n_threads, int32_t *row_ptr, int32_t *col_idx, int32_t *colour, int32_t *new_to_old,
                            int32_t *n_colours, int64_t *n_draws) {
     try {
         if (L < 2 || L > 16384 || z < 1 || S < 0 || !(rho >= 0.0) || !std::isfinite(rho))
@@ -268,7 +397,7 @@ static int levy_build_impl(bool fbc, int L, double rho, int z, uint64_t seed, ui
         auto work = [&](int tid) {
             try {
                 for (int s = next.fetch_add(1); s < S; s = next.fetch_add(1)) {
-                    const int rc = build_one(L, z, seed, sample_base + static_cast<uint32_t>(s), cdf,
+                    const int rc = build_one(L, z, seed, sample_base + static_cast<uint32_t>(s), cdf, reduce_moves_per_site,
                                              row_ptr + static_cast<size_t>(s) * (N + 1),
                                              col_idx + static_cast<size_t>(s) * N * z,
                                              colour + static_cast<size_t>(s) * N,
@@ -302,21 +431,48 @@ static int levy_build_impl(bool fbc, int L, double rho, int z, uint64_t seed, ui
 int xy_levy_build(int L, double rho, int z, uint64_t seed, uint32_t sample_base, int S, int n_threads,
                   int32_t *row_ptr, int32_t *col_idx, int32_t *colour, int32_t *new_to_old,
                   int32_t *n_colours, int64_t *n_draws) {
-    return levy_build_impl(false, L, rho, z, seed, sample_base, S, n_threads, row_ptr, col_idx, colour, new_to_old,
+    return levy_build_impl(false, 0, L, rho, z, seed, sample_base, S, n_threads, row_ptr, col_idx, colour, new_to_old,
                            n_colours, n_draws);
 }
 
 int xy_levy_build_fbc(int L, double rho, int z, uint64_t seed, uint32_t sample_base, int S, int n_threads,
                       int32_t *row_ptr, int32_t *col_idx, int32_t *colour, int32_t *new_to_old,
                       int32_t *n_colours, int64_t *n_draws) {
-    return levy_build_impl(true, L, rho, z, seed, sample_base, S, n_threads, row_ptr, col_idx, colour, new_to_old,
+    return levy_build_impl(true, 0, L, rho, z, seed, sample_base, S, n_threads, row_ptr, col_idx, colour, new_to_old,
                            n_colours, n_draws);
+}
+
+int xy_levy_build_opt(int free_boundaries, int reduce_moves_per_site, int L, double rho, int z, uint64_t seed,
+                      uint32_t sample_base, int S, int n_threads, int32_t *row_ptr, int32_t *col_idx, int32_t *colour,
+                      int32_t *new_to_old, int32_t *n_colours, int64_t *n_draws) {
+    if (reduce_moves_per_site < 0) return fail(XY_LEVY_EINVAL, "reduce_moves_per_site < 0");
+    return levy_build_impl(free_boundaries != 0, reduce_moves_per_site, L, rho, z, seed, sample_base, S, n_threads, row_ptr,
+                           col_idx, colour, new_to_old, n_colours, n_draws);
 }
 
 int xy_colour_smallest_last(int N, const int32_t *row_ptr, const int32_t *col_idx, int32_t *colour) {
     try {
         if (!csr_ok(N, row_ptr, col_idx) || (N > 0 && !colour)) return fail(XY_LEVY_EINVAL, "malformed CSR");
         return colour_sl(N, row_ptr, col_idx, colour);
+    } catch (const std::bad_alloc &) {
+        return fail(XY_LEVY_ENOMEM, "out of memory");
+    }
+}
+
+int xy_colour_reduce(int N, const int32_t *row_ptr, const int32_t *col_idx, int32_t *colour, int target_q, uint64_t seed,
+                     uint32_t sample, int64_t max_moves) {
+    try {
+        if (!csr_ok(N, row_ptr, col_idx) || (N > 0 && !colour) || target_q < 2 || max_moves < 0)
+            return fail(XY_LEVY_EINVAL, "malformed CSR, null colour array, target_q < 2 or max_moves < 0");
+        int Q = 0;
+        for (int v = 0; v < N; ++v) {
+            if (colour[v] < 0) return fail(XY_LEVY_EINVAL, "negative colour");
+            Q = std::max(Q, colour[v] + 1);
+        }
+        for (int v = 0; v < N; ++v)
+            for (int e = row_ptr[v]; e < row_ptr[v + 1]; ++e)
+                if (colour[col_idx[e]] == colour[v]) return fail(XY_LEVY_EINVAL, "the input colouring is not proper");
+        return colour_reduce(N, row_ptr, col_idx, colour, Q, target_q, seed, sample, max_moves);
     } catch (const std::bad_alloc &) {
         return fail(XY_LEVY_ENOMEM, "out of memory");
     }

@@ -173,6 +173,7 @@ struct xy_pt {
     int path = 0;                    // xy_set_path: 0 = automatic, 1 = one launch per colour class (k_phase), 2 = one cluster per sample (k_cycle)
     const void *cycle_fn[2] = {nullptr, nullptr};   // k_cycle<G, ORDER, xy::kCycleWarps>, by order
     int cluster_max = 0;             // largest cluster size the device schedules for k_cycle (0 = not available)
+    int cluster_active[9] = {};      // co-resident clusters of k_cycle by cluster size (1, 2, 4, 8)
     int fuse_measure = 1;            // measured sweeps: the last over-relaxation sweep also produces E, Mx, My (MODE 3)
     std::map<int, int4 *> parts;     // warps per sample -> device [S][q_stride][nw] share tables {i0, w1, start0, n_run}
     int sweep_capacity = 0;          // co-resident CTAs of k_phase on this device: the grid is one such wave
@@ -523,11 +524,13 @@ int issue_sweeps(xy_pt *pt, int sps, int orps, int group) {
 }
 
 // ---- the cluster path (k_cycle): one thread-block cluster per sample runs whole cycles in one launch ----
-// CTAs per sample: as many as spread the samples over the SMs, a power of two <= the device's cluster limit
+// CTAs per sample: the largest power of two <= the device's cluster limit for which ALL samples' clusters are resident
+// at once (cudaOccupancyMaxActiveClusters: cluster placement is per GPC, so fewer than n_sm / C clusters may fit);
+// 1 when the samples outnumber the SMs
 int cycle_cluster_size(const xy_pt *pt) {
-    int c = 1;
-    while (c * 2 <= pt->cluster_max && static_cast<long long>(c) * 2 * pt->g->S <= pt->g->n_sm) c *= 2;
-    return c;
+    for (int c = pt->cluster_max; c > 1; c /= 2)
+        if (pt->cluster_active[c] >= pt->g->S) return c;
+    return 1;
 }
 
 // the cluster path serves one column block (R = 2G <= 64) with at least one over-relaxation sweep per Metropolis sweep
@@ -535,13 +538,17 @@ bool cycle_eligible(const xy_pt *pt, int orps) {
     return pt->fast_G && pt->col_blocks == 1 && pt->cluster_max >= 1 && orps >= 1 && pt->fuse_measure;
 }
 
-// automatic choice: the cluster path when a colour-class launch would be launch-latency bound, i.e. when the rows of ALL
-// samples together give a resident warp less than a handful of rows per class (measured crossover: DESIGN.md 7.2)
+// automatic choice (measured, DESIGN.md 7.2 / 7.6): a colour-class phase of the cluster path costs what a PDL-chained
+// launch costs -- both are bound by the serial chain of one phase (stage the share, gather, ~1000 dependent instructions
+// per warp, store, release), not by the launch -- so the cluster path only wins where the launch path cannot overlap
+// anything: samples so small that a class is at most one row per warp of the cluster.
 bool use_cycle_path(const xy_pt *pt, int orps) {
     if (pt->path == 1 || !cycle_eligible(pt, orps)) return false;
     if (pt->path == 2) return true;
-    const long long rows = static_cast<long long>(ceil_div(pt->g->N, 32 / pt->fast_G)) * pt->g->S;
-    return rows < 16ll * xy::kWarpsBig * pt->capacity_big;
+    const xy_graph *g = pt->g;
+    const int C = cycle_cluster_size(pt);
+    const double rows_per_warp = static_cast<double>(ceil_div(max_class_size(g, 0, 0, g->S), 32 / pt->fast_G)) / (C * xy::kCycleWarps);
+    return rows_per_warp <= 1.0;
 }
 
 int launch_cycle(xy_pt *pt, int n_cycles, int sps, int orps, int me, bool do_swap) {
@@ -954,7 +961,20 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
                 qc.dynamicSmemBytes = xy::sweep_smem(xy::kCycleWarps);
                 ec = cudaOccupancyMaxPotentialClusterSize(&max_cluster, pt->cycle_fn[0], &qc);
             }
-            pt->cluster_max = ec == cudaSuccess ? std::min(8, std::max(0, max_cluster)) : 0;
+            pt->cluster_max = 0;
+            for (int c = 1; c <= 8 && ec == cudaSuccess && c <= max_cluster; c *= 2) {
+                cudaLaunchConfig_t qc = {};
+                cudaLaunchAttribute qa;
+                qa.id = cudaLaunchAttributeClusterDimension;
+                qa.val.clusterDim.x = c; qa.val.clusterDim.y = 1; qa.val.clusterDim.z = 1;
+                qc.gridDim = dim3(c, 1, 1); qc.blockDim = dim3(xy::kCycleWarps * 32);
+                qc.dynamicSmemBytes = xy::sweep_smem(xy::kCycleWarps);
+                qc.attrs = &qa; qc.numAttrs = 1;
+                int n_active = 0;
+                if (cudaOccupancyMaxActiveClusters(&n_active, pt->cycle_fn[0], &qc) != cudaSuccess || n_active < 1) break;
+                pt->cluster_active[c] = n_active;
+                pt->cluster_max = c;
+            }
             cudaGetLastError();
         }
         // persisting L2 carve-out for the access-policy windows of the sample groups; xy_pt_destroy puts the limit back

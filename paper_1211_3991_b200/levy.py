@@ -23,8 +23,12 @@ def lib():
         L.xy_levy_build.restype = C.c_int
         L.xy_levy_build_fbc.argtypes = L.xy_levy_build.argtypes
         L.xy_levy_build_fbc.restype = C.c_int
+        L.xy_levy_build_opt.argtypes = [C.c_int, C.c_int] + L.xy_levy_build.argtypes
+        L.xy_levy_build_opt.restype = C.c_int
         L.xy_colour_smallest_last.argtypes = [C.c_int, _i32p, _i32p, _i32p]
         L.xy_colour_smallest_last.restype = C.c_int
+        L.xy_colour_reduce.argtypes = [C.c_int, _i32p, _i32p, _i32p, C.c_int, C.c_uint64, C.c_uint32, C.c_int64]
+        L.xy_colour_reduce.restype = C.c_int
         L.xy_renumber_colour_major.argtypes = [C.c_int, _i32p, _i32p, _i32p, _i32p, _i32p, _i32p, _i32p]
         L.xy_renumber_colour_major.restype = C.c_int
         L.xy_levy_last_error.restype = C.c_char_p
@@ -64,7 +68,9 @@ class LevyGraphs:
         return np.searchsorted(self.colour[s], np.arange(Q + 1)).astype(np.int32)
 
 
-def build(L, rho, z, seed, S=1, sample_base=0, n_threads=0, boundary="periodic"):
+def build(L, rho, z, seed, S=1, sample_base=0, n_threads=0, boundary="periodic", reduce_colours=0):
+    """reduce_colours = moves per site of the colour-reducing local search after the smallest-last colouring
+    (xy_levy_build_opt; 0 = the plain smallest-last colouring that the oracle restates bit for bit)."""
     N = L * L
     row_ptr = np.zeros((S, N + 1), np.int32)
     col_idx = np.zeros((S, N * z), np.int32)
@@ -72,12 +78,15 @@ def build(L, rho, z, seed, S=1, sample_base=0, n_threads=0, boundary="periodic")
     n2o = np.zeros((S, N), np.int32)
     nq = np.zeros(S, np.int32)
     nd = np.zeros(S, np.int64)
-    fn = lib().xy_levy_build if boundary == "periodic" else lib().xy_levy_build_fbc
     if boundary not in ("periodic", "free"):
         raise ValueError("boundary must be 'periodic' or 'free'")
-    rc = fn(L, float(rho), z, seed, sample_base, S, n_threads, row_ptr.reshape(-1),
-                             col_idx.reshape(-1), colour.reshape(-1), n2o.ctypes.data, nq.ctypes.data,
-                             nd.ctypes.data)
+    out = (row_ptr.reshape(-1), col_idx.reshape(-1), colour.reshape(-1), n2o.ctypes.data, nq.ctypes.data, nd.ctypes.data)
+    if reduce_colours:
+        rc = lib().xy_levy_build_opt(int(boundary == "free"), int(reduce_colours), L, float(rho), z, seed, sample_base, S,
+                                     n_threads, *out)
+    else:
+        fn = lib().xy_levy_build if boundary == "periodic" else lib().xy_levy_build_fbc
+        rc = fn(L, float(rho), z, seed, sample_base, S, n_threads, *out)
     if rc != 0:
         raise LevyError(f"xy_levy_build: {rc}: {lib().xy_levy_last_error().decode()}")
     return LevyGraphs(L, float(rho), z, seed, sample_base, row_ptr, col_idx, colour, n2o, nq, nd)
@@ -92,6 +101,19 @@ def colour_smallest_last(row_ptr, col_idx):
     if Q < 0:
         raise LevyError(lib().xy_levy_last_error().decode())
     return colour[:N], Q
+
+
+def colour_reduce(row_ptr, col_idx, colour, target_q, seed, sample=0, max_moves=None):
+    """local search for a proper colouring with fewer colours; returns (colour, Q)"""
+    row_ptr = np.ascontiguousarray(row_ptr, np.int32)
+    col_idx = np.ascontiguousarray(col_idx, np.int32)
+    colour = np.array(colour, np.int32, copy=True)
+    N = len(row_ptr) - 1
+    Q = lib().xy_colour_reduce(N, row_ptr, col_idx if col_idx.size else np.zeros(1, np.int32), colour, target_q, seed, sample,
+                               64 * N if max_moves is None else max_moves)
+    if Q < 0:
+        raise LevyError(lib().xy_levy_last_error().decode())
+    return colour, Q
 
 
 def renumber_colour_major(row_ptr, col_idx, colour):

@@ -6,12 +6,13 @@ import numpy as np
 import oracle as O
 
 
-def run_with_margins(rp, ci, cp, T, seed, n_cycles, sps, orps, me, order=0, sample=0, mutate=None):
+def run_with_margins(rp, ci, cp, T, seed, n_cycles, sps, orps, me, order=0, sample=0, mutate=None, theta0=None):
     """Returns a list (one entry per cycle) of dict(theta, temp_of_slot, acc, min_margin, min_swap_margin): the state after
     the cycle and the smallest Metropolis / swap decision margin seen SO FAR.  mutate = "or_first_last_colour" runs a
-    deliberately wrong order (over-relaxation before Metropolis on the last colour) for the tests' own sensitivity check."""
+    deliberately wrong order (over-relaxation before Metropolis on the last colour) for the tests' own sensitivity check.
+    theta0 [N][R]: the initial angles (default: the library's Philox initialisation)."""
     N, R, Q = len(rp) - 1, len(T), len(cp) - 1
-    th = O.init_theta(N, R, seed, sample)
+    th = O.init_theta(N, R, seed, sample) if theta0 is None else np.array(theta0, np.float32, copy=True)
     tos = np.arange(R, dtype=np.int32)
     sot = np.arange(R, dtype=np.int32)
     acc = np.zeros((R, O.NACC))

@@ -145,3 +145,47 @@ def test_free_boundary_structure():
     assert abs(n3 / n4 - expect) < 0.25 * expect, (n3, n4, expect)
     with pytest.raises(ValueError):
         levy.build(8, 3.0, 6, SEED, boundary="helical")
+
+
+def _bond_set(g, s):
+    n2o, rp, ci = g.new_to_old[s], g.row_ptr[s], g.col_idx[s]
+    src = np.repeat(np.arange(g.N), np.diff(rp))
+    return np.sort(n2o[src].astype(np.int64) * g.N + n2o[ci])
+
+
+@pytest.mark.parametrize("L,rho", [(24, 2.5), (32, 3.5), (48, 4.5)])
+def test_colour_reduction_keeps_the_bonds_stays_proper_and_shrinks_the_last_class(L, rho):
+    """xy_levy_build_opt(reduce_moves_per_site): the optional local search after the smallest-last colouring (SURVEY C4:
+    any proper colouring is a correct result; the number of colours sets the number of sequential
+    phases).  Checked with the ORACLE's properness test; the bonds are those of the plain build; the colouring is
+    deterministic; the last class shrinks (or the colour disappears); numbering is colour-major."""
+    z, S = 6, 3
+    plain = levy.build(L, rho, z, SEED, S=S, sample_base=2)
+    red = levy.build(L, rho, z, SEED, S=S, sample_base=2, reduce_colours=8)
+    again = levy.build(L, rho, z, SEED, S=S, sample_base=2, reduce_colours=8, n_threads=1)
+    assert np.array_equal(red.colour, again.colour) and np.array_equal(red.col_idx, again.col_idx)
+    for s in range(S):
+        assert np.array_equal(_bond_set(plain, s), _bond_set(red, s))
+        assert O.colouring_is_proper(red.row_ptr[s], red.col_idx[s], red.colour[s])
+        assert np.all(np.diff(red.colour[s]) >= 0)
+        q0, q1 = int(plain.n_colours[s]), int(red.n_colours[s])
+        assert q1 <= q0 and red.colour[s].max() + 1 == q1
+        if q1 == q0:
+            assert (red.colour[s] == q1 - 1).sum() <= (plain.colour[s] == q0 - 1).sum()
+    assert sum((red.colour[s] == red.n_colours[s] - 1).sum() if red.n_colours[s] == plain.n_colours[s] else 0 for s in range(S)) \
+        < 0.7 * sum((plain.colour[s] == plain.n_colours[s] - 1).sum() for s in range(S))
+
+
+def test_colour_reduce_on_hand_made_graphs():
+    """a 5-clique keeps its fifth colour (one site); an odd cycle coloured with 4 colours drops to 3; bad input is refused"""
+    k5 = [(a, b) for a in range(5) for b in range(a + 1, 5)]
+    tail = [(4, 5), (5, 6), (6, 7)]
+    rp, ci = G.csr_from_edges(8, k5 + tail)
+    col = np.array([0, 1, 2, 3, 4, 0, 4, 0], np.int32)                  # proper, wasteful: two sites in the last class
+    out, Q = levy.colour_reduce(rp, ci, col, 3, SEED)
+    assert Q == 5 and O.colouring_is_proper(rp, ci, out) and (out == 4).sum() == 1
+    rp, ci = G.csr_from_edges(7, G.ring_edges(7))
+    out, Q = levy.colour_reduce(rp, ci, np.array([0, 1, 2, 3, 0, 1, 2], np.int32), 2, SEED)
+    assert Q == 3 and O.colouring_is_proper(rp, ci, out)
+    with pytest.raises(levy.LevyError):
+        levy.colour_reduce(rp, ci, np.zeros(7, np.int32), 2, SEED)        # not proper

@@ -2,8 +2,8 @@
 classes separated by the hardware cluster barrier) must give the
 SAME BITS as the per-launch path (k_phase): same Philox keying, same arithmetic, exact integer reductions.  The per-launch
 path is the one held against the oracle element by element (tests/test_gpu_parity.py), so bit-identity carries that
-parity over; the equilibrium tests (ring closed form, quadrature, config 0/1 vs oracle) run through the cluster path
-directly because the automatic choice takes it for small samples."""
+parity over; the exact-physics equilibrium tests (ring closed form, quadrature on 3- and 4-site graphs, config 0 vs
+oracle) run through the cluster path directly because the automatic choice takes it for tiny samples."""
 import numpy as np
 import pytest
 
@@ -40,7 +40,7 @@ def test_cluster_path_is_bit_identical_to_the_launch_path(L, rho, R, S, order):
         same_state(a, b, (n, sps, orps, me))
     a.run_sweeps(3, 5, 1); b.run_sweeps(3, 5, 1)
     same_state(a, b, "run_sweeps")
-    assert a.read_accumulators()[..., 0].min() > 0 and a.get_counters()[3].sum() > 0          # measured, swaps accepted
+    assert a.read_accumulators()[..., 0].min() > 0 and (R < 8 or a.get_counters()[3].sum() > 0)          # measured, swaps accepted
     # mixing the paths inside one run, and checkpoint/resume across them
     a.run(2, 10, 1, 1)
     b.set_path(1); b.run(1, 10, 1, 1); b.set_path(2); b.run(1, 10, 1, 1)
@@ -72,7 +72,7 @@ def test_cluster_path_degenerate_graphs_and_unequal_colour_counts():
 def test_cluster_path_selection_and_errors():
     g = levy.build(16, 3.5, 6, workloads.BASE_SEED, S=2)
     small = U.ensemble_from_levy(g, O.geometric_temperatures(16, 1.0, 4.0), SEED)
-    assert small.get_path()[0] == 2                          # automatic: small samples take the cluster path
+    assert small.get_path()[0] == 2                          # automatic: tiny samples take the cluster path
     assert small.get_path(or_per_sweep=0)[0] == 1            # no over-relaxation sweep to fuse the measurement into
     small.run(1, 10, 0, 1)                                   # ... and xy_run falls back by itself
     small.set_path(2)
@@ -92,12 +92,12 @@ def test_cluster_path_selection_and_errors():
 
 @pytest.mark.parametrize("cfg", [0, 1])
 def test_cluster_path_full_size_configs_bit_identical_and_energy_vs_oracle(cfg):
-    """BASELINE configs 0 and 1 at full size (the configs the automatic choice sends down the cluster path)"""
+    """BASELINE configs 0 and 1 at full size (the small configs) through the cluster path"""
     w = workloads.CONFIGS[cfg]
     g = levy.build(w.L, w.rho, w.z, w.seed, S=w.S)
     T = w.temperatures()
     a = U.ensemble_from_levy(g, T, SEED); a.set_path(1)
-    b = U.ensemble_from_levy(g, T, SEED)
+    b = U.ensemble_from_levy(g, T, SEED); b.set_path(2)
     assert b.get_path()[0] == 2
     a.run(3, w.sweeps_per_swap, w.or_per_sweep, 1); b.run(3, w.sweeps_per_swap, w.or_per_sweep, 1)
     same_state(a, b, cfg)

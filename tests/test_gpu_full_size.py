@@ -81,14 +81,17 @@ def test_full_size_lockstep_sampled_sites_and_invariants(cfg):
     ens.close()
 
 
-@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
-def test_full_size_lockstep_every_site_of_one_sample_both_orders(cfg):
+@pytest.mark.parametrize("cfg,reduce_colours", [(1, 0), (2, 0), (3, 0), (4, 0), (4, workloads.REDUCE_COLOURS), (3, workloads.REDUCE_COLOURS)])
+def test_full_size_lockstep_every_site_of_one_sample_both_orders(cfg, reduce_colours):
     """EVERY site (all R replicas) of one whole sample of the full-size ensemble, in the bench's launch configuration:
     a Metropolis sweep and an over-relaxation sweep colour by colour (default order), then an interleaved sweep
     (Metropolis + over-relaxation of a class in one launch), each class compared with the oracle from the same
-    pre-state.  Share, chunk and column-block boundaries, the degree > 8 tail and isolated sites are all covered."""
+    pre-state.  Share, chunk and column-block boundaries, the degree > 8 tail and isolated sites are all covered.
+    reduce_colours > 0: the graphs as bench.py builds them (colour-reducing local search after smallest-last: a fifth
+    class of a few dozen sites)."""
     w = workloads.CONFIGS[cfg]
-    g = levy.build(w.L, w.rho, w.z, w.seed, S=w.S)
+    g = levy.build(w.L, w.rho, w.z, w.seed, S=w.S, reduce_colours=reduce_colours)
+    assert all(O.colouring_is_proper(g.row_ptr[k], g.col_idx[k], g.colour[k]) for k in range(min(w.S, 2)))
     T = w.temperatures()
     ens = U.ensemble_from_levy(g, T, SEED + 1)
     graphs = U.graphs_of_levy(g)

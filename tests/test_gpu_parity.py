@@ -199,27 +199,34 @@ def test_run_equals_stepwise_calls_and_schedule_invariance():
 def test_run_matches_oracle_protocol_full_cycles(order):
     """xy_run against the oracle's protocol over FULL PT cycles (10 sweeps x (Metropolis, over-relaxation, measure) + a
     swap round each): the order of the phases, the measurement cadence, the filing under temperatures and the swap
-    bookkeeping.  The chain is chaotic, so the comparison is exact only while no decision falls near its threshold:
-    tests/protocol.py replays the oracle's loop (bit-identical to orc_run_order, tests/test_oracle_equilibrium.py) and
-    reports the smallest decision margin so far; a seed is searched (deterministically) whose first cycles stay 1e-4
-    away from every threshold and that accepts a swap.  While that holds: labels bit-exact, accumulator counts exact,
-    angles within 1e-3 rad (a phase out of order moves angles by ~3 rad: checked on the oracle side, same file), energies
-    and m^2 sums within the fp32 drift.  Afterwards only the integer bookkeeping is compared."""
+    bookkeeping.  The chain is chaotic, so whole cycles can be compared only where it is not: in the ORDERED phase
+    (T = 0.2 .. 0.8, start near alignment) every local field has |h| >= 1, so the over-relaxation map does not amplify
+    the 1e-6 rad differences between the fast fp32 kernels and the fp64 oracle, and a decision can differ only if it falls
+    within ~1e-5 of its threshold.  tests/protocol.py replays the oracle's loop (bit-identical to orc_run_order,
+    tests/test_oracle_equilibrium.py) and reports the smallest decision margin so far; a seed is searched
+    (deterministically) whose first cycle(s) stay 2e-4 away from every threshold and permute the labels.  While that
+    holds: labels bit-exact, accumulator counts exact, angles within 1e-3 rad (measured drift: 3e-5 after one cycle, 3e-4
+    after three; one phase out of order moves angles by 0.8 rad: checked on the oracle side, same file), energy / magnetisation sums within fp32 round-off.  Afterwards only
+    the integer bookkeeping is compared."""
     import protocol as P
     L, R, sps = 8, 8, 10
     g = small_levy(L, 3.5, 1)
-    T = O.geometric_temperatures(R, 1.0, 4.0)
+    T = O.geometric_temperatures(R, 0.2, 0.8)
     rp, ci, cp = g.row_ptr[0], g.col_idx[0], g.class_ptr(0)
+    th0 = (1.0 + 0.05 * np.random.default_rng(5).standard_normal((L * L, R))).astype(np.float32)
     n_cycles = 4
-    for seed in range(2, 200):
-        h = P.run_with_margins(rp, ci, cp, T, seed, n_cycles, sps, 1, 1, order=order)
-        safe = [k for k in range(n_cycles) if min(h[k]["min_margin"], h[k]["min_swap_margin"]) > 1e-4]
+    for seed in range(2, 400):
+        h = P.run_with_margins(rp, ci, cp, T, seed, n_cycles, sps, 1, 1, order=order, theta0=th0)
+        safe = [k for k in range(n_cycles) if min(h[k]["min_margin"], h[k]["min_swap_margin"]) > 2e-4]
         if safe and any(not np.array_equal(h[k]["temp_of_slot"], np.arange(R)) for k in safe):
             break
     else:
         pytest.fail("no seed with a threshold-free first cycle")
+    bad = P.run_with_margins(rp, ci, cp, T, seed, 1, sps, 1, 1, order=0, theta0=th0, mutate="or_first_last_colour")
+    assert order == 1 or U.circ(bad[0]["theta"], h[0]["theta"]).max() > 0.1           # the bar below would notice
     ens = U.ensemble_from_levy(g, T, seed)
     ens.set_order(order)
+    ens.set_theta(th0[None])
     worst = 0.0
     for k in range(n_cycles):
         ens.run(1, sps, 1, 1)
@@ -232,10 +239,10 @@ def test_run_matches_oracle_protocol_full_cycles(order):
             err = U.circ(ens.get_theta()[0], h[k]["theta"]).max()
             worst = max(worst, err)
             assert err < 1e-3, f"cycle {k}: max |dtheta| {err}"
-            assert np.allclose(acc[:, 1], h[k]["acc"][:, 1], rtol=0, atol=2e-2)
-            assert np.allclose(acc[:, 4], h[k]["acc"][:, 4], rtol=0, atol=2e-4)
-            assert np.allclose(acc[:, 6:8], h[k]["acc"][:, 6:8], rtol=0, atol=2e-3)
-    print(f"\n[protocol order {order}] seed {seed}: {len(safe)} threshold-free cycles compared, max |dtheta| {worst:.2e}")
+            assert np.allclose(acc[:, 1], h[k]["acc"][:, 1], rtol=0, atol=5e-3)
+            assert np.allclose(acc[:, 3:6], h[k]["acc"][:, 3:6], rtol=0, atol=1e-4)
+            assert np.allclose(acc[:, 6:8], h[k]["acc"][:, 6:8], rtol=0, atol=1e-3)
+    print(f"\n[protocol order {order}] seed {seed}: {len(safe)} threshold-free cycle(s) compared, max |dtheta| {worst:.2e}")
     ens.close()
 
 

@@ -61,14 +61,18 @@ R_KT = paper_value("r_kt_log")                       # 1/16
 
 def test_square_lattice_kt_susceptibility_exponent_at_the_paper_tc():
     """The paper's own benchmark of its algorithm: on the 2D square lattice (the rho = infinity
-    limit, z = 4, two colours) the susceptibility at T_c = 0.8929 scales as chi ~ L^(2 - eta)
-    (ln L)^(-2r) with eta = 1/4, r = 1/16 (Eq. 27); eta(T) = the exponent "numerically interpolating Eq. (27) at
-    different temperatures" grows with T, passes 1/4 at T_c, and chi stops growing with L in the vortex phase.
-    chi = N <m^2> (item (3): <m>^2 is negligible).  L = 16, 32, 64; 16 independent copies of the lattice."""
+    limit, z = 4, two colours) the susceptibility at T_c = 0.8929 scales as chi ~ L^(2 - eta) with
+    eta = 1/4 (Eq. 27); eta(T), "numerically interpolating Eq. (27) at different temperatures", grows with T, passes 1/4
+    at T_c (the paper's independent estimate T_c = 0.894(5)), and chi stops growing with L in the vortex phase.
+    chi = N <m^2> (item (3): <m>^2 is negligible).  L = 32, 64, 128 (the largest is the lattice of the
+    paper's Table III); 16 independent copies of each lattice.  Coarse check (R22): the leading power law is
+    fitted; Eq. 27's factor (ln L)^(-2r), whose sign differs between the paper (r = 1/16) and the KT literature it cites
+    (r = -1/16) and which shifts eta by -+0.03 at these sizes, is reported beside it, not asserted."""
     T = np.sort(np.append(np.linspace(0.70, 1.30, 15), TC_SQUARE))
     k_c = int(np.where(T == TC_SQUARE)[0][0])
+    sizes = (32, 64, 128)
     lnchi, err = {}, {}
-    for L in (16, 32, 64):
+    for L in sizes:
         w = workloads.square_lattice(L, len(T), T[0], T[-1], 16)
         g = levy.build(w.L, w.rho, w.z, w.seed, S=1)
         assert int(g.n_colours[0]) == 2 and np.all(np.diff(g.row_ptr[0]) == 4)
@@ -77,18 +81,22 @@ def test_square_lattice_kt_susceptibility_exponent_at_the_paper_tc():
         blocks = []
         for _ in range(20):
             ens.reset_accumulators()
-            ens.run(400, 10, 1, 1)
+            ens.run(300, 10, 1, 1)
             blocks.append(ens.read_accumulators().sum(0))             # pool the 16 copies of the same lattice
         ens.close()
         est, sig = S.jackknife(np.array(blocks), lambda m: np.log(L * L * m[..., S.M2_]))
         lnchi[L], err[L] = est, sig
-    x = np.log(np.array([16.0, 32.0, 64.0]))
-    y = np.array([lnchi[L] + 2 * R_KT * np.log(np.log(L)) for L in (16, 32, 64)])        # Eq. 27 with the log factor removed
-    slope = ((x - x.mean())[:, None] * (y - y.mean(0))).sum(0) / ((x - x.mean()) ** 2).sum()
-    eta = 2.0 - slope
+    x = np.log(np.array(sizes, np.float64))
+
+    def eta_of(r):              # Eq. 27: ln chi + 2 r ln ln L = (2 - eta) ln L + const
+        y = np.array([lnchi[L] + 2 * r * np.log(np.log(L)) for L in sizes])
+        return 2.0 - ((x - x.mean())[:, None] * (y - y.mean(0))).sum(0) / ((x - x.mean()) ** 2).sum()
+
+    eta = eta_of(0.0)
     print("\nsquare lattice: T        " + " ".join(f"{t:6.3f}" for t in T))
     print("                eta(T)   " + " ".join(f"{e:6.3f}" for e in eta))
-    print(f"eta at the paper's T_c = {TC_SQUARE}: {eta[k_c]:.4f} (paper / KT theory: {ETA_KT}); max jackknife sigma of ln chi {max(e.max() for e in err.values()):.1e}")
+    print(f"eta at the paper's T_c = {TC_SQUARE}: {eta[k_c]:.4f} (paper / KT theory: {ETA_KT}); with Eq. 27's log factor, r = +1/16: "
+          f"{eta_of(R_KT)[k_c]:.4f}, r = -1/16: {eta_of(-R_KT)[k_c]:.4f}; max jackknife sigma of ln chi {max(e.max() for e in err.values()):.1e}")
     assert abs(eta[k_c] - ETA_KT) < 0.03
     assert np.all(np.diff(eta) > -0.01)                  # eta grows with T
     assert eta[0] < 0.20 and eta[-1] > 1.0               # spin-wave phase below, saturating chi above
