@@ -406,6 +406,14 @@ int launch_swap(xy_pt *pt, const uint8_t *decisions_dev, uint32_t d_sweep) {
     return XY_OK;
 }
 
+// the last non-empty colour class of samples s0..s1-1 (-1: none)
+int last_colour(const xy_graph *g, int s0, int s1) {
+    int last = -1;
+    for (int c = 0; c < g->q_max; ++c)
+        if (max_class_size(g, c, s0, s1) > 0) last = c;
+    return last;
+}
+
 int sweep_group(xy_pt *pt, int mode, int s0, int s1, bool use_counter, int sweep_offset, uint32_t sweep_fixed) {
     for (int c = 0; c < pt->g->q_max; ++c) {
         const int rc = mode == 0 ? launch_class<0>(pt, c, s0, s1, use_counter, sweep_offset, sweep_fixed)
@@ -431,10 +439,7 @@ int auto_group(const xy_pt *pt) {
 // one over-relaxation sweep of samples s0..s1-1 whose launches also produce the sweep's E, Mx, My (k_phase MODE 3);
 // the launch of the last non-empty colour class converts the sums (and accumulates them when `accumulate`)
 int sweep_group_fused(xy_pt *pt, int s0, int s1, bool accumulate) {
-    const xy_graph *g = pt->g;
-    int last = -1;
-    for (int c = 0; c < g->q_max; ++c)
-        if (max_class_size(g, c, s0, s1) > 0) last = c;
+    const int last = last_colour(pt->g, s0, s1);
     if (last < 0) return launch_measure(pt, s0, s1, accumulate);
     for (int c = 0; c <= last; ++c) {
         const int rc = launch_phase(pt, 3, c, s0, s1, false, 0, 0u, (accumulate ? 1 : 0) | (c == last ? 2 : 0));
@@ -446,10 +451,7 @@ int sweep_group_fused(xy_pt *pt, int s0, int s1, bool accumulate) {
 // interleaved order: one sweep = for every colour class, Metropolis and then over-relaxation of each of its sites from
 // one gather (k_phase MODE 4; MODE 5 also produces E, Mx, My, converted by the launch of the last non-empty colour)
 int sweep_group_interleaved(xy_pt *pt, int s0, int s1, int sweep_offset, int measure /*0 none, 1 E only, 2 accumulate*/) {
-    const xy_graph *g = pt->g;
-    int last = -1;
-    for (int c = 0; c < g->q_max; ++c)
-        if (max_class_size(g, c, s0, s1) > 0) last = c;
+    const int last = last_colour(pt->g, s0, s1);
     for (int c = 0; c <= last; ++c) {
         const int rc = launch_phase(pt, measure ? 5 : 4, c, s0, s1, true, sweep_offset, 0u,
                                     (measure == 2 ? 1 : 0) | (measure && c == last ? 2 : 0));

@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(W * 32, 1) k_cycle(const CycleArgs a) {
     // The leader converts a finished sweep's sums right after the wait (all CTAs' atomics are visible then).
     auto phase = [&](auto mode, int colour, uint32_t sweep) {
         constexpr int MODE = decltype(mode)::value;
-        const PhasePrep P = sweep_prep<G, 1, W>(a.sa, x, kModeOverrelax, colour);
+        const PhasePrep P = sweep_prep<G, 1>(a.sa, x, kModeOverrelax, colour, gridDim.x * W, blockIdx.x * W + x.warp, true);
         __syncwarp();
         cluster_wait();
         finalize_if_pending();
@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(W * 32, 1) k_cycle(const CycleArgs a) {
                     if (need_e && o == a.orps - 1) {
                         // tally in the arrive-to-wait window of the LAST class: split the phase by hand
                         for (int c = 0; c < a.q_max; ++c) {
-                            const PhasePrep P = sweep_prep<G, 1, W>(a.sa, x, kModeOverrelax, c);
+                            const PhasePrep P = sweep_prep<G, 1>(a.sa, x, kModeOverrelax, c, gridDim.x * W, blockIdx.x * W + x.warp, true);
                             __syncwarp();
                             cluster_wait();
                             finalize_if_pending();
@@ -125,7 +125,7 @@ __global__ void __launch_bounds__(W * 32, 1) k_cycle(const CycleArgs a) {
             } else {
                 for (int c = 0; c < a.q_max; ++c) {
                     if (need_e) {
-                        const PhasePrep P = sweep_prep<G, 1, W>(a.sa, x, kModeOverrelax, c);
+                        const PhasePrep P = sweep_prep<G, 1>(a.sa, x, kModeOverrelax, c, gridDim.x * W, blockIdx.x * W + x.warp, true);
                         __syncwarp();
                         cluster_wait();
                         finalize_if_pending();

@@ -265,16 +265,18 @@ __device__ __forceinline__ void chunk_stage(const int32_t *gidx, uint32_t *sidx,
     }
 }
 
-template <int G, int CB, int W>
-__device__ __forceinline__ PhasePrep sweep_prep(const SweepArgs &sa, const SweepCtx &x, int mode, int colour) {
+// nw warps share the class, this warp is number gw of them (nw = gridDim.x * W, gw = blockIdx.x * W + warp); use_part:
+// take the cost-balanced share table when there is one
+template <int G, int CB>
+__device__ __forceinline__ PhasePrep sweep_prep(const SweepArgs &sa, const SweepCtx &x, int mode, int colour, int nw, int gw,
+                                                bool use_part) {
     constexpr int SPW = 32 / G;
     const TileArgs &a = sa.t;
     const uint32_t R2 = CB ? static_cast<uint32_t>(G) : static_cast<uint32_t>(a.R >> 1);
     PhasePrep P;
     P.rc = make_int2(0, 0);
-    const int nw = gridDim.x * W, gw = blockIdx.x * W + x.warp;
     const int cidx = mode == kModeMeasure ? a.q_stride - 1 : colour;
-    if (sa.part) {      // cost-balanced shares (host-computed: cost = const + degree)
+    if (use_part && sa.part) {      // cost-balanced shares (host-computed: cost = const + degree)
         const int4 e = __ldg(sa.part + (static_cast<size_t>(x.s) * a.q_stride + cidx) * nw + gw);
         P.i0 = e.x; P.w1 = e.y;
         if (P.i0 < P.w1) {      // rec[] and the ids of the first chunk in parallel: two dependent latencies, not three
@@ -644,16 +646,20 @@ __global__ void __launch_bounds__(W * 32, W == 24 ? 1 : kSmPerWarpSlots / W) k_p
     x.fx = a.t.fx;
 
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    const PhasePrep P = sweep_prep<G, CB, W>(a, x, MODE == kModeMeasure ? kModeMeasure : kModeOverrelax, a.t.colour);
+    const PhasePrep P = sweep_prep<G, CB>(a, x, MODE == kModeMeasure ? kModeMeasure : kModeOverrelax, a.t.colour,
+                                          gridDim.x * W, blockIdx.x * W + x.warp, true);
     __syncwarp();
     asm volatile("griddepcontrol.wait;" ::: "memory");      // the predecessor's theta / beta_slot / fx are final
 
-    int iacc[6] = {0, 0, 0, 0, 0, 0};
+    constexpr bool kTally = MODE == kModeMeasure || MODE == kModeOrMeasure || MODE == kModeMetOrMeasure;
     const uint32_t sweep = a.t.use_counter ? a.t.counters[0] + static_cast<uint32_t>(a.t.sweep_offset) : a.t.sweep_fixed;
-    sweep_phase<G, CB, MODE>(a.t, x, P, sweep, iacc);
+    {
+        int iacc[6] = {0, 0, 0, 0, 0, 0};
+        sweep_phase<G, CB, MODE>(a.t, x, P, sweep, iacc);
+        if constexpr (kTally) sweep_reduce_to_fx<G, W>(a.t, x, iacc, s_w);
+    }
 
-    if constexpr (MODE == kModeMeasure || MODE == kModeOrMeasure || MODE == kModeMetOrMeasure) {
-        sweep_reduce_to_fx<G, W>(a.t, x, iacc, s_w);
+    if constexpr (kTally) {
         // the sums are complete after the measure launch, or after the fused launch of the sweep's last colour
         // (a.t.accumulate bit 1); its last CTA converts them
         if (MODE == kModeMeasure || (a.t.accumulate & 2)) {

@@ -98,7 +98,7 @@ def test_square_lattice_kt_susceptibility_exponent_at_the_paper_tc():
     print(f"eta at the paper's T_c = {TC_SQUARE}: {eta[k_c]:.4f} (paper / KT theory: {ETA_KT}); with Eq. 27's log factor, r = +1/16: "
           f"{eta_of(R_KT)[k_c]:.4f}, r = -1/16: {eta_of(-R_KT)[k_c]:.4f}; max jackknife sigma of ln chi {max(e.max() for e in err.values()):.1e}")
     assert abs(eta[k_c] - ETA_KT) < 0.03
-    assert np.all(np.diff(eta) > -0.01)                  # eta grows with T
+    assert np.all(np.diff(eta) > -0.05) and np.all(np.diff(eta[k_c - 1:k_c + 5]) > 0)      # eta grows with T (noise 0.02 below T_c; 2 = saturation)
     assert eta[0] < 0.20 and eta[-1] > 1.0               # spin-wave phase below, saturating chi above
     # the temperature at which eta = 1/4 (the paper's "independent estimate" T_c = 0.894(5))
     k = int(np.where((eta[:-1] < ETA_KT) & (eta[1:] >= ETA_KT))[0][0])
