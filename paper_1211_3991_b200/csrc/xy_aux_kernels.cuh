@@ -6,6 +6,8 @@
 // PAPER.md:444,:454 (coloured single-spin Metropolis), :460 (over-relaxation, ref 66), :167-181 (E, m), :183-190 (chi(k)),
 // :436-440 (random walks), :460-472 (parallel tempering); readings R5-R11, R18, R19 in DESIGN.md.
 #pragma once
+#include <type_traits>
+
 #include "xy_kernels.cuh"
 
 namespace xy {
@@ -199,76 +201,153 @@ __global__ void __launch_bounds__(kBlock) k_fourier(const FourierArgs a) {
     }
 }
 
+// packed fp32x2 helpers of k_fourier2 (one FFMA2 serves the lane's two slots)
+__device__ __forceinline__ void fma2(unsigned long long &acc, unsigned long long a, unsigned long long b) {
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(a), "l"(b));
+}
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ float2 unpack2(unsigned long long v) {
+    float2 r;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
+    return r;
+}
+
 // float2 flavour of k_fourier for R = 2G (G a power of two <= 32) or R a multiple of 64 (G = 32, blockIdx.z = block
-// of 64 slots): a lane owns two adjacent slots, G lanes cover a site, a warp reads 32/G sites per step (one fully used
-// 256-byte request at R >= 64), four steps of loads in flight.  Same fixed-point sums, same finalisation.
+// of 64 slots): a lane owns two adjacent slots, G lanes cover a site, a warp reads 32/G sites per row (one fully used
+// 256-byte request at R >= 64).  The pass is a pure stream and the kernel is bound by ISSUE SLOTS, not by bytes in flight
+// (ncu, profiles/r2b_fourier.md: 64 instructions per row at 69 % issue utilisation), so the row is stripped to the bone:
+//   * a ring of kFourierRing rows per warp filled by cp.async copies of the lane's own 8 bytes (no registers held by
+//     loads in flight, 128 KB per SM on their way), ring slots at compile-time offsets, the source offset a running 32-bit
+//     count, no bounds test on full blocks (the last block of a warp's range runs the predicated variant);
+//   * the site's phase factors (cos, sin)(2 pi x / Lx), (cos, sin)(2 pi y / Ly): lane l loads the coordinates of site
+//     32 b + l two blocks ahead and its table entries one block ahead (no exposed latency; the tables need not survive in
+//     L1, which the stream flushes) and posts the four values in shared memory; a row reads its site's with one LDS.128;
+//   * 4 MUFU + 8 packed FFMA2 (fp32x2, the factor as the scalar operand) for the lane's two slots.
+// Same fixed-point sums, same finalisation as k_fourier.
+constexpr int kFourierRing = 16;
+struct __align__(16) FourierWarp {
+    float2 ring[kFourierRing][32];
+    float4 fac[32];
+};
+constexpr size_t kFourierRed = sizeof(long long) * kWarps * 32 * 16;
+constexpr size_t kFourierSmem = sizeof(FourierWarp) * kWarps > kFourierRed ? sizeof(FourierWarp) * kWarps : kFourierRed;
+
 template <int G>
-__global__ void __launch_bounds__(kBlock) k_fourier2(const FourierArgs a) {
+__global__ void __launch_bounds__(kBlock, 4) k_fourier2(const FourierArgs a) {
     constexpr int SPW = 32 / G;
+    constexpr int NS = kFourierRing;
+    constexpr int RPB = 32 / SPW;         // rows per block of 32 sites
+    constexpr bool kConstSlots = RPB % NS == 0;
+    extern __shared__ __align__(16) unsigned char f_raw[];
     __shared__ int s_last;
     const int s = a.s0 + blockIdx.y;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int sub = lane / G, q = blockIdx.z * G + lane % G;           // slot pair of this lane
-    const int R2 = a.R >> 1;
+    const uint32_t R2 = static_cast<uint32_t>(a.R >> 1);
     const int i0 = (blockIdx.x * kWarps + warp) * a.sites_per_warp;
     const int i1 = min(a.N, i0 + a.sites_per_warp);
     const float2 *th = reinterpret_cast<const float2 *>(a.theta) + static_cast<size_t>(s) * a.N * R2 + q;
     const uint32_t *co = a.coords + static_cast<size_t>(s) * a.N;
-    // fp32 partial sums over <= 256 sites of the lane's own range (fixed order: the partition is a function of N, S
-    // and R only, so a run is bit-reproducible), then exact fixed-point sums across flushes and warps
-    float part[16];
+    FourierWarp *fw = reinterpret_cast<FourierWarp *>(f_raw) + warp;
+    const float2 *ring_l = &fw->ring[0][lane];
+    const uint32_t ring_s = static_cast<uint32_t>(__cvta_generic_to_shared(ring_l));
+    // eight packed fp32x2 partial sums over <= 256 rows of the lane's own range: P[c] = (sum c of the lane's even slot,
+    // of its odd slot).  Fixed order (the partition is a function of N, S and R only), so a run is bit-reproducible;
+    // exact fixed-point sums across flushes, warps and CTAs.
+    unsigned long long P[8];
 #pragma unroll
-    for (int c = 0; c < 16; ++c) part[c] = 0.f;
-    int n_part = 0;
-    auto tally = [&](float t, const float2 p1, const float2 p2, int o) {
-        float sn, cs;
-        __sincosf(t, &sn, &cs);
-        part[o + 0] = fmaf(cs, p1.x, part[o + 0]); part[o + 1] = fmaf(cs, p1.y, part[o + 1]);
-        part[o + 2] = fmaf(sn, p1.x, part[o + 2]); part[o + 3] = fmaf(sn, p1.y, part[o + 3]);
-        part[o + 4] = fmaf(cs, p2.x, part[o + 4]); part[o + 5] = fmaf(cs, p2.y, part[o + 5]);
-        part[o + 6] = fmaf(sn, p2.x, part[o + 6]); part[o + 7] = fmaf(sn, p2.y, part[o + 7]);
+    for (int c = 0; c < 8; ++c) P[c] = 0ull;
+    // f = (c1, s1, c2, s2) = (cos, sin)(2 pi x / Lx), (cos, sin)(2 pi y / Ly) of the row's site
+    auto tally = [&](const float2 t, const float4 f) {
+        float sx, cx, sy, cy;
+        __sincosf(t.x, &sx, &cx);
+        __sincosf(t.y, &sy, &cy);
+        const unsigned long long cs = pack2(cx, cy), sn = pack2(sx, sy);
+        const unsigned long long c1p = pack2(f.x, f.x), s1p = pack2(f.y, f.y), c2p = pack2(f.z, f.z), s2p = pack2(f.w, f.w);
+        fma2(P[0], cs, c1p); fma2(P[1], cs, s1p); fma2(P[2], sn, c1p); fma2(P[3], sn, s1p);
+        fma2(P[4], cs, c2p); fma2(P[5], cs, s2p); fma2(P[6], sn, c2p); fma2(P[7], sn, s2p);
     };
-    auto flush = [&]() {      // rare (once per <= 256 sites and lane): no 64-bit accumulators live in the loop
+    float part[16];                      // [0..7] the even slot's sums, [8..15] the odd slot's (unpacked at a flush only)
+    auto unpack = [&]() {
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            const float2 v = unpack2(P[c]);
+            part[c] = v.x; part[8 + c] = v.y;
+            P[c] = 0ull;
+        }
+    };
+    auto flush = [&]() {      // rare (once per 256 rows and lane): no 64-bit accumulators live in the loop
         unsigned long long *f = reinterpret_cast<unsigned long long *>(a.fk) + (static_cast<size_t>(s) * a.R + 2 * q) * 8;
+        unpack();
 #pragma unroll
-        for (int c = 0; c < 16; ++c) {
+        for (int c = 0; c < 16; ++c)
             atomicAdd(f + c, static_cast<unsigned long long>(__double2ll_rn(static_cast<double>(part[c]) * 4194304.0)));
-            part[c] = 0.f;
-        }
     };
-    // software pipeline: the loads of batch k+1 (4 steps of theta + coordinates) fly while batch k is tallied
-    constexpr int UB = 4;
-    float2 t[UB], tn[UB];
-    uint32_t xy[UB], xyn[UB];
-    auto load = [&](int i, float2 (&tt)[UB], uint32_t (&cc)[UB]) {
-#pragma unroll
-        for (int u = 0; u < UB; ++u) {
-            const int iu = i + u * SPW;
-            tt[u] = make_float2(0.f, 0.f); cc[u] = 0u;
-            if (iu < i1) { tt[u] = __ldcs(th + static_cast<size_t>(iu) * R2); cc[u] = __ldg(co + iu); }
-        }
+    // row r of the warp = sites i0 + r SPW + sub; its copy lands in ring slot r % NS.  n_full = rows whose SPW sites all exist.
+    const int n_rows = i0 < i1 ? (i1 - i0 + SPW - 1) / SPW : 0;
+    const int n_full = i0 < i1 ? (i1 - i0) / SPW : 0;
+    uint32_t off = static_cast<uint32_t>(i0 + sub) * R2;        // float2 offset of the next row to issue (N R / 2 < 2^31)
+    int r_issue = 0;
+    auto issue = [&](auto full, int slot) {     // copy of row r_issue into ring slot `slot`; one group per row, empty or not
+        if (decltype(full)::value || (r_issue < n_rows && i0 + r_issue * SPW + sub < i1))
+            cp_async8(ring_s + static_cast<uint32_t>(slot) * 256u, th + static_cast<unsigned long long>(off));
+        cp_async_commit();
+        off += SPW * R2;
+        r_issue += 1;
     };
-    load(i0 + sub, t, xy);
-    for (int i = i0 + sub; i < i1; i += UB * SPW) {
-        load(i + UB * SPW, tn, xyn);
+    for (int r = 0; r < NS - 1; ++r) issue(std::false_type{}, r);
+    auto load_cw = [&](int b) {
+        const int i = i0 + b * 32 + lane;
+        return i < i1 ? __ldg(co + i) : 0u;
+    };
+    float2 p1n, p2n;
+    uint32_t cw_next = load_cw(1);
+    {
+        const uint32_t cw0 = load_cw(0);
+        p1n = __ldg(a.tab1 + (cw0 & 0xffffu));
+        p2n = __ldg(a.tab2 + (cw0 >> 16));
+    }
+    // one block of 32 sites = RPB rows; FULL: every row read and every row issued by this block exists entirely
+    auto block = [&](auto full, int r0) {
+        constexpr bool FULL = decltype(full)::value;
+        __syncwarp();                                 // the previous block's factors have been read
+        fw->fac[lane] = make_float4(p1n.x, p1n.y, p2n.x, p2n.y);
+        p1n = __ldg(a.tab1 + (cw_next & 0xffffu));
+        p2n = __ldg(a.tab2 + (cw_next >> 16));
+        cw_next = load_cw(r0 / RPB + 2);
+        __syncwarp();
+        constexpr int U = RPB < NS ? RPB : NS;      // unrolled rows: ring slots at compile-time offsets when RPB % NS == 0
+#pragma unroll 1
+        for (int k0 = 0; k0 < RPB; k0 += U) {
 #pragma unroll
-        for (int u = 0; u < UB; ++u) {
-            if (i + u * SPW < i1) {
-                const float2 p1 = __ldg(a.tab1 + (xy[u] & 0xffffu)), p2 = __ldg(a.tab2 + (xy[u] >> 16));
-                tally(t[u].x, p1, p2, 0);
-                tally(t[u].y, p1, p2, 8);
+            for (int u = 0; u < U; ++u) {
+                const int k = k0 + u;
+                const int slot = kConstSlots ? u : (r0 + k) % NS;
+                issue(full, (slot + NS - 1) % NS);
+                cp_async_wait<NS - 1>();      // at most NS - 1 younger groups pending: row r0 + k has landed
+                if (FULL || (r0 + k < n_rows && i0 + (r0 + k) * SPW + sub < i1))
+                    tally(ring_l[slot * 32], fw->fac[k * SPW + sub]);
             }
         }
-#pragma unroll
-        for (int u = 0; u < UB; ++u) { t[u] = tn[u]; xy[u] = xyn[u]; }
-        n_part += UB;
-        if (n_part >= 256) {
-            flush();
-            n_part = 0;
-        }
+    };
+    int r0 = 0;
+    for (; r0 + RPB + NS - 1 <= n_full; r0 += RPB) {
+        block(std::true_type{}, r0);
+        if ((r0 / RPB) % (256 / RPB) == 256 / RPB - 1) flush();
     }
+    for (; r0 < n_rows; r0 += RPB) {
+        block(std::false_type{}, r0);
+        if ((r0 / RPB) % (256 / RPB) == 256 / RPB - 1) flush();
+    }
+    cp_async_wait<0>();
+    unpack();
+    __syncthreads();                      // every warp is done with its ring: the space now serves the reduction
     // end of the range: quantise, add the CTA's warps in shared memory (exact integers), one atomic per CTA and sum
-    __shared__ long long s_red[kWarps][32][16];
+    long long (*s_red)[32][16] = reinterpret_cast<long long (*)[32][16]>(f_raw);
 #pragma unroll
     for (int c = 0; c < 16; ++c) s_red[warp][lane][c] = __double2ll_rn(static_cast<double>(part[c]) * 4194304.0);
     __syncthreads();

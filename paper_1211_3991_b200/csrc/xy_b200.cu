@@ -1214,18 +1214,22 @@ int xy_measure_fourier(xy_pt *pt, double *out_host) {
     a.theta = pt->theta; a.coords = g->coords; a.tab1 = g->tab1; a.tab2 = g->tab2;
     a.fk = pt->fk; a.ticket = pt->ticket; a.temp_of_slot = pt->temp_of_slot;
     a.G_slot = pt->G_slot; a.acc_k = pt->acc_k; a.N = g->N; a.R = R; a.s0 = 0;
-    // one wave of CTAs over all samples and column blocks, at least 32 sites per warp
+    // two waves of 4 CTAs per SM over all samples and column blocks (measured on config 4: one wave 194 us, two 114 us,
+    // three 127 us), at least 32 sites per warp, and at most 224 rows per warp: k_fourier2 flushes its fp32 partial sums
+    // with same-address atomics after 256 rows, which a warp's range should never reach
     const int cb = pt->fast_G ? pt->col_blocks : 1;
-    const int warps_per_sample = std::max(1, std::min(ceil_div(g->N, 32), std::max(1, g->n_sm * 8 * xy::kWarps / (S * cb))));   // two waves of 4 CTAs per SM (one wave measured slower)
+    const int spw = pt->fast_G ? 32 / pt->fast_G : 1;
+    const int warps_per_sample = std::max(1, std::min(ceil_div(g->N, 32), std::max(ceil_div(g->N, 224 * spw),
+                                                                                   g->n_sm * 8 * xy::kWarps / (S * cb))));
     a.sites_per_warp = ceil_div(g->N, warps_per_sample);
     const dim3 grid(ceil_div(ceil_div(g->N, a.sites_per_warp), xy::kWarps), S, cb);
     switch (pt->fast_G) {
-        case 32: xy::k_fourier2<32><<<grid, xy::kBlock, 0, pt->stream>>>(a); break;
-        case 16: xy::k_fourier2<16><<<grid, xy::kBlock, 0, pt->stream>>>(a); break;
-        case 8: xy::k_fourier2<8><<<grid, xy::kBlock, 0, pt->stream>>>(a); break;
-        case 4: xy::k_fourier2<4><<<grid, xy::kBlock, 0, pt->stream>>>(a); break;
-        case 2: xy::k_fourier2<2><<<grid, xy::kBlock, 0, pt->stream>>>(a); break;
-        case 1: xy::k_fourier2<1><<<grid, xy::kBlock, 0, pt->stream>>>(a); break;
+        case 32: xy::k_fourier2<32><<<grid, xy::kBlock, xy::kFourierSmem, pt->stream>>>(a); break;
+        case 16: xy::k_fourier2<16><<<grid, xy::kBlock, xy::kFourierSmem, pt->stream>>>(a); break;
+        case 8: xy::k_fourier2<8><<<grid, xy::kBlock, xy::kFourierSmem, pt->stream>>>(a); break;
+        case 4: xy::k_fourier2<4><<<grid, xy::kBlock, xy::kFourierSmem, pt->stream>>>(a); break;
+        case 2: xy::k_fourier2<2><<<grid, xy::kBlock, xy::kFourierSmem, pt->stream>>>(a); break;
+        case 1: xy::k_fourier2<1><<<grid, xy::kBlock, xy::kFourierSmem, pt->stream>>>(a); break;
         default: xy::k_fourier<<<grid, xy::kBlock, 0, pt->stream>>>(a); break;      // any R
     }
     XY_CUDA(cudaGetLastError());

@@ -60,6 +60,14 @@ __device__ __forceinline__ float u01(uint32_t x) {
     return fmaf(static_cast<float>(x >> 9), 1.1920928955078125e-07f, 5.9604644775390625e-08f);
 }
 
+// ---- cp.async (LDGSTS): 8 bytes per lane, global -> shared, no register staging ---------------------------
+__device__ __forceinline__ void cp_async8(uint32_t smem_addr, const void *gptr) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_addr), "l"(gptr) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 // ---- arguments shared by the update / measure kernels -----------------------------------------------------------------
 struct TileArgs {
     const int2 *rec;           // [S][N] {first col_idx entry (absolute), degree | n_lower << 16}

@@ -79,14 +79,6 @@ __device__ __forceinline__ int quant1(float x) { return __float_as_int(__fadd_rn
 //   |x| <= 32: x + 96 lies in [64, 128], ulp 2^-17, so bits(x + 96) - bits(96) = rn(x 2^17)
 __device__ __forceinline__ int quant32(float x) { return __float_as_int(__fadd_rn(x, 96.0f)) - 0x42C00000; }
 
-// ---- cp.async (LDGSTS): 8 bytes per lane, global -> shared, no register staging ---------------------------
-__device__ __forceinline__ void cp_async8(uint32_t smem_addr, const void *gptr) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_addr), "l"(gptr) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
 // ---- per-lane state of one site (two slots) ----------------------------------------------------------
 // add(t, k): t = the angles of the site's k-th neighbour (CSR order) in the lane's two slots
 template <int MODE> struct PairAcc;
