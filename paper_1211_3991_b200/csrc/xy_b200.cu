@@ -171,9 +171,11 @@ struct xy_pt {
     int capacity_big = 0;            // co-resident 32-warp CTAs (one per SM)
     int cta_shape = 0;               // 0 = by class size, 1 = always 8-warp CTAs, 2 = always 32-warp CTAs
     int path = 0;                    // xy_set_path: 0 = automatic, 1 = one launch per colour class (k_phase), 2 = one cluster per sample (k_cycle)
-    const void *cycle_fn[2] = {nullptr, nullptr};   // k_cycle<G, ORDER, xy::kCycleWarps>, by order
-    int cluster_max = 0;             // largest cluster size the device schedules for k_cycle (0 = not available)
-    int cluster_active[9] = {};      // co-resident clusters of k_cycle by cluster size (1, 2, 4, 8)
+    const void *cycle_fn[2] = {nullptr, nullptr};   // k_cycle<G, ORDER>, by order
+    int cycle_smem_max = 0;          // largest dynamic shared memory of a k_cycle CTA on this device (0 = cluster path not available)
+    // the plan of the cluster path (cycle_plan; made at the first use): CTAs per sample, per-warp resident pool
+    int cycle_planned = 0;           // 0 = not yet, 1 = planned, -1 = the samples do not fit
+    int cycle_C = 0, cycle_k_cap = 0, cycle_id_cap = 0, cycle_resident = 0;
     int fuse_measure = 1;            // measured sweeps: the last over-relaxation sweep also produces E, Mx, My (MODE 3)
     std::map<int, int4 *> parts;     // warps per sample -> device [S][q_stride][nw] share tables {i0, w1, start0, n_run}
     int sweep_capacity = 0;          // co-resident CTAs of k_phase on this device: the grid is one such wave
@@ -525,50 +527,96 @@ int issue_sweeps(xy_pt *pt, int sps, int orps, int group) {
     return XY_OK;
 }
 
-// ---- the cluster path (k_cycle): one thread-block cluster per sample runs whole cycles in one launch ----
-// CTAs per sample: the largest power of two <= the device's cluster limit for which ALL samples' clusters are resident
-// at once (cudaOccupancyMaxActiveClusters: cluster placement is per GPC, so fewer than n_sm / C clusters may fit);
-// 1 when the samples outnumber the SMs
-int cycle_cluster_size(const xy_pt *pt) {
-    for (int c = pt->cluster_max; c > 1; c /= 2)
-        if (pt->cluster_active[c] >= pt->g->S) return c;
-    return 1;
+// ---- the cluster path (k_cycle): one thread-block cluster per sample runs whole cycles in one launch; its warps keep
+// their rows resident in shared memory (xy_cycle.cuh) ----
+// Plan: the largest cluster size C in {8, 4, 2, 1} whose per-warp pool (descriptors + neighbour ids of the rows dealt to a
+// warp, maximum over warps and samples) fits a CTA's shared memory AND for which all S clusters are resident at once
+// (cudaOccupancyMaxActiveClusters with the launch's real shared-memory size: cluster placement is per GPC, so fewer than
+// n_sm / C clusters may fit).  If no C has room for all samples at once, the largest C that fits is used and the clusters
+// run in waves (samples are independent).  Host bookkeeping only.
+void cycle_plan(xy_pt *pt) {
+    if (pt->cycle_planned) return;
+    pt->cycle_planned = -1;
+    const xy_graph *g = pt->g;
+    if (!pt->fast_G || pt->col_blocks != 1 || pt->cycle_smem_max <= 0) return;
+    if (g->q_max > xy::kCycleMaxQ || g->max_degree > 255) return;
+    const int G = pt->fast_G, spw = 32 / G, S = g->S, N = g->N, QS = g->q_stride;
+    int fallback_C = 0, fallback_k = 0, fallback_ids = 0;
+    for (int C = 8; C >= 1; C /= 2) {
+        const int nw = C * xy::kCycleWarps;
+        std::vector<int> rows(nw), ids(nw);
+        int k_cap = 0, id_cap = 0;
+        for (int s = 0; s < S; ++s) {
+            std::fill(rows.begin(), rows.end(), 0);
+            std::fill(ids.begin(), ids.end(), 0);
+            const uint32_t *dg = g->h_deg.data() + static_cast<size_t>(s) * N;
+            const int32_t *cp = g->h_class_ptr.data() + static_cast<size_t>(s) * QS;
+            long long rho = 0;
+            for (int c = 0; c < g->q_max; ++c)
+                for (int i = cp[c]; i < cp[c + 1]; i += spw, ++rho) {
+                    const int owner = static_cast<int>(rho % nw);
+                    rows[owner] += 1;
+                    for (int k = i; k < std::min(i + spw, cp[c + 1]); ++k) ids[owner] += static_cast<int>(dg[k] & 0xffffu);
+                }
+            k_cap = std::max(k_cap, *std::max_element(rows.begin(), rows.end()));
+            id_cap = std::max(id_cap, *std::max_element(ids.begin(), ids.end()));
+        }
+        k_cap = std::max(k_cap, 1);
+        id_cap = std::max((id_cap + 3) / 4 * 4, 4);
+        if (id_cap > 0xffff) continue;
+        const size_t smem = xy::cycle_pool_bytes(G, k_cap, id_cap) * xy::kCycleWarps;
+        if (smem > static_cast<size_t>(pt->cycle_smem_max)) continue;
+        if (!fallback_C) { fallback_C = C; fallback_k = k_cap; fallback_ids = id_cap; }
+        cudaLaunchConfig_t qc = {};
+        cudaLaunchAttribute qa;
+        qa.id = cudaLaunchAttributeClusterDimension;
+        qa.val.clusterDim.x = C; qa.val.clusterDim.y = 1; qa.val.clusterDim.z = 1;
+        qc.gridDim = dim3(C, 1, 1); qc.blockDim = dim3(xy::kCycleWarps * 32);
+        qc.dynamicSmemBytes = smem;
+        qc.attrs = &qa; qc.numAttrs = 1;
+        int n_active = 0;
+        if (cudaOccupancyMaxActiveClusters(&n_active, pt->cycle_fn[0], &qc) != cudaSuccess) { cudaGetLastError(); continue; }
+        if (n_active >= S) {
+            pt->cycle_C = C; pt->cycle_k_cap = k_cap; pt->cycle_id_cap = id_cap; pt->cycle_resident = 1; pt->cycle_planned = 1;
+            return;
+        }
+    }
+    if (fallback_C) {
+        pt->cycle_C = fallback_C; pt->cycle_k_cap = fallback_k; pt->cycle_id_cap = fallback_ids; pt->cycle_resident = 0;
+        pt->cycle_planned = 1;
+    }
 }
 
-// the cluster path serves one column block (R = 2G <= 64) with at least one over-relaxation sweep per Metropolis sweep
-bool cycle_eligible(const xy_pt *pt, int orps) {
-    return pt->fast_G && pt->col_blocks == 1 && pt->cluster_max >= 1 && orps >= 1 && pt->fuse_measure;
+// the cluster path serves one column block (R = 2G <= 64) with at least one over-relaxation sweep per Metropolis sweep,
+// samples whose rows fit the warps' resident pools, at most kCycleMaxQ colours and degrees <= 255
+bool cycle_eligible(xy_pt *pt, int orps) {
+    if (!(pt->fast_G && pt->col_blocks == 1 && orps >= 1 && pt->fuse_measure)) return false;
+    cycle_plan(pt);
+    return pt->cycle_planned == 1;
 }
 
-// automatic choice (measured, DESIGN.md 7.2 / 7.6): a colour-class phase of the cluster path costs what a PDL-chained
-// launch costs -- both are bound by the serial chain of one phase (stage the share, gather, ~1000 dependent instructions
-// per warp, store, release), not by the launch -- so the cluster path only wins where the launch path cannot overlap
-// anything: samples so small that a class is at most one row per warp of the cluster.
-bool use_cycle_path(const xy_pt *pt, int orps) {
+// automatic choice (measured): the cluster path wins while a class is a few rows per warp -- the serial
+// chain of one class (barrier, one L2 round trip, the update) is then what a sweep costs -- and all samples' clusters are
+// resident at once; with many rows per warp the per-launch path's 32 warps per SM and cost-balanced shares are faster.
+bool use_cycle_path(xy_pt *pt, int orps) {
     if (pt->path == 1 || !cycle_eligible(pt, orps)) return false;
     if (pt->path == 2) return true;
-    const xy_graph *g = pt->g;
-    const int C = cycle_cluster_size(pt);
-    const double rows_per_warp = static_cast<double>(ceil_div(max_class_size(g, 0, 0, g->S), 32 / pt->fast_G)) / (C * xy::kCycleWarps);
-    return rows_per_warp <= 1.0;
+    return pt->cycle_resident && pt->cycle_k_cap <= xy::kCycleAutoRows;
 }
 
 int launch_cycle(xy_pt *pt, int n_cycles, int sps, int orps, int me, bool do_swap) {
     const xy_graph *g = pt->g;
     if (n_cycles <= 0) return XY_OK;
-    const int C = cycle_cluster_size(pt);
+    const int C = pt->cycle_C;
     xy::CycleArgs a;
-    a.sa = sweep_args(pt, 0);
-    if (pt->balance) {
-        const int rc = get_partition(pt, C * xy::kCycleWarps, &a.sa.part);
-        if (rc != XY_OK) return rc;
-    }
+    a.t = tile_args(pt, 0, 0);
     a.sw = swap_args(pt, nullptr);
     a.n_cycles = n_cycles; a.sps = sps; a.orps = orps; a.me = me; a.q_max = g->q_max; a.do_swap = do_swap ? 1 : 0;
+    a.k_cap = pt->cycle_k_cap; a.id_cap = pt->cycle_id_cap;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(C, g->S, 1);
     cfg.blockDim = dim3(xy::kCycleWarps * 32);
-    cfg.dynamicSmemBytes = xy::sweep_smem(xy::kCycleWarps);
+    cfg.dynamicSmemBytes = xy::cycle_pool_bytes(pt->fast_G, a.k_cap, a.id_cap) * xy::kCycleWarps;
     cfg.stream = pt->stream;
     cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -947,36 +995,23 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
         }
         pt->sweep_capacity = per_sm * n_sm;
         pt->capacity_big = std::max(1, per_sm_big) * n_sm;
-        // the cluster path (k_cycle): one column block only; ask the device which cluster sizes it schedules
+        // the cluster path (k_cycle): one column block only; opt in to all the shared memory a CTA may have (the plan made at
+        // the first use sizes the launch)
         if (pt->col_blocks == 1) {
             pt->cycle_fn[0] = xy::cycle_function(0, pt->fast_G);
             pt->cycle_fn[1] = xy::cycle_function(1, pt->fast_G);
-            cudaError_t ec = cudaSuccess;
+            int optin = 0;
+            cudaError_t ec = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+            int dyn_max = 0;
             for (int o = 0; o < 2 && ec == cudaSuccess; ++o) {
-                ec = cudaFuncSetAttribute(pt->cycle_fn[o], cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          static_cast<int>(xy::sweep_smem(xy::kCycleWarps)));
+                cudaFuncAttributes fa;
+                ec = cudaFuncGetAttributes(&fa, pt->cycle_fn[o]);
+                if (ec != cudaSuccess) break;
+                const int room = optin - static_cast<int>(fa.sharedSizeBytes);
+                dyn_max = o == 0 ? room : std::min(dyn_max, room);
+                ec = cudaFuncSetAttribute(pt->cycle_fn[o], cudaFuncAttributeMaxDynamicSharedMemorySize, room);
             }
-            int max_cluster = 0;
-            if (ec == cudaSuccess) {
-                cudaLaunchConfig_t qc = {};
-                qc.gridDim = dim3(8, 1, 1); qc.blockDim = dim3(xy::kCycleWarps * 32);
-                qc.dynamicSmemBytes = xy::sweep_smem(xy::kCycleWarps);
-                ec = cudaOccupancyMaxPotentialClusterSize(&max_cluster, pt->cycle_fn[0], &qc);
-            }
-            pt->cluster_max = 0;
-            for (int c = 1; c <= 8 && ec == cudaSuccess && c <= max_cluster; c *= 2) {
-                cudaLaunchConfig_t qc = {};
-                cudaLaunchAttribute qa;
-                qa.id = cudaLaunchAttributeClusterDimension;
-                qa.val.clusterDim.x = c; qa.val.clusterDim.y = 1; qa.val.clusterDim.z = 1;
-                qc.gridDim = dim3(c, 1, 1); qc.blockDim = dim3(xy::kCycleWarps * 32);
-                qc.dynamicSmemBytes = xy::sweep_smem(xy::kCycleWarps);
-                qc.attrs = &qa; qc.numAttrs = 1;
-                int n_active = 0;
-                if (cudaOccupancyMaxActiveClusters(&n_active, pt->cycle_fn[0], &qc) != cudaSuccess || n_active < 1) break;
-                pt->cluster_active[c] = n_active;
-                pt->cluster_max = c;
-            }
+            pt->cycle_smem_max = ec == cudaSuccess ? dyn_max : 0;
             cudaGetLastError();
         }
         // persisting L2 carve-out for the access-policy windows of the sample groups; xy_pt_destroy puts the limit back
@@ -1273,8 +1308,9 @@ int xy_set_schedule(xy_pt *pt, int samples_per_group) {
 
 int xy_set_path(xy_pt *pt, int path) {
     if (!check_pt(pt) || path < 0 || path > 2) return fail(XY_EINVAL, "bad handle or path not in {0, 1, 2}");
-    if (path == 2 && !(pt->fast_G && pt->col_blocks == 1 && pt->cluster_max >= 1))
-        return fail(XY_ESTATE, "the cluster path needs R = 2 * 2^k <= 64 and a device that schedules thread-block clusters");
+    if (path == 2 && !cycle_eligible(pt, 1))
+        return fail(XY_ESTATE, "the cluster path needs R = 2 * 2^k <= 64, fused measurement, samples whose rows fit the warps' "
+                               "resident pools (shared memory), at most 12 colours and degrees <= 255");
     pt->path = path;
     return XY_OK;
 }
@@ -1283,7 +1319,7 @@ int xy_get_path(xy_pt *pt, int or_per_sweep, int *path, int *cluster_size) {
     if (!check_pt(pt)) return fail(XY_EINVAL, "bad handle");
     const bool cyc = use_cycle_path(pt, or_per_sweep);
     if (path) *path = cyc ? 2 : 1;
-    if (cluster_size) *cluster_size = cyc ? cycle_cluster_size(pt) : 0;
+    if (cluster_size) *cluster_size = cyc ? pt->cycle_C : 0;
     return XY_OK;
 }
 
@@ -1314,7 +1350,7 @@ int xy_run(xy_pt *pt, int n_cycles, int sps, int orps, int me) {
     DeviceGuard guard(pt->g->device);
     if (pt->order == 1 && orps != 1) return fail(XY_EINVAL, "the interleaved order needs or_per_sweep == 1");
     if (pt->path == 2 && !cycle_eligible(pt, orps))
-        return fail(XY_ESTATE, "xy_set_path(2): the cluster path needs R = 2 * 2^k <= 64, or_per_sweep >= 1 and fused measurement");
+        return fail(XY_ESTATE, "xy_set_path(2): the cluster path needs R = 2 * 2^k <= 64, or_per_sweep >= 1, fused measurement and samples that fit its resident pools");
     if (use_cycle_path(pt, orps)) {          // small samples: all cycles in one launch, one cluster per sample
         int rc = settle_upload(pt);
         if (rc == XY_OK) rc = launch_cycle(pt, n_cycles, sps, orps, me, true);
@@ -1357,7 +1393,7 @@ int xy_run_sweeps(xy_pt *pt, int n_blocks, int sps, int orps) {
     { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
     if (pt->order == 1 && orps != 1) return fail(XY_EINVAL, "the interleaved order needs or_per_sweep == 1");
     if (pt->path == 2 && !cycle_eligible(pt, orps))
-        return fail(XY_ESTATE, "xy_set_path(2): the cluster path needs R = 2 * 2^k <= 64, or_per_sweep >= 1 and fused measurement");
+        return fail(XY_ESTATE, "xy_set_path(2): the cluster path needs R = 2 * 2^k <= 64, or_per_sweep >= 1, fused measurement and samples that fit its resident pools");
     if (use_cycle_path(pt, orps)) {
         const int rc = launch_cycle(pt, n_blocks, sps, orps, 0, false);
         if (rc != XY_OK) return rc;

@@ -5,12 +5,14 @@
 
 namespace xy {
 
-constexpr int kCycleWarps = 16;      // warps per CTA of k_cycle (128 registers per thread, one CTA per SM)
+constexpr int kCycleWarps = 16;      // warps per CTA of k_cycle (64 registers per thread, up to two CTAs per SM)
+constexpr int kCycleMaxQ = 12;       // most colours a sample may have on the cluster path
+constexpr int kCycleAutoRows = 10;   // automatic path choice: cluster path while a warp owns at most this many rows
 
 // k_phase<G, CB, MODE, W> for W in {8, 32} (MODE 0..5) and W = 24 (MODE 3, 5 only); CB = single_block ? 1 : 0 (G = 32 only).
 // nullptr for a combination that is not built.
 const void *phase_function(int W, int G, bool single_block, int mode);
-// k_cycle<G, ORDER, kCycleWarps>
+// k_cycle<G, ORDER>
 const void *cycle_function(int order, int G);
 
 // per translation unit

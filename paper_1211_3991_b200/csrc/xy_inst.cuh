@@ -24,12 +24,12 @@ const void *phase_function_mode(int G, bool single_block) {
 template <int ORDER>
 const void *cycle_function_order(int G) {
     switch (G) {
-        case 32: return reinterpret_cast<const void *>(k_cycle<32, ORDER, kCycleWarps>);
-        case 16: return reinterpret_cast<const void *>(k_cycle<16, ORDER, kCycleWarps>);
-        case 8: return reinterpret_cast<const void *>(k_cycle<8, ORDER, kCycleWarps>);
-        case 4: return reinterpret_cast<const void *>(k_cycle<4, ORDER, kCycleWarps>);
-        case 2: return reinterpret_cast<const void *>(k_cycle<2, ORDER, kCycleWarps>);
-        default: return reinterpret_cast<const void *>(k_cycle<1, ORDER, kCycleWarps>);
+        case 32: return reinterpret_cast<const void *>(k_cycle<32, ORDER>);
+        case 16: return reinterpret_cast<const void *>(k_cycle<16, ORDER>);
+        case 8: return reinterpret_cast<const void *>(k_cycle<8, ORDER>);
+        case 4: return reinterpret_cast<const void *>(k_cycle<4, ORDER>);
+        case 2: return reinterpret_cast<const void *>(k_cycle<2, ORDER>);
+        default: return reinterpret_cast<const void *>(k_cycle<1, ORDER>);
     }
 }
 

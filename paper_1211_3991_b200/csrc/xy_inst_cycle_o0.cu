@@ -1,4 +1,4 @@
-// k_cycle<G, ORDER = 0, kCycleWarps> (see xy_dispatch.h)
+// k_cycle<G, ORDER = 0> (see xy_dispatch.h)
 #include "xy_inst.cuh"
 
 namespace xy {
