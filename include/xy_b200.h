@@ -137,13 +137,15 @@ int xy_set_schedule(xy_pt *pt, int samples_per_group);
 
 /* Execution path of xy_run / xy_run_sweeps ("subsets ... processed sequentially on
  * each MCS").  1 = one launch per colour class (k_phase) captured in a CUDA graph with programmatic-dependent-launch
- * edges: right when a class fills the chip.  2 = one THREAD-BLOCK CLUSTER per sample (k_cycle): all colour classes of all
- * sweeps of all requested cycles, the fused measurement and the swap round run in ONE launch, the classes separated by
- * the hardware cluster barrier -- right when a class is a few hundred rows and a launch is latency-bound; needs
- * R = 2 * 2^k <= 64, or_per_sweep >= 1 and fused measurement (else XY_ESTATE from xy_set_path / xy_run).  0 (default) =
- * automatic: path 2 where it applies and the samples are small, else path 1.  Both paths give bit-identical angles,
- * labels, accumulators and counters.  xy_get_path reports what xy_run(or_per_sweep) would use (1 or 2) and the cluster
- * size (CTAs per sample; 0 for path 1); either output may be NULL. */
+ * edges: right when a class fills the chip.  2 = one THREAD-BLOCK CLUSTER per sample (k_cycle): the sample's angles live
+ * in the cluster's distributed shared memory for the whole launch, every warp owns a fixed set of rows, and all colour
+ * classes of all sweeps of all requested cycles, the fused measurement and the swap round run in ONE launch, the classes
+ * separated by the hardware cluster barrier -- right when a class is a few rows per warp and a launch is latency-bound.
+ * It needs R = 2 * 2^k <= 64, or_per_sweep >= 1, fused measurement, at most 12 colours, degrees <= 255 and samples small
+ * enough for the shared memory of a cluster of <= 16 CTAs (else XY_ESTATE from xy_set_path / xy_run).  0 (default) =
+ * automatic: path 2 where it applies, all samples' clusters are resident at once and a warp owns at most 20 rows, else
+ * path 1.  Both paths give bit-identical angles, labels, accumulators and counters.  xy_get_path reports what
+ * xy_run(or_per_sweep) would use (1 or 2) and the cluster size (CTAs per sample; 0 for path 1); either output may be NULL. */
 int xy_set_path(xy_pt *pt, int path);
 int xy_get_path(xy_pt *pt, int or_per_sweep, int *path, int *cluster_size);
 

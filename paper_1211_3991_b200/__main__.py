@@ -25,6 +25,8 @@ def main(argv=None):
     ap.add_argument("--replicas", type=int, default=64)
     ap.add_argument("--samples", type=int, default=8)
     ap.add_argument("--seed", type=lambda v: int(v, 0), default=0xB200_1211_3991)
+    ap.add_argument("--colouring", default="reduced", choices=["reduced", "smallest-last"],
+                    help="reduced = smallest-last followed by the builder's colour-reducing local search (bench.py's default)")
     a = ap.parse_args(argv)
 
     import torch
@@ -43,7 +45,8 @@ def main(argv=None):
     else:
         w = workloads.square_lattice(k, a.replicas, 0.7, 1.3, a.samples)
         tile = w.S
-    g = levy.build(w.L, w.rho, w.z, w.seed, S=1 if tile > 1 else w.S)
+    g = levy.build(w.L, w.rho, w.z, w.seed, S=1 if tile > 1 else w.S,
+                   reduce_colours=workloads.REDUCE_COLOURS if a.colouring == "reduced" else 0)
     rp, ci, col = (np.tile(x, (tile, 1)) for x in (g.row_ptr, g.col_idx, g.colour))
     ens = B.Ensemble(rp, ci, col, w.temperatures(), a.seed)
     ens.set_order(a.order)

@@ -173,6 +173,7 @@ struct xy_pt {
     int path = 0;                    // xy_set_path: 0 = automatic, 1 = one launch per colour class (k_phase), 2 = one cluster per sample (k_cycle)
     const void *cycle_fn[2] = {nullptr, nullptr};   // k_cycle<G, ORDER>, by order
     int cycle_smem_max = 0;          // largest dynamic shared memory of a k_cycle CTA on this device (0 = cluster path not available)
+    int cycle_C_max = 8;             // largest cluster size tried: 16 when the device allows the non-portable size
     // the plan of the cluster path (cycle_plan; made at the first use): CTAs per sample, per-warp resident pool
     int cycle_planned = 0;           // 0 = not yet, 1 = planned, -1 = the samples do not fit
     int cycle_C = 0, cycle_k_cap = 0, cycle_id_cap = 0, cycle_resident = 0;
@@ -542,7 +543,7 @@ void cycle_plan(xy_pt *pt) {
     if (g->q_max > xy::kCycleMaxQ || g->max_degree > 255) return;
     const int G = pt->fast_G, spw = 32 / G, S = g->S, N = g->N, QS = g->q_stride;
     int fallback_C = 0, fallback_k = 0, fallback_ids = 0;
-    for (int C = 8; C >= 1; C /= 2) {
+    for (int C = pt->cycle_C_max; C >= 1; C /= 2) {
         const int nw = C * xy::kCycleWarps;
         std::vector<int> rows(nw), ids(nw);
         int k_cap = 0, id_cap = 0;
@@ -1010,6 +1011,12 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
                 const int room = optin - static_cast<int>(fa.sharedSizeBytes);
                 dyn_max = o == 0 ? room : std::min(dyn_max, room);
                 ec = cudaFuncSetAttribute(pt->cycle_fn[o], cudaFuncAttributeMaxDynamicSharedMemorySize, room);
+                if (ec == cudaSuccess && cudaFuncSetAttribute(pt->cycle_fn[o], cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) {
+                    cudaGetLastError();
+                    pt->cycle_C_max = 8;
+                } else if (o == 0) {
+                    pt->cycle_C_max = 16;
+                }
             }
             pt->cycle_smem_max = ec == cudaSuccess ? dyn_max : 0;
             cudaGetLastError();

@@ -34,7 +34,7 @@ def test_cluster_path_is_bit_identical_to_the_launch_path(L, rho, R, S, order):
     T = O.geometric_temperatures(R, 1.0, 4.0)
     a = U.ensemble_from_levy(g, T, SEED, sample_base=3); a.set_path(1); a.set_order(order)
     b = U.ensemble_from_levy(g, T, SEED, sample_base=3); b.set_path(2); b.set_order(order)
-    assert a.get_path()[0] == 1 and b.get_path()[0] == 2 and 1 <= b.get_path()[1] <= 8
+    assert a.get_path()[0] == 1 and b.get_path()[0] == 2 and 1 <= b.get_path()[1] <= 16
     for (n, sps, orps, me) in [(3, 10, 1, 1), (2, 4, 1 if order else 2, 3), (1, 1, 1, 0), (4, 3, 1, 2)]:
         a.run(n, sps, orps, me); b.run(n, sps, orps, me)
         same_state(a, b, (n, sps, orps, me))
