@@ -229,14 +229,42 @@ __device__ __forceinline__ float2 unpack2(unsigned long long v) {
 //   * 4 MUFU + 8 packed FFMA2 (fp32x2, the factor as the scalar operand) for the lane's two slots.
 // Same fixed-point sums, same finalisation as k_fourier.
 constexpr int kFourierRing = 16;
+constexpr int kFourierStageRows = 4;                                   // BULK: rows per bulk copy (1 KB) and mbarrier
+constexpr int kFourierStages = kFourierRing / kFourierStageRows;
 struct __align__(16) FourierWarp {
     float2 ring[kFourierRing][32];
     float4 fac[32];
+    unsigned long long bar[kFourierStages];      // BULK: one mbarrier per stage of the ring
 };
+
+// ---- bulk asynchronous copies (cp.async.bulk: the TMA engine moves a contiguous run global -> shared without passing
+// L1TEX and signals an mbarrier with the bytes it delivered) ----
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_copy_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "FOURIER_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra FOURIER_DONE;\n"
+        "bra FOURIER_WAIT;\n"
+        "FOURIER_DONE:\n"
+        "}" ::"r"(bar), "r"(parity) : "memory");
+}
+
 constexpr size_t kFourierRed = sizeof(long long) * kWarps * 32 * 16;
 constexpr size_t kFourierSmem = sizeof(FourierWarp) * kWarps > kFourierRed ? sizeof(FourierWarp) * kWarps : kFourierRed;
 
-template <int G>
+template <int G, bool BULK>
 __global__ void __launch_bounds__(kBlock, 4) k_fourier2(const FourierArgs a) {
     constexpr int SPW = 32 / G;
     constexpr int NS = kFourierRing;
@@ -293,13 +321,50 @@ __global__ void __launch_bounds__(kBlock, 4) k_fourier2(const FourierArgs a) {
     uint32_t off = static_cast<uint32_t>(i0 + sub) * R2;        // float2 offset of the next row to issue (N R / 2 < 2^31)
     int r_issue = 0;
     auto issue = [&](auto full, int slot) {     // copy of row r_issue into ring slot `slot`; one group per row, empty or not
-        if (decltype(full)::value || (r_issue < n_rows && i0 + r_issue * SPW + sub < i1))
-            cp_async8(ring_s + static_cast<uint32_t>(slot) * 256u, th + static_cast<unsigned long long>(off));
-        cp_async_commit();
-        off += SPW * R2;
-        r_issue += 1;
+        if constexpr (!BULK) {
+            if (decltype(full)::value || (r_issue < n_rows && i0 + r_issue * SPW + sub < i1))
+                cp_async8(ring_s + static_cast<uint32_t>(slot) * 256u, th + static_cast<unsigned long long>(off));
+            cp_async_commit();
+            off += SPW * R2;
+            r_issue += 1;
+        }
     };
-    for (int r = 0; r < NS - 1; ++r) issue(std::false_type{}, r);
+    // BULK: the ring is filled a stage (kFourierStageRows rows, 1 KB) at a time by lane 0: one bulk copy when the rows
+    // are contiguous in memory (R = 2 G: one column block), else one per row; the stage's mbarrier counts the bytes
+    constexpr int RS = kFourierStageRows, NST = kFourierStages;
+    const uint32_t bar_s = static_cast<uint32_t>(__cvta_generic_to_shared(&fw->bar[0]));
+    const uint32_t stage_s = static_cast<uint32_t>(__cvta_generic_to_shared(&fw->ring[0][0]));
+    const unsigned char *row_src = reinterpret_cast<const unsigned char *>(
+        reinterpret_cast<const float2 *>(a.theta) + static_cast<size_t>(s) * a.N * R2 + blockIdx.z * G);      // + 8 R2 per site
+    auto issue_stage = [&](int st) {
+        if (st * RS < n_rows && lane == 0) {
+            const uint32_t bar = bar_s + static_cast<uint32_t>(st % NST) * 8u, dst = stage_s + static_cast<uint32_t>(st % NST) * (RS * 256u);
+            const int site0 = i0 + st * RS * SPW;
+            const int n_sites = min(RS * SPW, i1 - site0);                       // sites of the stage that exist
+            const uint32_t total = static_cast<uint32_t>(n_sites) * (G * 8u);
+            mbar_expect_tx(bar, total);
+            const unsigned char *src = row_src + static_cast<size_t>(site0) * R2 * 8u;
+            if (R2 == static_cast<uint32_t>(G)) {
+                bulk_copy_g2s(dst, src, total, bar);
+            } else {      // R > 64: a row is one site's 256 bytes, rows R2 * 8 bytes apart
+                for (int k = 0; k < n_sites; ++k) bulk_copy_g2s(dst + k * 256u, src + static_cast<size_t>(k) * R2 * 8u, 256u, bar);
+            }
+        }
+    };
+    auto wait_stage = [&](int st) {
+        if (st * RS < n_rows) mbar_wait(bar_s + static_cast<uint32_t>(st % NST) * 8u, static_cast<uint32_t>(st / NST) & 1u);
+    };
+    if constexpr (BULK) {
+        if (lane == 0) {
+#pragma unroll
+            for (int k = 0; k < NST; ++k) mbar_init(bar_s + k * 8u, 1u);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        __syncwarp();
+        for (int st = 0; st < NST - 1; ++st) issue_stage(st);
+    } else {
+        for (int r = 0; r < NS - 1; ++r) issue(std::false_type{}, r);
+    }
     auto load_cw = [&](int b) {
         const int i = i0 + b * 32 + lane;
         return i < i1 ? __ldg(co + i) : 0u;
@@ -327,8 +392,16 @@ __global__ void __launch_bounds__(kBlock, 4) k_fourier2(const FourierArgs a) {
             for (int u = 0; u < U; ++u) {
                 const int k = k0 + u;
                 const int slot = kConstSlots ? u : (r0 + k) % NS;
-                issue(full, (slot + NS - 1) % NS);
-                cp_async_wait<NS - 1>();      // at most NS - 1 younger groups pending: row r0 + k has landed
+                if constexpr (BULK) {
+                    if ((kConstSlots ? u : r0 + k) % RS == 0) {      // first row of a stage: refill the stage just read, wait for this one
+                        __syncwarp();
+                        issue_stage((r0 + k) / RS + NST - 1);
+                        wait_stage((r0 + k) / RS);
+                    }
+                } else {
+                    issue(full, (slot + NS - 1) % NS);
+                    cp_async_wait<NS - 1>();      // at most NS - 1 younger groups pending: row r0 + k has landed
+                }
                 if (FULL || (r0 + k < n_rows && i0 + (r0 + k) * SPW + sub < i1))
                     tally(ring_l[slot * 32], fw->fac[k * SPW + sub]);
             }
@@ -343,7 +416,7 @@ __global__ void __launch_bounds__(kBlock, 4) k_fourier2(const FourierArgs a) {
         block(std::false_type{}, r0);
         if ((r0 / RPB) % (256 / RPB) == 256 / RPB - 1) flush();
     }
-    cp_async_wait<0>();
+    if constexpr (!BULK) cp_async_wait<0>();
     unpack();
     __syncthreads();                      // every warp is done with its ring: the space now serves the reduction
     // end of the range: quantise, add the CTA's warps in shared memory (exact integers), one atomic per CTA and sum

@@ -1265,15 +1265,18 @@ int xy_measure_fourier(xy_pt *pt, double *out_host) {
                                                                                    g->n_sm * 8 * xy::kWarps / (S * cb))));
     a.sites_per_warp = ceil_div(g->N, warps_per_sample);
     const dim3 grid(ceil_div(ceil_div(g->N, a.sites_per_warp), xy::kWarps), S, cb);
+    // bulk-copy flavour (TMA fills the ring): needs 16-byte aligned rows -- G >= 2 and a 16-byte aligned theta
+    const bool bulk = pt->fast_G >= 2 && (reinterpret_cast<uintptr_t>(pt->theta) & 15u) == 0;
+#define XY_FOURIER2(GG)                                                                                     \
+    case GG:                                                                                                \
+        if (bulk) xy::k_fourier2<GG, (GG >= 2)><<<grid, xy::kBlock, xy::kFourierSmem, pt->stream>>>(a);     \
+        else xy::k_fourier2<GG, false><<<grid, xy::kBlock, xy::kFourierSmem, pt->stream>>>(a);              \
+        break;
     switch (pt->fast_G) {
-        case 32: xy::k_fourier2<32><<<grid, xy::kBlock, xy::kFourierSmem, pt->stream>>>(a); break;
-        case 16: xy::k_fourier2<16><<<grid, xy::kBlock, xy::kFourierSmem, pt->stream>>>(a); break;
-        case 8: xy::k_fourier2<8><<<grid, xy::kBlock, xy::kFourierSmem, pt->stream>>>(a); break;
-        case 4: xy::k_fourier2<4><<<grid, xy::kBlock, xy::kFourierSmem, pt->stream>>>(a); break;
-        case 2: xy::k_fourier2<2><<<grid, xy::kBlock, xy::kFourierSmem, pt->stream>>>(a); break;
-        case 1: xy::k_fourier2<1><<<grid, xy::kBlock, xy::kFourierSmem, pt->stream>>>(a); break;
+        XY_FOURIER2(32) XY_FOURIER2(16) XY_FOURIER2(8) XY_FOURIER2(4) XY_FOURIER2(2) XY_FOURIER2(1)
         default: xy::k_fourier<<<grid, xy::kBlock, 0, pt->stream>>>(a); break;      // any R
     }
+#undef XY_FOURIER2
     XY_CUDA(cudaGetLastError());
     pt->launches += 1;
     if (out_host) {
