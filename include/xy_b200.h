@@ -143,7 +143,7 @@ int xy_set_schedule(xy_pt *pt, int samples_per_group);
  * separated by the hardware cluster barrier -- right when a class is a few rows per warp and a launch is latency-bound.
  * It needs R = 2 * 2^k <= 64, or_per_sweep >= 1, fused measurement, at most 12 colours, degrees <= 255 and samples small
  * enough for the shared memory of a cluster of <= 16 CTAs (else XY_ESTATE from xy_set_path / xy_run).  0 (default) =
- * automatic: path 2 where it applies, all samples' clusters are resident at once and a warp owns at most 20 rows, else
+ * automatic: path 2 where it applies, all samples' clusters are resident at once and a warp owns at most 36 rows, else
  * path 1.  Both paths give bit-identical angles, labels, accumulators and counters.  xy_get_path reports what
  * xy_run(or_per_sweep) would use (1 or 2) and the cluster size (CTAs per sample; 0 for path 1); either output may be NULL. */
 int xy_set_path(xy_pt *pt, int path);

@@ -544,21 +544,28 @@ void cycle_plan(xy_pt *pt) {
     const int G = pt->fast_G, spw = 32 / G, S = g->S, N = g->N, QS = g->q_stride;
     int fallback_C = 0, fallback_k = 0, fallback_ids = 0;
     for (int C = pt->cycle_C_max; C >= 1; C /= 2) {
-        const int nw = C * xy::kCycleWarps;
+        const int W = xy::kCycleWarps, nw = C * W;
         std::vector<int> rows(nw), ids(nw);
         int k_cap = 0, id_cap = 0;
-        for (int s = 0; s < S; ++s) {
+        for (int s = 0; s < S; ++s) {      // the ownership rule of k_cycle (xy_cycle.cuh): CTA b owns a contiguous range of every class
             std::fill(rows.begin(), rows.end(), 0);
             std::fill(ids.begin(), ids.end(), 0);
             const uint32_t *dg = g->h_deg.data() + static_cast<size_t>(s) * N;
             const int32_t *cp = g->h_class_ptr.data() + static_cast<size_t>(s) * QS;
-            long long rho = 0;
-            for (int c = 0; c < g->q_max; ++c)
-                for (int i = cp[c]; i < cp[c + 1]; i += spw, ++rho) {
-                    const int owner = static_cast<int>(rho % nw);
-                    rows[owner] += 1;
-                    for (int k = i; k < std::min(i + spw, cp[c + 1]); ++k) ids[owner] += static_cast<int>(dg[k] & 0xffffu);
+            std::vector<int> nu0(C, 0);                                  // rows of the earlier classes per CTA
+            for (int c = 0; c < g->q_max; ++c) {
+                const int n_rows = (cp[c + 1] - cp[c] + spw - 1) / spw;
+                for (int b = 0; b < C; ++b) {
+                    const int k0 = xy::cycle_first_row(b, n_rows, C), k1 = xy::cycle_first_row(b + 1, n_rows, C);
+                    for (int k = k0; k < k1; ++k) {
+                        const int owner = b * W + (nu0[b] + k - k0) % W;
+                        rows[owner] += 1;
+                        for (int i = cp[c] + k * spw; i < std::min(cp[c] + (k + 1) * spw, cp[c + 1]); ++i)
+                            ids[owner] += static_cast<int>(dg[i] & 0xffffu);
+                    }
+                    nu0[b] += k1 - k0;
                 }
+            }
             k_cap = std::max(k_cap, *std::max_element(rows.begin(), rows.end()));
             id_cap = std::max(id_cap, *std::max_element(ids.begin(), ids.end()));
         }

@@ -12,11 +12,12 @@
 // and a small sample fits the shared memory of a few SMs.  So a cluster of C CTAs (C <= 8) owns a sample for the whole
 // launch:
 //
-//   * rows (32/G consecutive sites of one class x G lanes x 2 slots) are dealt round-robin to the C * kCycleWarps warps of
-//     the cluster, class after class, so every class and every warp's total is balanced to within one row;
+//   * every CTA owns a contiguous C-th of the rows (32/G consecutive sites x G lanes x 2 slots) of EVERY colour class --
+//     the same region of the lattice in every class, so most neighbours are in the CTA's own shared memory -- and deals
+//     them round-robin to its warps, class after class: every class and every warp's total is balanced to within a row;
 //   * at launch a warp copies, once, what its rows need into its slice of shared memory: the rows' angles, one descriptor
 //     per site, and for every neighbour WHERE ITS ANGLE LIVES: the rank of the owner's CTA and the offset in its shared
-//     memory (row rho belongs to warp rho mod nw, slot rho div nw -- a closed form, no table);
+//     memory (closed forms, no table);
 //   * a colour class is then: cluster wait -> gather the neighbours' angles from the owners' shared memory
 //     (mapa + ld.shared::cluster: ~200 cycles instead of an L2 round trip) -> update -> write the new angle to the warp's
 //     OWN shared memory -> cluster arrive.  No global memory access at all between two swap rounds: the measured sums of
@@ -49,10 +50,14 @@ struct CycleArgs {
 };
 
 // one warp's slice of shared memory: its rows' angles [k_cap][32] float2, site descriptors [k_cap][32 / G] int2 and
-// neighbour descriptors [id_cap] uint32 (owner's CTA rank << 24 | byte offset of the neighbour's row in a CTA's dynamic
-// shared memory)
+// neighbour descriptors [id_cap] uint32 (the shared::cluster address of the neighbour's angles, slot pair 0)
 __host__ __device__ constexpr size_t cycle_pool_bytes(int G, int k_cap, int id_cap) {
     return (static_cast<size_t>(k_cap) * (256 + (32 / G) * 8) + static_cast<size_t>(id_cap) * 4 + 15) / 16 * 16;
+}
+
+// first row of a class of n_rows rows that CTA b of n_cta owns: ceil(b n_rows / n_cta) (host and device)
+__host__ __device__ constexpr int cycle_first_row(int b, int n_rows, int n_cta) {
+    return static_cast<int>((static_cast<long long>(b) * n_rows + n_cta - 1) / n_cta);
 }
 
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
@@ -74,9 +79,11 @@ __device__ __forceinline__ uint32_t cluster_map(uint32_t local_addr, uint32_t ra
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(local_addr), "r"(rank));
     return ra;
 }
-__device__ __forceinline__ float2 ld_cluster_f2(uint32_t local_addr, uint32_t rank) {
+// a neighbour's angles by shared::cluster address (mapped once, at launch; an address of the CTA's own shared-memory
+// window is a valid shared::cluster address of this CTA)
+__device__ __forceinline__ float2 ldc_f2(uint32_t cluster_addr) {
     float2 v;
-    asm volatile("ld.shared::cluster.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(cluster_map(local_addr, rank)) : "memory");
+    asm volatile("ld.shared::cluster.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(cluster_addr) : "memory");
     return v;
 }
 __device__ __forceinline__ unsigned long long ld_cluster_u64(uint32_t local_addr, uint32_t rank) {
@@ -90,8 +97,8 @@ struct CycleCtx {
     float2 *lb;                 // this lane's column of the sample in global memory: theta2 + s*N*G + q (load and write-back)
     float2 *own;                // this lane's column of the warp's resident rows: [k_cap], stride 32
     const int2 *meta;           // the warp's site descriptors [k_cap][SPW] {site or -1, first id | degree << 16 | n_lower << 24}
-    const uint32_t *ids;        // the warp's neighbour descriptors
-    uint32_t dyn_q;             // shared-space address of the CTA's dynamic shared memory + 8 q: base of a neighbour's offset
+    const uint32_t *ids;        // the warp's neighbour descriptors: shared::cluster address of the neighbour's angles, slot pair 0
+    uint32_t q8;                // 8 q: the lane's slot pair inside a site's 8 G bytes
     unsigned long long *sacc;   // the CTA's measured sums of the sweep being tallied [G][6]
     int s, lane, sub, q;
 };
@@ -111,10 +118,7 @@ __device__ __forceinline__ void cycle_row(const TileArgs &a, const CycleCtx &x, 
     const int deg = valid ? (m.y >> 16) & 0xff : 0, nlow = valid ? static_cast<int>(static_cast<uint32_t>(m.y) >> 24) : 0;
     const int dmax = UNI ? deg : static_cast<int>(__reduce_max_sync(kFull, static_cast<unsigned>(deg)));
     const float2 own = x.own[j * 32];
-    auto neighbour = [&](int k) {
-        const uint32_t d = x.ids[pos + k];
-        return ld_cluster_f2(x.dyn_q + (d & 0xffffffu), d >> 24);
-    };
+    auto neighbour = [&](int k) { return ldc_f2(x.ids[pos + k] + x.q8); };
     // the gathers first (the only remote reads of the row): up to kDB neighbours in registers
     float2 v[kDB];
 #pragma unroll
@@ -242,7 +246,8 @@ __global__ void __launch_bounds__(kCycleWarps * 32, 512 / (kCycleWarps * 32)) k_
     constexpr int SPW = 32 / G;
     extern __shared__ __align__(16) unsigned char s_raw[];
     __shared__ unsigned short s_jb[W][kCycleMaxQ + 1];      // per warp: first resident row of every colour class
-    __shared__ int s_cp[kCycleMaxQ + 1], s_rb[kCycleMaxQ + 1];   // first site and first row of every colour class
+    __shared__ int s_cp[kCycleMaxQ + 1];                       // first site of every colour class
+    __shared__ int s_rb[kCycleMaxQ + 1][kCycleMaxCtas];        // rows of the classes before c owned by CTA b
     __shared__ unsigned long long s_acc[2][G][6];            // the CTA's running measured sums (exact integers), two buffers
     __shared__ CycleLeader s_ld;                             // used by the leader CTA only
     const TileArgs &t = a.t;
@@ -261,23 +266,30 @@ __global__ void __launch_bounds__(kCycleWarps * 32, 512 / (kCycleWarps * 32)) k_
     uint32_t *ids = reinterpret_cast<uint32_t *>(pool + static_cast<size_t>(a.k_cap) * (256 + SPW * 8));
     x.meta = meta;
     x.ids = ids;
-    x.dyn_q = static_cast<uint32_t>(__cvta_generic_to_shared(s_raw)) + static_cast<uint32_t>(x.q) * 8u;
+    x.q8 = static_cast<uint32_t>(x.q) * 8u;
+    const uint32_t dyn_base = static_cast<uint32_t>(__cvta_generic_to_shared(s_raw));
     x.sacc = &s_acc[0][0][0];
     const uint32_t sacc_addr = static_cast<uint32_t>(__cvta_generic_to_shared(&s_acc[0][0][0]));
     const int n_cta = gridDim.x;
     const bool leader = blockIdx.x == 0;                 // cluster dims (C, 1, 1), grid (C, samples): rank = blockIdx.x
-    const int nw = n_cta * W, gw = blockIdx.x * W + warp;     // nw is a power of two (C in {1, 2, 4, 8, 16})
-    const int nw_shift = __ffs(nw) - 1;
 
-    // ---- once per launch: the sample moves into the cluster's shared memory.  Rows are numbered class after class; row
-    // rho belongs to warp rho mod nw and is that warp's row number rho div nw. ----
+    // ---- once per launch: the sample moves into the cluster's shared memory.  CTA b owns rows [ceil(b n_c / C),
+    // ceil((b+1) n_c / C)) of every colour class c (n_c rows): the sites of a class keep their lattice order (colour-major
+    // numbering), so a CTA holds the same REGION of the lattice in every class and most neighbours of its sites are in
+    // its own shared memory.  Inside the CTA its rows, numbered class after class (nu), go to warp nu mod W as that
+    // warp's row nu div W -- closed forms, so a neighbour's location needs no table. ----
     if (threadIdx.x == 0) {
         const int32_t *cp = t.class_ptr + x.s * t.q_stride;
-        int rb = 0;
-        for (int c = 0; c <= a.q_max; ++c) {
-            s_cp[c] = cp[c];
-            s_rb[c] = rb;
-            if (c < a.q_max) rb += (cp[c + 1] - cp[c] + SPW - 1) / SPW;
+        for (int c = 0; c <= a.q_max; ++c) s_cp[c] = cp[c];
+        for (int b = 0; b < n_cta; ++b) {
+            int before = 0;
+            for (int c = 0; c <= a.q_max; ++c) {
+                s_rb[c][b] = before;                     // rows of the classes < c that CTA b owns
+                if (c < a.q_max) {
+                    const int n_rows = (cp[c + 1] - cp[c] + SPW - 1) / SPW;
+                    before += cycle_first_row(b + 1, n_rows, n_cta) - cycle_first_row(b, n_rows, n_cta);
+                }
+            }
         }
     }
     for (int e = threadIdx.x; e < 2 * G * 6; e += blockDim.x) (&s_acc[0][0][0])[e] = 0ull;
@@ -294,10 +306,10 @@ __global__ void __launch_bounds__(kCycleWarps * 32, 512 / (kCycleWarps * 32)) k_
         for (int c = 0; c < a.q_max; ++c) {
             if (x.lane == 0) s_jb[warp][c] = static_cast<unsigned short>(j);
             const int cbeg = s_cp[c], cend = s_cp[c + 1];
-            const int n_rows = s_rb[c + 1] - s_rb[c];
-            int k = (gw - (s_rb[c] & (nw - 1)) + nw) & (nw - 1);
-            for (; k < n_rows; k += nw, ++j) {
-                const int i = cbeg + k * SPW + x.sub;
+            const int n_rows = (cend - cbeg + SPW - 1) / SPW;
+            const int k_first = cycle_first_row(blockIdx.x, n_rows, n_cta), mine = cycle_first_row(blockIdx.x + 1, n_rows, n_cta) - k_first;
+            for (int kk = (warp - s_rb[c][blockIdx.x] % W + W) % W; kk < mine; kk += W, ++j) {
+                const int i = cbeg + (k_first + kk) * SPW + x.sub;
                 const bool valid = i < cend;
                 int2 rc = make_int2(0, 0);
                 if (valid) rc = rec[i];
@@ -314,10 +326,12 @@ __global__ void __launch_bounds__(kCycleWarps * 32, 512 / (kCycleWarps * 32)) k_
                     const int n = t.col_idx[rc.x + e];
                     int cn = 0;
                     while (cn + 1 < a.q_max && n >= s_cp[cn + 1]) ++cn;
-                    const int rho = s_rb[cn] + (n - s_cp[cn]) / SPW, sbn = (n - s_cp[cn]) % SPW;
-                    const int gwn = rho & (nw - 1), jn = rho >> nw_shift;
-                    const uint32_t off = static_cast<uint32_t>((gwn % W) * pool_bytes) + static_cast<uint32_t>(jn * 256 + sbn * G * 8);
-                    ids[pos + e] = (static_cast<uint32_t>(gwn / W) << 24) | off;
+                    const int kn = (n - s_cp[cn]) / SPW, sbn = (n - s_cp[cn]) % SPW;
+                    const int nr = (s_cp[cn + 1] - s_cp[cn] + SPW - 1) / SPW;
+                    const int bn = static_cast<int>(static_cast<long long>(kn) * n_cta / nr);      // the CTA whose range holds row kn
+                    const int nu = s_rb[cn][bn] + kn - cycle_first_row(bn, nr, n_cta);
+                    const uint32_t off = static_cast<uint32_t>((nu % W) * pool_bytes) + static_cast<uint32_t>((nu / W) * 256 + sbn * G * 8);
+                    ids[pos + e] = bn == static_cast<int>(blockIdx.x) ? dyn_base + off : cluster_map(dyn_base + off, static_cast<uint32_t>(bn));
                 }
                 if (x.q == 0) meta[j * SPW + x.sub] = make_int2(valid ? i : -1, pos | (deg << 16) | (nlow << 24));
                 x.own[j * 32] = valid ? x.lb[static_cast<unsigned long long>(static_cast<uint32_t>(i) * static_cast<uint32_t>(G))]

@@ -8,8 +8,9 @@ namespace xy {
 constexpr int kCycleWarps = 8;       // warps per CTA of k_cycle: 256 threads x 128 registers (no spills, all gathers of a row in
                                      // flight), two CTAs per SM.  Measured: 16 warps x 64 registers (134 B of spills, twice the warps
                                      // per sample) gives the same throughput
+constexpr int kCycleMaxCtas = 16;    // largest cluster of k_cycle (the non-portable size)
 constexpr int kCycleMaxQ = 12;       // most colours a sample may have on the cluster path
-constexpr int kCycleAutoRows = 20;   // automatic path choice: cluster path while a warp owns at most this many rows
+constexpr int kCycleAutoRows = 36;   // automatic path choice: cluster path while a warp owns at most this many rows
 
 // k_phase<G, CB, MODE, W> for W in {8, 32} (MODE 0..5) and W = 24 (MODE 3, 5 only); CB = single_block ? 1 : 0 (G = 32 only).
 // nullptr for a combination that is not built.
