@@ -19,7 +19,7 @@ def levy_coords(g):
     return (g.new_to_old % g.L).astype(np.int32), (g.new_to_old // g.L).astype(np.int32)
 
 
-@pytest.mark.parametrize("L,R,S", [(16, 8, 2), (16, 64, 2), (24, 32, 1), (12, 3, 2), (20, 128, 1), (33, 16, 1)])
+@pytest.mark.parametrize("L,R,S", [(16, 8, 2), (16, 64, 2), (24, 32, 1), (12, 3, 2), (20, 128, 1), (33, 16, 1), (16, 2, 2), (40, 4, 1)])
 def test_fourier_matches_oracle(L, R, S):
     g = levy.build(L, 3.5, 6, workloads.BASE_SEED, S=S)
     T = O.geometric_temperatures(R, 1.0, 4.0)
@@ -49,6 +49,36 @@ def test_fourier_matches_oracle(L, R, S):
     with pytest.raises(B.XYError):
         ens.set_coords(L, L, x + L, y)                        # out of range
     ens.close()
+
+
+@pytest.mark.parametrize("L,R", [(24, 8), (40, 32), (24, 64), (20, 128), (33, 16)])
+def test_fourier_bulk_copy_and_cp_async_flavours_give_the_same_bits(L, R):
+    """k_fourier2 fills its ring with the TMA engine (cp.async.bulk) when theta is 16-byte aligned and with per-lane
+    cp.async copies otherwise: the same rows in the same order, so G1, G2 must be bit-identical -- and equal the oracle's."""
+    import torch
+    g = levy.build(L, 3.5, 6, workloads.BASE_SEED, S=2)
+    T = O.geometric_temperatures(R, 1.0, 4.0)
+    x, y = levy_coords(g)
+    S, N = g.colour.shape
+    rng = np.random.default_rng(L * 1000 + R)
+    th = (rng.random((S, N, R)) * 6.28).astype(np.float32)
+    outs = []
+    for shift in (0, 2):                                     # floats: 0 = 16-byte aligned (bulk copies), 2 = 8 mod 16 (cp.async)
+        stream = torch.cuda.Stream()
+        buf = torch.empty(S * N * R + 4, dtype=torch.float32, device="cuda:0")
+        ptr = buf.data_ptr() + 4 * shift
+        assert buf.data_ptr() % 16 == 0
+        graph = B.xy_graph_load(g.row_ptr, g.col_idx, g.colour, stream.cuda_stream)
+        pt = B.xy_pt_create(graph, T, SEED, None, 0, ptr, stream.cuda_stream)
+        B.xy_graph_set_coords(graph, L, L, x, y)
+        B.xy_set_theta(pt, th)
+        outs.append(B.xy_measure_fourier(pt, (S, R)))
+        B.xy_pt_destroy(pt)
+        B.xy_graph_free(graph)
+    assert np.array_equal(outs[0], outs[1])
+    for s in range(S):
+        G1, G2 = O.fourier(L, L, x[s], y[s], th[s])
+        assert np.all(np.abs(outs[0][s, :, 0] - G1) <= 2e-5 * (1.0 + G1)) and np.all(np.abs(outs[0][s, :, 1] - G2) <= 2e-5 * (1.0 + G2))
 
 
 def test_fourier_closed_form_configurations_on_gpu():
