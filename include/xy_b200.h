@@ -100,6 +100,13 @@ int xy_pt_destroy(xy_pt *pt);
 /* ---- the hot-path calls named by BASELINE.json north_star ---- */
 /* n Metropolis sweeps: colours 0..Q-1 in order, sweep counter += 1 per sweep. */
 int xy_sweep(xy_pt *pt, int n_sweeps);
+/* One Metropolis sweep exactly as xy_sweep(pt, 1), which also reports the ACCEPTANCE RATE of the proposals per temperature
+ * (SURVEY.md section 5 metrics; the rate the proposal width 2 pi min(1, T/2) of BASELINE.json is meant to keep usable):
+ * acc_host[s][t] (host, [S][R] doubles, indexed by temperature) = sites of sample s whose angle in the slot of
+ * temperature t changed / N.  An accepted proposal always changes the stored angle except when |delta| is below half an
+ * ulp of the angle (probability ~1e-7 per update).  Costs one device copy of theta (scratch memory of theta's size,
+ * freed before returning) and one comparison pass; synchronises the stream. */
+int xy_sweep_acceptance(xy_pt *pt, double *acc_host);
 /* n over-relaxation sweeps (ref 66): no randoms, counters untouched. */
 int xy_overrelax(xy_pt *pt, int n_sweeps);
 /* one swap round (ref 65): pairs (t,t+1), t = round mod 2 (mod 2); energies are

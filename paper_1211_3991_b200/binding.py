@@ -35,6 +35,7 @@ SYMBOLS = {
                                C.c_void_p, C.POINTER(C.c_void_p)]),
     "xy_pt_destroy": (C.c_int, [C.c_void_p]),
     "xy_sweep": (C.c_int, [C.c_void_p, C.c_int]),
+    "xy_sweep_acceptance": (C.c_int, [C.c_void_p, C.c_void_p]),
     "xy_overrelax": (C.c_int, [C.c_void_p, C.c_int]),
     "xy_pt_swap": (C.c_int, [C.c_void_p]),
     "xy_measure": (C.c_int, [C.c_void_p, C.c_void_p]),
@@ -201,6 +202,13 @@ def xy_pt_destroy(pt):
 
 def xy_sweep(pt, n_sweeps=1):
     _check(lib().xy_sweep(pt, n_sweeps))
+
+
+def xy_sweep_acceptance(pt, shape):
+    """one Metropolis sweep + the fraction of accepted proposals [S][R] by temperature; shape = (S, R)"""
+    out = np.zeros(shape, np.float64)
+    _check(lib().xy_sweep_acceptance(pt, out.ctypes.data_as(C.c_void_p)))
+    return out
 
 
 def xy_overrelax(pt, n_sweeps=1):
@@ -377,6 +385,7 @@ class Ensemble:
 
     # forwarding
     def sweep(self, n=1): xy_sweep(self.pt, n)
+    def sweep_acceptance(self): return xy_sweep_acceptance(self.pt, (self.S, self.R))
     def overrelax(self, n=1): xy_overrelax(self.pt, n)
     def pt_swap(self): xy_pt_swap(self.pt)
     def measure(self, want=False): return xy_measure(self.pt, (self.S, self.R) if want else None)

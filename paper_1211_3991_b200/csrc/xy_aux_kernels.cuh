@@ -501,6 +501,23 @@ __global__ void __launch_bounds__(kBlock) k_random_walk(const WalkArgs a) {
         if (s_hist[t]) atomicAdd(a.hist + static_cast<size_t>(s) * (a.n_steps + 1) + t, static_cast<unsigned long long>(s_hist[t]));
 }
 
+// ---- acceptance of a Metropolis sweep: angles that differ from the copy taken before it, per (sample, slot) ----
+// grid (chunks of sites, samples); a thread owns the slots r = threadIdx.x, + blockDim.x, ... (coalesced rows)
+__global__ void __launch_bounds__(kBlock) k_count_changed(const float *before, const float *after, unsigned long long *count,
+                                                          int N, int R, int sites_per_block) {
+    const int s = blockIdx.y;
+    const int i0 = blockIdx.x * sites_per_block, i1 = min(N, i0 + sites_per_block);
+    const size_t base = static_cast<size_t>(s) * N * R;
+    for (int r = threadIdx.x; r < R; r += blockDim.x) {
+        unsigned int c = 0;
+        for (int i = i0; i < i1; ++i) {
+            const size_t k = base + static_cast<size_t>(i) * R + r;
+            c += __float_as_uint(before[k]) != __float_as_uint(after[k]) ? 1u : 0u;
+        }
+        if (c) atomicAdd(count + static_cast<size_t>(s) * R + r, static_cast<unsigned long long>(c));
+    }
+}
+
 // ---- init: theta = 2 pi_f * u, Philox domain 0, sweep 0 ------------------------------------------------
 __global__ void k_init_theta(float *theta, int S, int N, int R, PhiloxKeys keys, uint32_t sample_base) {
     const size_t total = static_cast<size_t>(S) * N * R;

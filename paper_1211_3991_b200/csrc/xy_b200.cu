@@ -1132,6 +1132,46 @@ int xy_sweep(xy_pt *pt, int n_sweeps) {
     return XY_OK;
 }
 
+int xy_sweep_acceptance(xy_pt *pt, double *acc_host) {
+    if (!check_pt(pt) || !acc_host) return fail(XY_EINVAL, "bad handle or NULL output");
+    DeviceGuard guard(pt->g->device);
+    { const int rc_up = settle_upload(pt); if (rc_up != XY_OK) return rc_up; }
+    const int S = pt->g->S, N = pt->g->N, R = pt->R;
+    const size_t n = static_cast<size_t>(S) * N * R, SR = static_cast<size_t>(S) * R;
+    float *before = nullptr;
+    unsigned long long *count = nullptr;
+    int rc;
+    if ((rc = dev_alloc(&before, n)) != XY_OK) return rc;
+    if ((rc = dev_alloc(&count, SR)) != XY_OK) { cudaFree(before); return rc; }
+    cudaError_t e = cudaMemcpyAsync(before, pt->theta, n * sizeof(float), cudaMemcpyDeviceToDevice, pt->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(count, 0, SR * sizeof(unsigned long long), pt->stream);
+    rc = e == cudaSuccess ? xy_sweep(pt, 1) : fail(XY_ECUDA, std::string("xy_sweep_acceptance: ") + cudaGetErrorString(e));
+    if (rc == XY_OK) {
+        const int spb = std::max(1, ceil_div(N, std::max(1, pt->g->n_sm * 8 / S)));
+        xy::k_count_changed<<<dim3(ceil_div(N, spb), S), xy::kBlock, 0, pt->stream>>>(before, pt->theta, count, N, R, spb);
+        pt->launches += 1;
+        try {
+            std::vector<unsigned long long> h(SR);
+            std::vector<int32_t> tos(SR);
+            e = cudaGetLastError();
+            if (e == cudaSuccess) e = cudaMemcpyAsync(h.data(), count, SR * sizeof(unsigned long long), cudaMemcpyDeviceToHost, pt->stream);
+            if (e == cudaSuccess) e = cudaMemcpyAsync(tos.data(), pt->temp_of_slot, SR * sizeof(int32_t), cudaMemcpyDeviceToHost, pt->stream);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(pt->stream);
+            if (e != cudaSuccess) rc = fail(XY_ECUDA, std::string("xy_sweep_acceptance: ") + cudaGetErrorString(e));
+            else
+                for (int s = 0; s < S; ++s)
+                    for (int r = 0; r < R; ++r)
+                        acc_host[static_cast<size_t>(s) * R + tos[static_cast<size_t>(s) * R + r]] =
+                            static_cast<double>(h[static_cast<size_t>(s) * R + r]) / N;
+        } catch (const std::bad_alloc &) {
+            rc = fail(XY_ENOMEM, "host allocation failed");
+        }
+    }
+    cudaStreamSynchronize(pt->stream);
+    cudaFree(before); cudaFree(count);
+    return rc;
+}
+
 int xy_overrelax(xy_pt *pt, int n_sweeps) {
     if (!check_pt(pt) || n_sweeps < 0) return fail(XY_EINVAL, "bad handle or n_sweeps < 0");
     DeviceGuard guard(pt->g->device);

@@ -524,3 +524,41 @@ def test_run_of_hub_sites_does_not_overflow_the_fixed_point_partial_sums():
         assert np.array_equal(ens.get_energy(), want), order
         assert not ens.get_theta().any()
     ens.close()
+
+
+@pytest.mark.parametrize("L,R,S", [(16, 8, 2), (12, 64, 1), (12, 6, 2)])
+def test_sweep_acceptance_per_temperature_matches_the_oracle(L, R, S):
+    """xy_sweep_acceptance = one Metropolis sweep (the same bits as xy_sweep) + the fraction of accepted proposals per
+    temperature (SURVEY.md section 5 metrics): against the oracle's accepted flags of the same sweep, up to the
+    near-threshold decisions (R6)."""
+    g = small_levy(L, 3.5, S)
+    T = O.geometric_temperatures(R, 1.0, 4.0)
+    a = U.ensemble_from_levy(g, T, SEED)
+    b = U.ensemble_from_levy(g, T, SEED)
+    rng = np.random.default_rng(11)
+    lab = np.stack([rng.permutation(R).astype(np.int32) for _ in range(S)])
+    a.set_labels(lab); b.set_labels(lab)
+    a.run_sweeps(1, 3, 1); b.run_sweeps(1, 3, 1)             # away from the uniform start
+    pre = a.get_theta()
+    acc = a.sweep_acceptance()
+    b.sweep(1)
+    assert np.array_equal(a.get_theta(), b.get_theta()) and a.get_counters()[0] == b.get_counters()[0] == 4
+    graphs = U.graphs_of_levy(g)
+    N = L * L
+    for s in range(S):
+        rp, ci, cp = graphs[s]
+        ref = pre[s].copy()
+        bs, ws = U.slot_params(T, lab[s])
+        n_acc, n_near = np.zeros(R), 0
+        for c in range(len(cp) - 1):
+            sites = np.arange(cp[c], cp[c + 1], dtype=np.int32)
+            if len(sites) == 0:
+                continue
+            margin, accepted = O.metropolis_sites(rp, ci, ref, sites, bs, ws, SEED, 4, s, want_margin=True)
+            n_acc += accepted.sum(0)
+            n_near += int((margin < 1e-5).sum())
+        by_temp = np.zeros(R)
+        by_temp[lab[s]] = n_acc / N
+        assert np.all(np.abs(acc[s] - by_temp) <= (n_near + 1) / N), (acc[s], by_temp)
+        assert 0.1 < acc[s].min() and acc[s].max() < 1.0 and acc[s][-1] > acc[s][0]     # hotter replicas accept more
+    a.close(); b.close()
