@@ -27,7 +27,8 @@ def same_state(a, b, what):
 
 
 @pytest.mark.parametrize("L,rho,R,S", [(16, 3.5, 8, 1), (24, 2.5, 16, 5), (16, 4.5, 32, 3), (12, 3.0, 2, 2), (12, 3.0, 4, 40),
-                                        (20, 3.5, 64, 2), (32, 2.5, 16, 32)])
+                                        (20, 3.5, 64, 2), (32, 2.5, 16, 32), (8, 3.0, 4, 320)])      # the last one: more samples than
+                                        # resident clusters of any size (the clusters run in waves)
 @pytest.mark.parametrize("order", [0, 1])
 def test_cluster_path_is_bit_identical_to_the_launch_path(L, rho, R, S, order):
     g = levy.build(L, rho, 6, workloads.BASE_SEED, S=S, sample_base=3)
