@@ -27,6 +27,9 @@ def main(argv=None):
     ap.add_argument("--seed", type=lambda v: int(v, 0), default=0xB200_1211_3991)
     ap.add_argument("--colouring", default="reduced", choices=["reduced", "smallest-last"],
                     help="reduced = smallest-last followed by the builder's colour-reducing local search (bench.py's default)")
+    ap.add_argument("--no-pdl", action="store_true", help="xy_set_tuning: no programmatic-dependent-launch edges")
+    ap.add_argument("--no-l2-window", action="store_true", help="xy_set_tuning: no persisting-L2 access window")
+    ap.add_argument("--no-balance", action="store_true", help="xy_set_tuning: equal shares instead of cost-balanced ones")
     a = ap.parse_args(argv)
 
     import torch
@@ -53,6 +56,8 @@ def main(argv=None):
     ens.set_path(a.path)
     if a.samples_per_group:
         ens.set_schedule(a.samples_per_group)
+    if a.no_pdl or a.no_l2_window or a.no_balance:
+        ens.set_tuning(balance=0 if a.no_balance else 1, pdl=0 if a.no_pdl else 1, l2_persist=0 if a.no_l2_window else 1)
     sps, orps = w.sweeps_per_swap, w.or_per_sweep
 
     def run(n):
