@@ -305,6 +305,12 @@ def main():
                 "traffic_note": "dram__bytes per launch: profiles/ (ncu --set full at the benched commit); not read at run time",
                 "bytes_per_update": bpu, **{kk: k[kk] for kk in ("updates_per_launch_avg", "avg_launch_us", "launches_timed",
                                                                   "met_or_updates_per_ns")}}
+    roofline["path"] = ens.path_name(orps)
+    if ens.get_path(orps)[0] == 2:
+        roofline["kernel"] = "k_cycle<G,ORDER> (cluster path: whole cycles per launch)"
+        roofline["schedule"] = ("cluster path: every sample stays in the distributed shared memory of its thread-block cluster for the "
+                                "whole launch; neither L2 nor HBM carries the gathers, the bound is the latency chain of a colour "
+                                "class (DESIGN.md 7.2) -- frac is the algorithmic bytes against the L2 bandwidth, for reference only")
 
     # ---- the genuinely streaming schedule: one launch per colour class over ALL samples (every sweep re-reads the whole
     #      state from HBM) -- the number "fraction of the HBM roofline" is literally about ----
