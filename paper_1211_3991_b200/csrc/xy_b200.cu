@@ -99,7 +99,7 @@ struct DeviceGuard {
 namespace xy {
 
 const void *phase_function(int W, int G, bool single_block, int mode) {
-    if (W == 24) return phase_function_w24(G, single_block, mode);
+    if (W == 24 || W == 28) return phase_function_w24(G, single_block, mode);      // the measuring modes' own CTA shapes
     if (W == kWarpsSmall) return mode < 3 ? phase_function_w8_a(G, single_block, mode) : phase_function_w8_b(G, single_block, mode);
     if (W == kWarpsBig) return mode < 3 ? phase_function_w32_a(G, single_block, mode) : phase_function_w32_b(G, single_block, mode);
     return nullptr;
@@ -166,7 +166,7 @@ struct xy_pt {
     int balance = 1;                 // cost-balanced share tables (1) or equal shares (0)
     int pdl = 1;                     // programmatic dependent launch edges between the k_phase launches
     const void *phase_fn[2][6] = {};   // k_phase<G, CB, MODE, W>: [0] W = 8 warps per CTA, [1] W = 32
-    const void *phase_fn24[2] = {nullptr, nullptr};   // measuring modes 3, 5 with 24-warp CTAs (85 registers: no spills)
+    const void *phase_fn24[2] = {nullptr, nullptr};   // measuring modes 3 (28-warp CTAs, 72 registers) and 5 (24-warp CTAs, 80): no spills
     int order = 0;                   // 0 = Metropolis sweep then OR sweep, 1 = interleaved by colour (xy_set_order)
     int capacity_big = 0;            // co-resident 32-warp CTAs (one per SM)
     int cta_shape = 0;               // 0 = by class size, 1 = always 8-warp CTAs, 2 = always 32-warp CTAs
@@ -281,9 +281,10 @@ int get_partition(xy_pt *pt, int nw, const int4 **out) {
 // CTA shape and CTAs per (sample, column block) for a launch over a group of ns samples whose largest class has nmax
 // sites: one wave of resident CTAs shared by the group, at most one row per warp.  The shape is chosen per group from
 // the whole sweep (all launches of a group alike): 32-warp CTAs when a warp gets at least 32 rows per sweep.
-// The measuring modes (3, 5) carry the fixed-point partial sums on top of the update's state: with 24-warp CTAs
-// (768 threads, 80 registers) they do not spill, which outweighs the lost quarter of the warps (measured: +25 % on the
-// interleaved cycle of config 4, +2 % on the default one).
+// The measuring modes (3, 5) carry the fixed-point partial sums on top of the update's state and spill at 64 registers:
+// MODE 3 (over-relaxation + measurement) runs 28-warp CTAs (896 threads, 72 registers, no spills), MODE 5 (interleaved +
+// measurement) 24-warp CTAs (768 threads, 80 registers; at 72 it spills ~100 bytes).  Measured on config 4: 24 instead of
+// 32 warps +25 % on the interleaved cycle and +6 % on the default one; 28 instead of 24 for MODE 3 another +2 %.
 struct SweepGrid { int big, gx, warps; };
 SweepGrid sweep_grid(const xy_pt *pt, int ns, int nmax, int mode) {
     const int spw = 32 / pt->fast_G;
@@ -291,7 +292,7 @@ SweepGrid sweep_grid(const xy_pt *pt, int ns, int nmax, int mode) {
     SweepGrid g;
     g.big = pt->cta_shape == 2 || (pt->cta_shape == 0 && rows >= 32ll * xy::kWarpsBig * pt->capacity_big);
     if (g.big && pt->capacity_big < ns * pt->col_blocks) g.big = 0;
-    g.warps = g.big ? ((mode == 3 || mode == 5) ? 24 : xy::kWarpsBig) : xy::kWarpsSmall;
+    g.warps = g.big ? (mode == 3 ? 28 : mode == 5 ? 24 : xy::kWarpsBig) : xy::kWarpsSmall;
     const int cap = g.big ? pt->capacity_big : pt->sweep_capacity;
     g.gx = std::max(1, std::min(ceil_div(nmax, g.warps * spw), cap / (ns * pt->col_blocks)));
     return g;
@@ -332,7 +333,7 @@ int launch_phase(xy_pt *pt, int mode, int colour, int s0, int s1, bool use_count
     a.t.sweep_fixed = sweep_fixed; a.t.sweep_offset = sweep_offset; a.t.use_counter = use_counter ? 1 : 0;
     a.t.accumulate = accumulate;
     const SweepGrid sg = sweep_grid(pt, s1 - s0, nmax, mode);
-    const void *fn = sg.warps == 24 ? pt->phase_fn24[mode == 5] : pt->phase_fn[sg.big][mode];
+    const void *fn = (sg.warps == 24 || sg.warps == 28) ? pt->phase_fn24[mode == 5] : pt->phase_fn[sg.big][mode];
     if (pt->balance) {
         const int rc = get_partition(pt, sg.gx * sg.warps, &a.part);
         if (rc != XY_OK) return rc;
@@ -651,8 +652,8 @@ int prepare_partitions(xy_pt *pt, int group) {
             const int nmax = c == g->q_max ? g->N : max_class_size(g, c, s0, s1);
             if (nmax == 0) continue;
             const int4 *unused = nullptr;
-            for (int mode : {0, 3}) {      // the update shapes and the measuring shape
-                if (c == g->q_max && mode == 3) continue;
+            for (int mode : {0, 3, 5}) {      // the update shapes and the two measuring shapes
+                if (c == g->q_max && mode != 0) continue;
                 const SweepGrid sg = sweep_grid(pt, s1 - s0, nmax, c == g->q_max ? 2 : mode);
                 const int rc = get_partition(pt, sg.gx * sg.warps, &unused);
                 if (rc != XY_OK) return rc;
@@ -984,9 +985,9 @@ int xy_pt_create(const xy_graph *g, int R, const double *T, const double *width,
             prepare(pt->phase_fn[1][m], xy::kWarpsBig);
         }
         // 32 resident warps x 5.5 KB of shared memory per SM in either CTA shape (carve-out set above)
-        pt->phase_fn24[0] = xy::phase_function(24, pt->fast_G, pt->col_blocks == 1, 3);
+        pt->phase_fn24[0] = xy::phase_function(28, pt->fast_G, pt->col_blocks == 1, 3);
         pt->phase_fn24[1] = xy::phase_function(24, pt->fast_G, pt->col_blocks == 1, 5);
-        prepare(pt->phase_fn24[0], 24);
+        prepare(pt->phase_fn24[0], 28);
         prepare(pt->phase_fn24[1], 24);
         int per_sm = 0, per_sm_big = 0;
         const int n_sm = g->n_sm, dev = g->device;

@@ -12,7 +12,7 @@ constexpr int kCycleMaxCtas = 16;    // largest cluster of k_cycle (the non-port
 constexpr int kCycleMaxQ = 12;       // most colours a sample may have on the cluster path
 constexpr int kCycleAutoRows = 36;   // automatic path choice: cluster path while a warp owns at most this many rows
 
-// k_phase<G, CB, MODE, W> for W in {8, 32} (MODE 0..5) and W = 24 (MODE 3, 5 only); CB = single_block ? 1 : 0 (G = 32 only).
+// k_phase<G, CB, MODE, W> for W in {8, 32} (MODE 0..5), W = 28 (MODE 3) and W = 24 (MODE 5); CB = single_block ? 1 : 0 (G = 32 only).
 // nullptr for a combination that is not built.
 const void *phase_function(int W, int G, bool single_block, int mode);
 // k_cycle<G, ORDER>

@@ -11,7 +11,8 @@
 // sites share no bond, so the gathers of row t+1 never read what row t stores: they are issued BEFORE
 // row t is computed, as cp.async (LDGSTS) copies of the lane's own 8 bytes into a per-warp ring in shared memory --
 // in-flight data costs no registers (64 per thread and 32 warps per SM for the update modes, without spills; 80
-// registers and 24 warps for the modes that also measure), each lane reads back only what it copied itself
+// registers and 24 warps for the interleaved mode that also measures, 72 registers and 28 warps for the over-relaxation
+// that also measures), each lane reads back only what it copied itself
 // (cp.async.wait_group, no cross-lane synchronisation), and the Philox / sin / exp work of row t covers the latency
 // of row t+1.  When SPW > 1 the sites of a row have different degrees: the loops run to the row maximum and lanes
 // whose site has fewer neighbours are predicated off (no memory request is made for them).
@@ -617,7 +618,7 @@ __device__ __forceinline__ void sweep_reduce_to_fx(const TileArgs &a, const Swee
 // gather, without / with the measurement by-product.
 
 template <int G, int CB, int MODE, int W>
-__global__ void __launch_bounds__(W * 32, W == 24 ? 1 : kSmPerWarpSlots / W) k_phase(const SweepArgs a) {
+__global__ void __launch_bounds__(W * 32, (W == 24 || W == 28) ? 1 : kSmPerWarpSlots / W) k_phase(const SweepArgs a) {
     extern __shared__ __align__(16) unsigned char s_raw[];
     SweepWarp *s_w = reinterpret_cast<SweepWarp *>(s_raw);
     __shared__ int s_last;
