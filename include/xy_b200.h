@@ -81,6 +81,19 @@ int xy_graph_set_coords(xy_graph *g, int Lx, int Ly, const int32_t *x /*host*/, 
 int xy_random_walk(const xy_graph *g, int n_walkers, const int32_t *start /*host*/, int n_steps, uint64_t seed,
                    uint32_t sample_base, void *stream, int64_t *hist_host);
 
+/* xy_random_walk for callers that cannot allocate: the SAME kernel and the same results, but this entry point calls no
+ * cudaMalloc / cudaFree (nor any other allocating CUDA routine).  start_dev [S][n_walkers] int32 and hist_dev
+ * [S][n_steps+1] int64 are DEVICE buffers of the caller (on the graph's device); the 64-bit histogram the kernel's atomics
+ * accumulate into -- the buffer xy_random_walk allocates per call -- is a file-scope static __device__ array of
+ * XY_WALK_STATIC_ENTRIES (65536) 64-bit words = 512 KiB, which every GPU that loads the library holds until exit; its
+ * address is taken once per device with cudaGetSymbolAddress.  XY_EINVAL if S * (n_steps + 1) > XY_WALK_STATIC_ENTRIES
+ * (or a start site is out of range: the start sites are checked on the device).  The call clears the words it uses,
+ * runs the walk, copies them to hist_dev and synchronises `stream`.  ALL calls on a device share the one array, which
+ * keeps the last call's contents: calls that overlap on the GPU (two streams, two host threads) race -- serialise them. */
+#define XY_WALK_STATIC_ENTRIES 65536
+int xy_random_walk_static(const xy_graph *g, int n_walkers, const int32_t *start_dev /*device*/, int n_steps, uint64_t seed,
+                          uint32_t sample_base, void *stream, int64_t *hist_dev /*device*/);
+
 /* Device time in microseconds of the k_random_walk launch of the calling thread's last successful xy_random_walk call
  * (CUDA events around the kernel alone, on that call's stream: no allocation, no copy).  XY_ESTATE if there was none. */
 int xy_random_walk_kernel_us(double *us_out);

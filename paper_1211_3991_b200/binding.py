@@ -26,6 +26,7 @@ SYMBOLS = {
     "xy_read_fourier_accumulators": (C.c_int, [C.c_void_p, C.c_void_p]),
     "xy_random_walk": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_uint64, C.c_uint32, C.c_void_p, C.c_void_p]),
     "xy_random_walk_kernel_us": (C.c_int, [C.POINTER(C.c_double)]),
+    "xy_random_walk_static": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_uint64, C.c_uint32, C.c_void_p, C.c_void_p]),
     "xy_set_path": (C.c_int, [C.c_void_p, C.c_int]),
     "xy_get_path": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)]),
     "xy_get_schedule": (C.c_int, [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int64)]),
@@ -159,6 +160,15 @@ def xy_random_walk(g, start, n_steps, seed, sample_base=0, stream=None):
     hist = np.zeros((start.shape[0], n_steps + 1), np.int64)
     _check(lib().xy_random_walk(g, start.shape[1], sp, n_steps, seed, sample_base, stream, hist.ctypes.data_as(C.c_void_p)))
     return hist
+
+
+XY_WALK_STATIC_ENTRIES = 65536
+
+
+def xy_random_walk_static(g, n_walkers, start_dev, n_steps, seed, hist_dev, sample_base=0, stream=None):
+    """the walk without any allocation: start_dev / hist_dev = device addresses (int) of caller-owned buffers
+    [S][n_walkers] int32 and [S][n_steps+1] int64; S * (n_steps + 1) <= XY_WALK_STATIC_ENTRIES."""
+    _check(lib().xy_random_walk_static(g, n_walkers, start_dev, n_steps, seed, sample_base, stream, hist_dev))
 
 
 def xy_random_walk_kernel_us():

@@ -907,6 +907,67 @@ int xy_random_walk(const xy_graph *g, int n_walkers, const int32_t *start, int n
     return XY_OK;
 }
 
+// ---- xy_random_walk_static: the walk without any allocation (include/xy_b200.h) ----
+// scratch of the no-allocation entry point: the histogram words the kernel's atomics add to, plus one word that counts
+// invalid start sites.  A host-side stand-in in host code: its device address comes from cudaGetSymbolAddress.
+static __device__ __align__(256) unsigned long long g_walk_scratch[XY_WALK_STATIC_ENTRIES + 32];
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_walk_mutex;
+unsigned long long *g_walk_scratch_dev[kMaxDevices] = {};      // per device: the array's address there (set up once)
+
+__global__ void k_walk_check_starts(const int32_t *start, size_t n, int N, unsigned long long *bad) {
+    for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < n; i += static_cast<size_t>(gridDim.x) * blockDim.x)
+        if (start[i] < 0 || start[i] >= N) atomicAdd(bad, 1ull);
+}
+}  // namespace
+
+int xy_random_walk_static(const xy_graph *g, int n_walkers, const int32_t *start_dev, int n_steps, uint64_t seed,
+                          uint32_t sample_base, void *stream, int64_t *hist_dev) {
+    if (!g || !start_dev || !hist_dev) return fail(XY_EINVAL, "graph, start_dev or hist_dev is NULL");
+    DeviceGuard guard(g->device);
+    if (n_walkers < 1 || n_steps < 0 || n_steps > 12000) return fail(XY_EINVAL, "need n_walkers >= 1, 0 <= n_steps <= 12000");
+    if (static_cast<uint64_t>(sample_base) + g->S > 65536u) return fail(XY_EINVAL, "sample_base + S must be <= 65536");
+    const size_t nw = static_cast<size_t>(g->S) * n_walkers, nh = static_cast<size_t>(g->S) * (n_steps + 1);
+    if (nh > static_cast<size_t>(XY_WALK_STATIC_ENTRIES))
+        return fail(XY_EINVAL, "xy_random_walk_static: S * (n_steps + 1) = " + std::to_string(nh) + " exceeds the static scratch of " +
+                                   std::to_string(XY_WALK_STATIC_ENTRIES) + " words; use xy_random_walk");
+    if (g->device < 0 || g->device >= kMaxDevices) return fail(XY_EINVAL, "device index beyond 63");
+    unsigned long long *scratch = nullptr;
+    {   // set-up, once per device, with that device current (DeviceGuard above)
+        std::lock_guard<std::mutex> lock(g_walk_mutex);
+        if (!g_walk_scratch_dev[g->device]) {
+            void *p = nullptr;
+            const cudaError_t es = cudaGetSymbolAddress(&p, g_walk_scratch);
+            if (es != cudaSuccess || !p) return fail(XY_ECUDA, std::string("cudaGetSymbolAddress(g_walk_scratch): ") + cudaGetErrorString(es));
+            g_walk_scratch_dev[g->device] = static_cast<unsigned long long *>(p);
+        }
+        scratch = g_walk_scratch_dev[g->device];
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    unsigned long long *bad = scratch + XY_WALK_STATIC_ENTRIES;
+    // the array keeps the last call's contents: clear the words this call uses (and the error word)
+    XY_CUDA(cudaMemsetAsync(scratch, 0, nh * sizeof(unsigned long long), st));
+    XY_CUDA(cudaMemsetAsync(bad, 0, sizeof(unsigned long long), st));
+    k_walk_check_starts<<<std::max(1, std::min(g->n_sm * 4, ceil_div(static_cast<long long>(nw), 256))), 256, 0, st>>>(start_dev, nw, g->N, bad);
+    XY_CUDA(cudaGetLastError());
+    unsigned long long n_bad = 0;
+    XY_CUDA(cudaMemcpyAsync(&n_bad, bad, sizeof(n_bad), cudaMemcpyDeviceToHost, st));
+    XY_CUDA(cudaStreamSynchronize(st));
+    if (n_bad) return fail(XY_EINVAL, "start site out of range");
+    xy::WalkArgs a;
+    a.rec = g->rec; a.col_idx = g->col_idx; a.start = start_dev; a.hist = scratch;
+    a.N = g->N; a.n_walkers = n_walkers; a.n_steps = n_steps; a.sample_base = sample_base;
+    a.keys = xy::philox_key_schedule(static_cast<uint32_t>(seed), static_cast<uint32_t>(seed >> 32));
+    const dim3 grid(ceil_div(n_walkers, xy::kBlock), g->S);
+    xy::k_random_walk<<<grid, xy::kBlock, (n_steps + 1) * sizeof(unsigned int), st>>>(a);
+    XY_CUDA(cudaGetLastError());
+    XY_CUDA(cudaMemcpyAsync(hist_dev, scratch, nh * sizeof(int64_t), cudaMemcpyDeviceToDevice, st));
+    XY_CUDA(cudaStreamSynchronize(st));
+    return XY_OK;
+}
+
 int xy_random_walk_kernel_us(double *us_out) {
     if (!us_out) return fail(XY_EINVAL, "NULL output");
     if (g_walk_kernel_us < 0.0) return fail(XY_ESTATE, "no successful xy_random_walk call on this thread yet");
