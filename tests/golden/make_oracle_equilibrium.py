@@ -70,6 +70,7 @@ def main():
     ap.add_argument("--configs", type=int, nargs="+", default=[2, 4, 3])
     ap.add_argument("--workers", type=int, default=max(1, (os.cpu_count() or 2) - 2))
     ap.add_argument("--partial-dir", default="/tmp/xy_oracle_equilibrium")
+    ap.add_argument("--seeds", type=int, default=0, help="use only the first N chains of the plan (0 = all)")
     args = ap.parse_args()
     os.makedirs(args.partial_dir, exist_ok=True)
     import oracle as O
@@ -79,10 +80,12 @@ def main():
         futs = {}
         for cfg in args.configs:
             n_seeds, n_cycles, per_block = PLAN[cfg]
+            n_seeds = min(n_seeds, args.seeds) if args.seeds > 0 else n_seeds
             for k in range(n_seeds):
                 futs[(cfg, k)] = pool.submit(run_chain, cfg, k, n_cycles, per_block, args.partial_dir)
         for cfg in args.configs:
             n_seeds, n_cycles, per_block = PLAN[cfg]
+            n_seeds = min(n_seeds, args.seeds) if args.seeds > 0 else n_seeds
             w = workloads.CONFIGS[cfg]
             parts = [np.load(futs[(cfg, k)].result()) for k in range(n_seeds)]
             dst = os.path.join(HERE, f"oracle_equilibrium_cfg{cfg}.npz")
