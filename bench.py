@@ -312,6 +312,22 @@ def main():
                                 "whole launch; neither L2 nor HBM carries the gathers, the bound is the latency chain of a colour "
                                 "class (DESIGN.md 7.2) -- frac is the algorithmic bytes against the L2 bandwidth, for reference only")
 
+    # ---- what actually bounds k_phase: ISSUE SLOTS.  peak = 4 warp schedulers per SM x SMs x SM clock warp
+    #      instructions per second; the warp instructions per row (one row = 64 spin updates: 32 lanes x 2 slots) of the
+    #      Metropolis launch and of the over-relaxation + measurement launch are ncu counts of smsp__inst_executed.sum /
+    #      rows (profiles/r2a_full_warm.md, r2f_full_warm.md: G = 32; profiles/r2d_cfg2_full_warm.md: G = 16), constants of
+    #      the kernels as built, not of this run.  One PT-cycle step executes one row of each per 128 updates. ----
+    if ens.get_path(orps)[0] == 1 and w.R % 2 == 0 and w.R >= 32 and orps == 1:
+        inst_met, inst_orm = (238.8, 199.9) if w.R % 64 == 0 else (338.7, 428.4)
+        props = torch.cuda.get_device_properties(local_rank)
+        sm_ghz = (clocks["sm_mhz"] if clocks and clocks.get("sm_mhz") else 1965.0) * 1e-3
+        peak_inst = 4.0 * props.multi_processor_count * sm_ghz                      # G warp instructions / s
+        peak_upd = peak_inst / (inst_met + inst_orm) * 128.0                         # updates / ns of the full cycle
+        roofline["issue"] = {"bound": "alu", "achieved": value / world, "peak": peak_upd, "unit": UNIT, "frac": value / world / peak_upd,
+                             "peak_derivation": f"4 schedulers x {props.multi_processor_count} SMs x {sm_ghz:.3f} GHz = {peak_inst:.0f} G warp "
+                                                f"instructions/s; {inst_met} (Metropolis) + {inst_orm} (over-relaxation + measurement) warp "
+                                                "instructions per 128 updates (ncu, profiles/); applies to `value` (the full cycle)"}
+
     # ---- the genuinely streaming schedule: one launch per colour class over ALL samples (every sweep re-reads the whole
     #      state from HBM) -- the number "fraction of the HBM roofline" is literally about ----
     streaming = None
